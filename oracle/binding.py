@@ -1,0 +1,235 @@
+"""ctypes view of oracle/libafm_oracle*.so (TEST INFRASTRUCTURE, not the product).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+--impl reference legs may import this module.  It imports nothing from the
+CUDA package.  Argument marshalling only; all arithmetic is in afm_oracle.c.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+LAW_NONE, LAW_DMT, LAW_DMT_VISC, LAW_LJ_EXP = 0, 1, 2, 3
+
+
+class Model(C.Structure):
+    _fields_ = [("k", C.c_double), ("f0", C.c_double), ("Q", C.c_double),
+                ("f_drive", C.c_double), ("A0", C.c_double),
+                ("z_c", C.c_double), ("R", C.c_double), ("a0", C.c_double),
+                ("law", C.c_int32), ("n_theta", C.c_int32), ("S", C.c_int32),
+                ("n_cycles", C.c_int32), ("n_skip", C.c_int32),
+                ("pad_", C.c_int32)]
+
+
+class Consts(C.Structure):
+    _fields_ = [("w0", C.c_double), ("w", C.c_double), ("m", C.c_double),
+                ("c", C.c_double), ("r", C.c_double), ("F0", C.c_double),
+                ("dt", C.c_double), ("N", C.c_int64), ("W", C.c_int64)]
+
+
+class Box(C.Structure):
+    _fields_ = [("lo", C.c_double * 4), ("hi", C.c_double * 4),
+                ("log10", C.c_int32 * 4)]
+
+
+class Swarm(C.Structure):
+    _fields_ = [("n_particles", C.c_int32), ("n_iters", C.c_int32),
+                ("w", C.c_double), ("c1", C.c_double), ("c2", C.c_double)]
+
+
+_dp = C.POINTER(C.c_double)
+_libs = {}
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(_dp)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def lib(openmp=False):
+    """Load (building if stale) the single-threaded or the OpenMP oracle."""
+    key = bool(openmp)
+    if key not in _libs:
+        paths = _build.build()
+        L = C.CDLL(paths[1] if openmp else paths[0])
+        L.orc_constants.argtypes = [C.POINTER(Model), C.POINTER(Consts)]
+        L.orc_constants.restype = None
+        L.orc_force.argtypes = [C.POINTER(Model), _dp, C.c_double, C.c_double]
+        L.orc_force.restype = C.c_double
+        L.orc_rhs.argtypes = [C.POINTER(Model), _dp, C.c_double, C.c_double,
+                              C.c_double, _dp, _dp]
+        L.orc_rhs.restype = None
+        L.orc_rk4_step.argtypes = [C.POINTER(Model), _dp, C.c_double,
+                                   C.c_double, _dp, _dp]
+        L.orc_rk4_step.restype = None
+        L.orc_integrate.argtypes = [C.POINTER(Model), _dp, C.c_double,
+                                    C.c_double, _dp, _dp]
+        L.orc_integrate.restype = C.c_int
+        L.orc_window.argtypes = [C.POINTER(Model), _dp, C.c_double, C.c_double,
+                                 _dp]
+        L.orc_window.restype = C.c_int
+        L.orc_misfit.argtypes = [C.POINTER(Model), _dp, C.c_double, C.c_double,
+                                 _dp]
+        L.orc_misfit.restype = C.c_double
+        L.orc_forward_batch.argtypes = [C.POINTER(Model), _dp, C.c_int64, _dp,
+                                        C.c_int32, _dp, C.c_double, C.c_double,
+                                        _dp]
+        L.orc_forward_batch.restype = None
+        L.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint32),
+                                        C.POINTER(C.c_uint32),
+                                        C.POINTER(C.c_uint32)]
+        L.orc_philox4x32_10.restype = None
+        L.orc_pso_uniforms.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32,
+                                       C.c_uint32, C.c_int32, _dp, _dp]
+        L.orc_pso_uniforms.restype = None
+        L.orc_theta_of_x.argtypes = [C.POINTER(Box), C.c_int32, _dp, _dp]
+        L.orc_theta_of_x.restype = None
+        L.orc_pso_invert.argtypes = [C.POINTER(Model), C.POINTER(Box),
+                                     C.POINTER(Swarm), C.c_uint64, _dp,
+                                     C.c_int32, C.c_double, C.c_double, _dp,
+                                     _dp, _dp, _dp]
+        L.orc_pso_invert.restype = None
+        _libs[key] = L
+    return _libs[key]
+
+
+# ---- marshalling from the workload dictionaries (inputs module) ------------
+
+def model_from(wl, law=None, n_cycles=None, S=None, n_skip=None):
+    """Build a Model from a workload dict (see paper_1109_0334_b200.workloads)."""
+    c = wl["cantilever"]
+    return Model(k=c["k"], f0=c["f0"], Q=c["Q"], f_drive=c["f_drive"],
+                 A0=c["A0"], z_c=c["z_c"], R=c["R"], a0=c["a0"],
+                 law=wl["law"] if law is None else law,
+                 n_theta=wl["n_params"],
+                 S=wl["steps_per_cycle"] if S is None else S,
+                 n_cycles=wl["n_cycles"] if n_cycles is None else n_cycles,
+                 n_skip=wl["n_skip_cycles"] if n_skip is None else n_skip,
+                 pad_=0)
+
+
+def box_from(wl):
+    b = Box()
+    for j in range(wl["n_params"]):
+        b.lo[j] = wl["bounds"]["lo"][j]
+        b.hi[j] = wl["bounds"]["hi"][j]
+        b.log10[j] = int(wl["bounds"]["log10"][j])
+    return b
+
+
+def swarm_from(wl, n_particles=None, n_iters=None):
+    s = wl["swarm"]
+    return Swarm(n_particles=s["n_particles"] if n_particles is None else n_particles,
+                 n_iters=s["n_iters"] if n_iters is None else n_iters,
+                 w=s["w"], c1=s["c1"], c2=s["c2"])
+
+
+# ---- thin calls -------------------------------------------------------------
+
+def constants(M):
+    c = Consts()
+    lib().orc_constants(C.byref(M), C.byref(c))
+    return c
+
+
+def force(M, theta, d, v=0.0):
+    th = _f64(theta)
+    return lib().orc_force(C.byref(M), _ptr(th), float(d), float(v))
+
+
+def rhs(M, theta, t, z, v):
+    th = _f64(theta)
+    dz, dv = C.c_double(), C.c_double()
+    lib().orc_rhs(C.byref(M), _ptr(th), t, z, v, C.byref(dz), C.byref(dv))
+    return dz.value, dv.value
+
+
+def rk4_step(M, theta, t, dt, z, v):
+    th = _f64(theta)
+    zz, vv = C.c_double(z), C.c_double(v)
+    lib().orc_rk4_step(C.byref(M), _ptr(th), t, dt, C.byref(zz), C.byref(vv))
+    return zz.value, vv.value
+
+
+def integrate(M, theta, z0, v0):
+    """Full trajectory: (diverged, zs[N+1], vs[N+1])."""
+    th = _f64(theta)
+    N = constants(M).N
+    zs = np.empty(N + 1)
+    vs = np.empty(N + 1)
+    bad = lib().orc_integrate(C.byref(M), _ptr(th), z0, v0, _ptr(zs), _ptr(vs))
+    return bad, zs, vs
+
+
+def window(M, theta, z0, v0):
+    th = _f64(theta)
+    w = np.empty(constants(M).W)
+    bad = lib().orc_window(C.byref(M), _ptr(th), z0, v0, _ptr(w))
+    return bad, w
+
+
+def misfit(M, theta, z0, v0, trace):
+    th, tr = _f64(theta), _f64(trace)
+    assert tr.size == constants(M).W
+    return lib().orc_misfit(C.byref(M), _ptr(th), z0, v0, _ptr(tr))
+
+
+def forward_batch(M, params, trace, z0v0=None, z0=0.0, v0=0.0, n_traces=1,
+                  openmp=False):
+    params = _f64(params)
+    P = params.shape[0]
+    assert params.shape[1] == M.n_theta and P % n_traces == 0
+    tr = _f64(trace)
+    assert tr.size == n_traces * constants(M).W
+    zv = None if z0v0 is None else _f64(z0v0)
+    out = np.empty(P)
+    lib(openmp).orc_forward_batch(C.byref(M), _ptr(params), P, _ptr(tr),
+                                  n_traces, _ptr(zv), z0, v0, _ptr(out))
+    return out
+
+
+def philox4x32_10(ctr, key):
+    c = (C.c_uint32 * 4)(*[int(x) for x in ctr])
+    k = (C.c_uint32 * 2)(*[int(x) for x in key])
+    o = (C.c_uint32 * 4)()
+    lib().orc_philox4x32_10(c, k, o)
+    return [int(x) for x in o]
+
+
+def pso_uniforms(seed, gp, it, purpose, D):
+    a = np.zeros(4)
+    b = np.zeros(4)
+    lib().orc_pso_uniforms(seed, gp, it, purpose, D, _ptr(a), _ptr(b))
+    return a[:D].copy(), b[:D].copy()
+
+
+def theta_of_x(B, D, x):
+    x = _f64(x)
+    th = np.empty(D)
+    lib().orc_theta_of_x(C.byref(B), D, _ptr(x), _ptr(th))
+    return th
+
+
+def pso_invert(M, B, Sw, seed, trace, z0, v0, n_traces=1, dump=False,
+               openmp=False):
+    """Returns dict(theta_star [T][D], J_star [T], dump [it][PT][3D+2] or None,
+    gbest_hist [it][T][D+1])."""
+    D = M.n_theta
+    PT = Sw.n_particles * n_traces
+    tr = _f64(trace)
+    assert tr.size == n_traces * constants(M).W
+    th = np.empty((n_traces, D))
+    Js = np.empty(n_traces)
+    dmp = np.empty((Sw.n_iters, PT, 3 * D + 2)) if dump else None
+    gh = np.empty((Sw.n_iters, n_traces, D + 1))
+    lib(openmp).orc_pso_invert(C.byref(M), C.byref(B), C.byref(Sw), seed,
+                               _ptr(tr), n_traces, z0, v0, _ptr(th), _ptr(Js),
+                               _ptr(dmp), _ptr(gh))
+    return dict(theta_star=th, J_star=Js, dump=dmp, gbest_hist=gh)
