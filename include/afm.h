@@ -1,0 +1,219 @@
+/*
+ * afm.h -- C ABI of the B200-native dAFM force-inversion hot path
+ * (arxiv/paper_1109_0334, Busch, Zou, Ganapathysubramanian).
+ *
+ * The library computes, entirely in hand-written sm_100a CUDA kernels:
+ *   - the batched forward problem FP: for every candidate
+ *     force-parameter vector theta, integrate
+ *         m z'' + (m w0/Q) z' + k z = F0 cos(w t) + F_ts(z + z_c, z'; theta)
+ *     (the m = 1 case of the modal equation, Eq. 2, as the
+ *     point mass BASELINE.json:north_star names) with the explicit classical
+ *     4th-order Runge-Kutta scheme at a fixed step of 1/S of a
+ *     drive period;
+ *   - the cost functional of Eq. 5 as the plain sum of squares
+ *         J = sum_{n=N-W+1..N} (z_n - U_{n-(N-W)-1})^2        [m^2]
+ *     over the last W post-step states (readings R5, R7);
+ *   - the particle-swarm optimisation of PAPER.md:209-214 (velocity update
+ *     Eq. 8, personal best, global best) that solves the inverse problem IP
+ *      as an unconstrained minimisation of J over theta.
+ *
+ * Conventions
+ *   - Every entry point returns AFM_OK (0) or a negative afm_status; the text
+ *     of the last error on the calling thread is afm_last_error().  Nothing
+ *     throws, nothing is allocated on behalf of the caller, every buffer is
+ *     caller-owned.  The library keeps one lazily created device workspace
+ *     per process (time-tile stream, swarm state); afm_shutdown() frees it.
+ *   - There is NO CPU fallback: without a CUDA device of compute capability
+ *     10.x the compute calls return AFM_EUNSUPPORTED / AFM_ECUDA.
+ *   - "device" pointers are CUDA device pointers valid on the current device;
+ *     "host" pointers are ordinary host memory.  All arrays are dense,
+ *     row-major, FP64, SI units at the ABI, whatever cfg->precision says: the
+ *     FP32 kernel converts internally.
+ *   - cuda_stream is a cudaStream_t passed as void* (NULL = legacy default
+ *     stream).  PyTorch is only ever the allocator and the stream provider.
+ */
+#ifndef AFM_H
+#define AFM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  AFM_OK = 0,
+  AFM_EINVAL = -1,       /* NULL pointer, bad size, law/D mismatch, ...        */
+  AFM_ECUDA = -2,        /* a CUDA runtime call failed; see afm_last_error()   */
+  AFM_EUNSUPPORTED = -3  /* no sm_100-class device, or an unsupported option   */
+} afm_status;
+
+/* Tip-sample force laws F_ts(d, d'; theta), d = z + z_c the tip-sample gap
+ * (BASELINE.json configs[0], [2], [3]; "Hertzian contact and Van der Waals
+ * forces").
+ *   AFM_LAW_NONE      F_ts = 0                                   D = 0..4
+ *   AFM_LAW_DMT       theta = (H, E*)                            D = 2
+ *       d >  a0:  -H R / (6 d^2)
+ *       d <= a0:  -H R / (6 a0^2) + (4/3) E* sqrt(R) (a0 - d)^{3/2}
+ *   AFM_LAW_DMT_VISC  theta = (H, E*, eta)                       D = 3
+ *       DMT, plus  -eta sqrt(R (a0 - d)) d'  for d <= a0
+ *   AFM_LAW_LJ_EXP    theta = (C_rep, C_att, F_ad, lambda)       D = 4
+ *       C_rep / d^8 - C_att / d^2 - F_ad exp(-d / lambda)
+ */
+typedef enum {
+  AFM_LAW_NONE = 0,
+  AFM_LAW_DMT = 1,
+  AFM_LAW_DMT_VISC = 2,
+  AFM_LAW_LJ_EXP = 3
+} afm_law;
+
+typedef enum { AFM_F64 = 0, AFM_F32 = 1 } afm_precision;
+
+/* Cantilever, drive, time grid.  Host, read-only, plain POD.
+ * F0 is fixed by A0: F0 = k A0 sqrt((1-r^2)^2 + (r/Q)^2), r = f_drive/f0, so
+ * that the free (F_ts = 0) steady-state amplitude is exactly A0.
+ * dt = 1 / (f_drive * steps_per_cycle); t_n = n dt; N = steps_per_cycle *
+ * n_cycles steps are taken; the misfit window is the last
+ * W = steps_per_cycle * (n_cycles - n_skip_cycles) post-step states.
+ * A trajectory whose state becomes non-finite or leaves |z| <= 100 A0 at any
+ * step is "diverged" and its misfit is +Inf (reading R12). */
+typedef struct {
+  double k;        /* spring constant, N/m                                  */
+  double f0;       /* natural frequency, Hz                                 */
+  double Q;        /* quality factor                                        */
+  double f_drive;  /* drive frequency, Hz                                   */
+  double A0;       /* free steady-state amplitude, m                        */
+  double z_c;      /* rest height of the tip above the sample, m            */
+  double R;        /* tip radius, m (DMT laws)                              */
+  double a0;       /* intermolecular distance, m (DMT laws)                 */
+  double z0, v0;   /* initial state used when z0v0 == NULL (m, m/s)         */
+  int32_t law;             /* afm_law                                       */
+  int32_t n_params;        /* D, must match the law (NONE: any 0..4)        */
+  int32_t steps_per_cycle; /* S >= 1                                        */
+  int32_t n_cycles;        /* >= 1                                          */
+  int32_t n_skip_cycles;   /* 0 <= n_skip_cycles < n_cycles                 */
+  int32_t n_traces;        /* >= 1: the particles are n_traces equal,
+                              contiguous segments; segment s is compared
+                              with trace[s][0..W)                           */
+  int32_t precision;       /* afm_precision of the integrate kernel         */
+  int32_t reserved_;       /* must be 0                                     */
+} afm_cfg;
+
+/* Search box in PSO coordinates x; theta_j = 10^x_j where log10_scale[j] != 0,
+ * else theta_j = x_j.  Entries j >= D are ignored. */
+typedef struct {
+  double lo[4];
+  double hi[4];
+  int32_t log10_scale[4];
+} afm_bounds;
+
+/* Swarm: n_particles PER TRACE; n_iters forward batches (iteration 0
+ * evaluates the initial positions; the result is the global best after the
+ * last batch).  w, c1, c2 are the weights of Eq. 8.
+ * j_target > 0 enables the paper's cutoff rule: the run
+ * ends after the first batch at which every trace's global best J is
+ * <= j_target; <= 0 disables it. */
+typedef struct {
+  int32_t n_particles;
+  int32_t n_iters;
+  double w, c1, c2;
+  double j_target;
+} afm_swarm_cfg;
+
+/* ---- forward problem + cost (Eq. 5) -------------
+ * misfit[p] = J(theta_p) for p in [0, n_particles).
+ *   params   device  [n_particles][D]   physical SI parameters
+ *   trace    device  [n_traces][W]      measured deflection U, metres
+ *   z0v0     device  [n_particles][2]   per-particle (z0, v0), or NULL ->
+ *                                       (cfg->z0, cfg->v0) for all
+ *   misfit   device  [n_particles]      out, m^2; +Inf if diverged
+ * n_particles must be a positive multiple of cfg->n_traces.
+ * Asynchronous on cuda_stream: returns after enqueueing. */
+int afm_forward_batch(const double* params, int64_t n_particles,
+                      const double* trace, const afm_cfg* cfg,
+                      const double* z0v0, double* misfit, void* cuda_stream);
+
+/* Same computation with HOST buffers: copies params/trace/z0v0 to the device,
+ * runs the batch, copies misfit back and synchronises the stream before
+ * returning (the end-to-end path bench.py times).  All pointers host. */
+int afm_forward_batch_host(const double* params, int64_t n_particles,
+                           const double* trace, const afm_cfg* cfg,
+                           const double* z0v0, double* misfit,
+                           void* cuda_stream);
+
+/* ---- inverse problem by PSO (Eq. 8) -------------
+ * One independent swarm per trace.  Philox4x32-10 random numbers, key =
+ * seed, counter = (particle, iteration, purpose) (reading R11), so
+ * a run is a pure function of its arguments.
+ *   bounds, swarm, cfg  host
+ *   trace       device [n_traces][W]
+ *   theta_star  host   [n_traces][D]   out: physical parameters of the best
+ *   J_star      host   [n_traces]      out: its misfit
+ *   swarm_dump  device [n_iters][n_traces*n_particles][3D+2] or NULL:
+ *               per iteration and particle (x[D], v[D], pbest[D], J, pbestJ)
+ *               after the personal-best update and before the move
+ *   gbest_hist  device [n_iters][n_traces][D+1] or NULL: (gbest x[D], gbestJ)
+ *   n_iters_done host  int32 or NULL: batches actually run (j_target)
+ * Synchronous: returns when the host outputs are valid. */
+int afm_pso_invert(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                   uint64_t seed, const double* trace, const afm_cfg* cfg,
+                   double* theta_star, double* J_star, double* swarm_dump,
+                   double* gbest_hist, int32_t* n_iters_done,
+                   void* cuda_stream);
+
+/* Same inversion with the trace in HOST memory (copied inside the call). */
+int afm_pso_invert_host(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                        uint64_t seed, const double* trace, const afm_cfg* cfg,
+                        double* theta_star, double* J_star,
+                        int32_t* n_iters_done, void* cuda_stream);
+
+/* One PSO move applied to caller-held swarm state (the a5-a7 steps of
+ * SURVEY.md 8(a) on their own, for tests and for callers that supply their
+ * own misfits): personal-best update from J, global best per trace, then
+ * Eq. 8 + position update + bound rule.  All device, FP64:
+ *   x, v, pbest [PT][D]; J, pbestJ [PT]; gbest [n_traces][D];
+ *   gbestJ [n_traces]; PT = n_traces * swarm->n_particles.
+ * do_move == 0 stops after the best updates.  Asynchronous. */
+int afm_pso_step(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                 int32_t n_dims, int32_t n_traces, uint64_t seed,
+                 int32_t iteration, int32_t do_move, const double* J,
+                 double* x, double* v, double* pbest, double* pbestJ,
+                 double* gbest, double* gbestJ, void* cuda_stream);
+
+/* Initial swarm (uniform positions and velocities in the box):
+ * fills x, v, pbest [PT][D] and sets pbestJ [PT], gbestJ [n_traces] to +Inf,
+ * gbest [n_traces][D] to the first particle of each trace.  Asynchronous. */
+int afm_pso_init(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                 int32_t n_dims, int32_t n_traces, uint64_t seed, double* x,
+                 double* v, double* pbest, double* pbestJ, double* gbest,
+                 double* gbestJ, void* cuda_stream);
+
+/* Philox4x32-10 on the device for n counters (tests: known answers).
+ *   ctr device [n][4] uint32, key host [2], out device [n][4].  Async. */
+int afm_philox4x32_10(const uint32_t* ctr, int64_t n, const uint32_t* key,
+                      uint32_t* out, void* cuda_stream);
+
+/* Trajectory of ONE particle through the same device step routine the batch
+ * kernel uses (tests and diagnostics only): zs, vs device [N+1] or NULL;
+ * index 0 is the initial state.  theta host [D].  Asynchronous. */
+int afm_trajectory(const double* theta, const afm_cfg* cfg, double z0,
+                   double v0, double* zs, double* vs, void* cuda_stream);
+
+/* Kernel launches enqueued by this library on the calling thread since the
+ * last reset (bench.py's gpu_launches). */
+int64_t afm_launch_count(void);
+void afm_reset_launch_count(void);
+
+/* Tuning knobs (optional).  name: "block" (threads per CTA of the integrate
+ * kernel: 32, 64 or 128; 0 = auto), "tile" (steps per time tile; 0 = auto).
+ * Returns AFM_EINVAL for an unknown name or value. */
+int afm_set_option(const char* name, int64_t value);
+
+const char* afm_last_error(void);
+const char* afm_version(void);
+void afm_shutdown(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AFM_H */

@@ -1,0 +1,343 @@
+"""Thin ctypes binding of libafm_b200.so (include/afm.h).
+
+Argument marshalling only: every step of the hot path runs in the library's
+CUDA kernels.  PyTorch appears here as the owner of device memory and of the
+CUDA stream, nothing else.  There is no CPU fallback: loading fails loudly if
+the library has not been built (`python -m paper_1109_0334_b200.build`), and
+every compute call raises AfmError when no sm_100 device is present.
+
+Function names and argument order follow include/afm.h.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libafm_b200.so")
+
+LAW_NONE, LAW_DMT, LAW_DMT_VISC, LAW_LJ_EXP = 0, 1, 2, 3
+F64, F32 = 0, 1
+OK, EINVAL, ECUDA, EUNSUPPORTED = 0, -1, -2, -3
+
+# every symbol include/afm.h declares (tests check the library exports them all)
+SYMBOLS = (
+    "afm_forward_batch", "afm_forward_batch_host", "afm_pso_invert",
+    "afm_pso_invert_host", "afm_pso_step", "afm_pso_init",
+    "afm_philox4x32_10", "afm_trajectory", "afm_launch_count",
+    "afm_reset_launch_count", "afm_set_option", "afm_last_error",
+    "afm_version", "afm_shutdown",
+)
+
+
+class AfmError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("afm error %d: %s" % (code, msg))
+        self.code = code
+
+
+class Cfg(C.Structure):
+    _fields_ = [("k", C.c_double), ("f0", C.c_double), ("Q", C.c_double),
+                ("f_drive", C.c_double), ("A0", C.c_double),
+                ("z_c", C.c_double), ("R", C.c_double), ("a0", C.c_double),
+                ("z0", C.c_double), ("v0", C.c_double),
+                ("law", C.c_int32), ("n_params", C.c_int32),
+                ("steps_per_cycle", C.c_int32), ("n_cycles", C.c_int32),
+                ("n_skip_cycles", C.c_int32), ("n_traces", C.c_int32),
+                ("precision", C.c_int32), ("reserved_", C.c_int32)]
+
+    @property
+    def n_steps(self):
+        return self.steps_per_cycle * self.n_cycles
+
+    @property
+    def n_window(self):
+        return self.steps_per_cycle * (self.n_cycles - self.n_skip_cycles)
+
+
+class Bounds(C.Structure):
+    _fields_ = [("lo", C.c_double * 4), ("hi", C.c_double * 4),
+                ("log10_scale", C.c_int32 * 4)]
+
+
+class SwarmCfg(C.Structure):
+    _fields_ = [("n_particles", C.c_int32), ("n_iters", C.c_int32),
+                ("w", C.c_double), ("c1", C.c_double), ("c2", C.c_double),
+                ("j_target", C.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    """The loaded library; raises if it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(
+                "%s is missing: build it with `python -m paper_1109_0334_b200.build` "
+                "(there is no CPU fallback)" % LIB_PATH)
+        L = C.CDLL(LIB_PATH)
+        vp, dp, i32, i64, u64 = C.c_void_p, C.c_void_p, C.c_int32, C.c_int64, C.c_uint64
+        L.afm_forward_batch.argtypes = [dp, i64, dp, C.POINTER(Cfg), dp, dp, vp]
+        L.afm_forward_batch_host.argtypes = [dp, i64, dp, C.POINTER(Cfg), dp, dp, vp]
+        L.afm_pso_invert.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), u64, dp,
+                                     C.POINTER(Cfg), dp, dp, dp, dp,
+                                     C.POINTER(i32), vp]
+        L.afm_pso_invert_host.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), u64,
+                                          dp, C.POINTER(Cfg), dp, dp,
+                                          C.POINTER(i32), vp]
+        L.afm_pso_step.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), i32, i32,
+                                   u64, i32, i32, dp, dp, dp, dp, dp, dp, dp, vp]
+        L.afm_pso_init.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), i32, i32,
+                                   u64, dp, dp, dp, dp, dp, dp, vp]
+        L.afm_philox4x32_10.argtypes = [dp, i64, C.POINTER(C.c_uint32), dp, vp]
+        L.afm_trajectory.argtypes = [dp, C.POINTER(Cfg), C.c_double, C.c_double,
+                                     dp, dp, vp]
+        for name in ("afm_forward_batch", "afm_forward_batch_host", "afm_pso_invert",
+                     "afm_pso_invert_host", "afm_pso_step", "afm_pso_init",
+                     "afm_philox4x32_10", "afm_trajectory"):
+            getattr(L, name).restype = C.c_int
+        L.afm_launch_count.restype = i64
+        L.afm_launch_count.argtypes = []
+        L.afm_reset_launch_count.restype = None
+        L.afm_set_option.argtypes = [C.c_char_p, i64]
+        L.afm_set_option.restype = C.c_int
+        L.afm_last_error.restype = C.c_char_p
+        L.afm_version.restype = C.c_char_p
+        L.afm_shutdown.restype = None
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        raise AfmError(rc, lib().afm_last_error().decode("utf-8", "replace"))
+
+
+# ---- marshalling from the workload dictionaries ------------------------------
+
+def cfg_from(wl, precision=F64, **over):
+    """afm_cfg from a paper_1109_0334_b200.workloads dict."""
+    c = wl["cantilever"]
+    cfg = Cfg(k=c["k"], f0=c["f0"], Q=c["Q"], f_drive=c["f_drive"], A0=c["A0"],
+              z_c=c["z_c"], R=c["R"], a0=c["a0"], z0=wl["z0"], v0=wl["v0"],
+              law=wl["law"], n_params=wl["n_params"],
+              steps_per_cycle=wl["steps_per_cycle"], n_cycles=wl["n_cycles"],
+              n_skip_cycles=wl["n_skip_cycles"], n_traces=wl["n_traces"],
+              precision=precision, reserved_=0)
+    for k, v in over.items():
+        setattr(cfg, k, v)
+    return cfg
+
+
+def bounds_from(wl):
+    b = Bounds()
+    for j in range(wl["n_params"]):
+        b.lo[j] = wl["bounds"]["lo"][j]
+        b.hi[j] = wl["bounds"]["hi"][j]
+        b.log10_scale[j] = int(wl["bounds"]["log10"][j])
+    return b
+
+
+def swarm_from(wl, j_target=0.0, **over):
+    s = wl["swarm"]
+    sc = SwarmCfg(n_particles=s["n_particles"], n_iters=s["n_iters"], w=s["w"],
+                  c1=s["c1"], c2=s["c2"], j_target=j_target)
+    for k, v in over.items():
+        setattr(sc, k, v)
+    return sc
+
+
+# ---- device-buffer helpers (torch = allocator + stream) ---------------------
+
+def _torch():
+    import torch
+    return torch
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        return _torch().cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+def _dev_f64(t, name):
+    torch = _torch()
+    if not isinstance(t, torch.Tensor):
+        t = torch.as_tensor(np.ascontiguousarray(t, dtype=np.float64), device="cuda")
+    if not t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
+        raise TypeError("%s must be a contiguous CUDA float64 tensor" % name)
+    return t
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _host_f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _hptr(a):
+    return None if a is None else C.c_void_p(a.ctypes.data)
+
+
+# ---- the calls of include/afm.h -------------------------------------------------
+
+def afm_forward_batch(params, trace, cfg, z0v0=None, misfit=None, stream=None):
+    """misfit[p] = J(theta_p) (device tensors in, device tensor out; async)."""
+    torch = _torch()
+    params = _dev_f64(params, "params")
+    trace = _dev_f64(trace, "trace")
+    P = params.shape[0]
+    if params.numel() != P * max(cfg.n_params, 0) and cfg.n_params > 0:
+        raise ValueError("params must be [P][D]")
+    if trace.numel() != cfg.n_traces * cfg.n_window:
+        raise ValueError("trace must hold n_traces * W = %d samples"
+                         % (cfg.n_traces * cfg.n_window))
+    if z0v0 is not None:
+        z0v0 = _dev_f64(z0v0, "z0v0")
+        if z0v0.numel() != 2 * P:
+            raise ValueError("z0v0 must be [P][2]")
+    if misfit is None:
+        misfit = torch.empty(P, dtype=torch.float64, device=params.device)
+    else:
+        misfit = _dev_f64(misfit, "misfit")
+    _check(lib().afm_forward_batch(_ptr(params), P, _ptr(trace), C.byref(cfg),
+                                   _ptr(z0v0), _ptr(misfit), _stream_ptr(stream)))
+    return misfit
+
+
+def afm_forward_batch_host(params, trace, cfg, z0v0=None, misfit=None, stream=None):
+    """Same with host (numpy) buffers; copies inside the call; synchronous."""
+    params = _host_f64(params)
+    trace = _host_f64(trace)
+    P = params.shape[0]
+    if trace.size != cfg.n_traces * cfg.n_window:
+        raise ValueError("trace must hold n_traces * W samples")
+    z0v0 = None if z0v0 is None else _host_f64(z0v0)
+    if misfit is None:
+        misfit = np.empty(P, dtype=np.float64)
+    _check(lib().afm_forward_batch_host(_hptr(params), P, _hptr(trace), C.byref(cfg),
+                                        _hptr(z0v0), _hptr(misfit),
+                                        _stream_ptr(stream)))
+    return misfit
+
+
+def afm_pso_invert(bounds, swarm, seed, trace, cfg, dump=False, hist=False,
+                   stream=None):
+    """Returns dict(theta_star [T][D], J_star [T], n_iters_done, dump, gbest_hist);
+    dump / gbest_hist are device tensors or None."""
+    torch = _torch()
+    trace = _dev_f64(trace, "trace")
+    if trace.numel() != cfg.n_traces * cfg.n_window:
+        raise ValueError("trace must hold n_traces * W samples")
+    D, T = cfg.n_params, cfg.n_traces
+    PT = swarm.n_particles * T
+    th = np.empty((T, D), dtype=np.float64)
+    Js = np.empty(T, dtype=np.float64)
+    dmp = (torch.empty((swarm.n_iters, PT, 3 * D + 2), dtype=torch.float64,
+                       device=trace.device) if dump else None)
+    gh = (torch.empty((swarm.n_iters, T, D + 1), dtype=torch.float64,
+                      device=trace.device) if hist else None)
+    done = C.c_int32(0)
+    _check(lib().afm_pso_invert(C.byref(bounds), C.byref(swarm), int(seed),
+                                _ptr(trace), C.byref(cfg), _hptr(th), _hptr(Js),
+                                _ptr(dmp), _ptr(gh), C.byref(done),
+                                _stream_ptr(stream)))
+    return dict(theta_star=th, J_star=Js, n_iters_done=done.value, dump=dmp,
+                gbest_hist=gh)
+
+
+def afm_pso_invert_host(bounds, swarm, seed, trace, cfg, stream=None):
+    trace = _host_f64(trace)
+    if trace.size != cfg.n_traces * cfg.n_window:
+        raise ValueError("trace must hold n_traces * W samples")
+    D, T = cfg.n_params, cfg.n_traces
+    th = np.empty((T, D), dtype=np.float64)
+    Js = np.empty(T, dtype=np.float64)
+    done = C.c_int32(0)
+    _check(lib().afm_pso_invert_host(C.byref(bounds), C.byref(swarm), int(seed),
+                                     _hptr(trace), C.byref(cfg), _hptr(th),
+                                     _hptr(Js), C.byref(done), _stream_ptr(stream)))
+    return dict(theta_star=th, J_star=Js, n_iters_done=done.value)
+
+
+def afm_pso_init(bounds, swarm, n_dims, n_traces, seed, stream=None):
+    """Allocates and fills the swarm state; returns a dict of device tensors."""
+    torch = _torch()
+    PT = swarm.n_particles * n_traces
+    kw = dict(dtype=torch.float64, device="cuda")
+    st = dict(x=torch.empty((PT, n_dims), **kw), v=torch.empty((PT, n_dims), **kw),
+              pbest=torch.empty((PT, n_dims), **kw), pbestJ=torch.empty(PT, **kw),
+              gbest=torch.empty((n_traces, n_dims), **kw),
+              gbestJ=torch.empty(n_traces, **kw))
+    _check(lib().afm_pso_init(C.byref(bounds), C.byref(swarm), n_dims, n_traces,
+                              int(seed), _ptr(st["x"]), _ptr(st["v"]),
+                              _ptr(st["pbest"]), _ptr(st["pbestJ"]),
+                              _ptr(st["gbest"]), _ptr(st["gbestJ"]),
+                              _stream_ptr(stream)))
+    return st
+
+
+def afm_pso_step(bounds, swarm, n_dims, n_traces, seed, iteration, do_move, J, st,
+                 stream=None):
+    J = _dev_f64(J, "J")
+    _check(lib().afm_pso_step(C.byref(bounds), C.byref(swarm), n_dims, n_traces,
+                              int(seed), int(iteration), int(bool(do_move)), _ptr(J),
+                              _ptr(st["x"]), _ptr(st["v"]), _ptr(st["pbest"]),
+                              _ptr(st["pbestJ"]), _ptr(st["gbest"]),
+                              _ptr(st["gbestJ"]), _stream_ptr(stream)))
+    return st
+
+
+def afm_philox4x32_10(ctr, key, stream=None):
+    """ctr [n][4] uint32 (numpy) -> [n][4] uint32 (numpy), computed on the device."""
+    torch = _torch()
+    ctr = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
+    n = ctr.shape[0]
+    d_in = torch.as_tensor(ctr.view(np.int32), device="cuda")
+    d_out = torch.empty_like(d_in)
+    k = (C.c_uint32 * 2)(int(key[0]), int(key[1]))
+    _check(lib().afm_philox4x32_10(_ptr(d_in), n, k, _ptr(d_out), _stream_ptr(stream)))
+    return d_out.cpu().numpy().view(np.uint32)
+
+
+def afm_trajectory(theta, cfg, z0, v0, stream=None):
+    """(zs[N+1], vs[N+1]) of one particle, as numpy arrays."""
+    torch = _torch()
+    theta = _host_f64(theta)
+    N = cfg.n_steps
+    zs = torch.empty(N + 1, dtype=torch.float64, device="cuda")
+    vs = torch.empty(N + 1, dtype=torch.float64, device="cuda")
+    _check(lib().afm_trajectory(_hptr(theta), C.byref(cfg), float(z0), float(v0),
+                                _ptr(zs), _ptr(vs), _stream_ptr(stream)))
+    torch.cuda.synchronize()
+    return zs.cpu().numpy(), vs.cpu().numpy()
+
+
+def afm_launch_count():
+    return int(lib().afm_launch_count())
+
+
+def afm_reset_launch_count():
+    lib().afm_reset_launch_count()
+
+
+def afm_set_option(name, value):
+    _check(lib().afm_set_option(name.encode(), int(value)))
+
+
+def afm_last_error():
+    return lib().afm_last_error().decode("utf-8", "replace")
+
+
+def afm_version():
+    return lib().afm_version().decode()
+
+
+def afm_shutdown():
+    lib().afm_shutdown()

@@ -1,0 +1,622 @@
+// afm_api.cu -- the C ABI of include/afm.h: argument validation, the scaled
+// model constants, the device workspace and the launch sequences.  No
+// arithmetic of the method runs here beyond the handful of scalar constants in
+// make_consts(); every step of the hot path is a kernel in afm_kernels.cu.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <mutex>
+
+#include "afm_internal.h"
+
+#ifndef M_PI
+#define M_PI 3.14159265358979323846
+#endif
+
+namespace {
+
+using namespace afm;
+
+thread_local char g_err[512] = "";
+thread_local int64_t g_launches = 0;
+
+int fail(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+#define CUDA_TRY(expr)                                                        \
+  do {                                                                        \
+    cudaError_t e_ = (expr);                                                  \
+    if (e_ != cudaSuccess)                                                    \
+      return fail(AFM_ECUDA, "%s failed: %s (%s:%d)", #expr,                  \
+                  cudaGetErrorString(e_), __FILE__, __LINE__);                \
+  } while (0)
+
+#define LAUNCHED(call)                                                        \
+  do {                                                                        \
+    int n_ = (call);                                                          \
+    if (n_ < 0) return fail(AFM_EINVAL, "no kernel for this law (%s)", #call);\
+    g_launches += n_;                                                         \
+    cudaError_t e_ = cudaGetLastError();                                      \
+    if (e_ != cudaSuccess)                                                    \
+      return fail(AFM_ECUDA, "launch %s failed: %s", #call,                   \
+                  cudaGetErrorString(e_));                                    \
+  } while (0)
+
+// ---- options -----------------------------------------------------------------
+int g_opt_block = 0;  // 0 = auto
+int g_opt_tile = 0;   // 0 = auto
+
+// ---- grow-only device workspace ------------------------------------------------
+struct Buffer {
+  void* p = nullptr;
+  size_t cap = 0;
+  int ensure(size_t bytes) {
+    if (bytes <= cap) return 0;
+    if (p) cudaFree(p);
+    p = nullptr;
+    cap = 0;
+    // round up so that slightly larger follow-up calls reuse the allocation
+    size_t want = (bytes + (size_t)(1 << 20) - 1) & ~((size_t)(1 << 20) - 1);
+    cudaError_t e = cudaMalloc(&p, want);
+    if (e != cudaSuccess) {
+      p = nullptr;
+      return -1;
+    }
+    cap = want;
+    return 0;
+  }
+  void release() {
+    if (p) cudaFree(p);
+    p = nullptr;
+    cap = 0;
+  }
+};
+
+struct Workspace {
+  std::mutex mu;
+  Buffer stream;                       // time-tile stream
+  Buffer swarm;                        // x, v, pbest, J, pbestJ, gbest, ...
+  Buffer cand;                         // block candidates
+  Buffer h_params, h_trace, h_z0v0, h_misfit;  // staging for the *_host calls
+  Buffer scratch;                      // theta for afm_trajectory
+  cudaEvent_t last_use = nullptr;      // orders reuse across streams
+  cudaStream_t last_stream = nullptr;
+  bool checked_device = false;
+  void* pinned = nullptr;              // small pinned host block
+  size_t pinned_cap = 0;
+} g_ws;
+
+int check_device() {
+  if (g_ws.checked_device) return AFM_OK;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess)
+    return fail(AFM_ECUDA, "no CUDA device: %s", cudaGetErrorString(e));
+  cudaDeviceProp prop;
+  CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+  if (prop.major != 10)
+    return fail(AFM_EUNSUPPORTED,
+                "device %s is sm_%d%d; this library is built for sm_100a only",
+                prop.name, prop.major, prop.minor);
+  g_ws.checked_device = true;
+  return AFM_OK;
+}
+
+// Serialise reuse of the shared workspace between calls on different streams.
+int acquire_ws(cudaStream_t st) {
+  if (g_ws.last_use == nullptr)
+    CUDA_TRY(cudaEventCreateWithFlags(&g_ws.last_use, cudaEventDisableTiming));
+  else if (g_ws.last_stream != st)
+    CUDA_TRY(cudaStreamWaitEvent(st, g_ws.last_use, 0));
+  return AFM_OK;
+}
+int release_ws(cudaStream_t st) {
+  CUDA_TRY(cudaEventRecord(g_ws.last_use, st));
+  g_ws.last_stream = st;
+  return AFM_OK;
+}
+
+int ensure_pinned(size_t bytes) {
+  if (bytes <= g_ws.pinned_cap) return AFM_OK;
+  if (g_ws.pinned) cudaFreeHost(g_ws.pinned);
+  g_ws.pinned = nullptr;
+  g_ws.pinned_cap = 0;
+  CUDA_TRY(cudaMallocHost(&g_ws.pinned, bytes));
+  g_ws.pinned_cap = bytes;
+  return AFM_OK;
+}
+
+// ---- validation + constants ------------------------------------------------------
+int law_dims(int law) {
+  switch (law) {
+    case AFM_LAW_DMT: return 2;
+    case AFM_LAW_DMT_VISC: return 3;
+    case AFM_LAW_LJ_EXP: return 4;
+    default: return -1;
+  }
+}
+
+int validate_cfg(const afm_cfg* c) {
+  if (!c) return fail(AFM_EINVAL, "cfg is NULL");
+  if (c->law < AFM_LAW_NONE || c->law > AFM_LAW_LJ_EXP)
+    return fail(AFM_EINVAL, "unknown law %d", c->law);
+  if (c->law == AFM_LAW_NONE) {
+    if (c->n_params < 0 || c->n_params > 4)
+      return fail(AFM_EINVAL, "n_params %d out of range 0..4", c->n_params);
+  } else if (c->n_params != law_dims(c->law)) {
+    return fail(AFM_EINVAL, "law %d needs n_params = %d, got %d", c->law,
+                law_dims(c->law), c->n_params);
+  }
+  if (!(c->k > 0) || !(c->f0 > 0) || !(c->Q > 0) || !(c->f_drive > 0))
+    return fail(AFM_EINVAL, "k, f0, Q, f_drive must be positive");
+  if (!(c->A0 > 0)) return fail(AFM_EINVAL, "A0 must be positive");
+  if ((c->law == AFM_LAW_DMT || c->law == AFM_LAW_DMT_VISC) &&
+      (!(c->R > 0) || !(c->a0 > 0)))
+    return fail(AFM_EINVAL, "DMT laws need R > 0 and a0 > 0");
+  if (c->steps_per_cycle < 1 || c->n_cycles < 1)
+    return fail(AFM_EINVAL, "steps_per_cycle and n_cycles must be >= 1");
+  if (c->n_skip_cycles < 0 || c->n_skip_cycles >= c->n_cycles)
+    return fail(AFM_EINVAL, "need 0 <= n_skip_cycles < n_cycles");
+  if ((int64_t)c->steps_per_cycle * c->n_cycles > (int64_t)1 << 30)
+    return fail(AFM_EINVAL, "more than 2^30 steps");
+  if (c->n_traces < 1) return fail(AFM_EINVAL, "n_traces must be >= 1");
+  if (c->precision != AFM_F64 && c->precision != AFM_F32)
+    return fail(AFM_EINVAL, "unknown precision %d", c->precision);
+  if (c->reserved_ != 0) return fail(AFM_EINVAL, "reserved_ must be 0");
+  if (!isfinite(c->z0) || !isfinite(c->v0) || !isfinite(c->z_c))
+    return fail(AFM_EINVAL, "z0, v0, z_c must be finite");
+  return AFM_OK;
+}
+
+void make_consts(const afm_cfg* c, int block, ModelConsts* mc) {
+  const double w0 = 2.0 * M_PI * c->f0;
+  const double w = 2.0 * M_PI * c->f_drive;
+  const double m = c->k / (w0 * w0);
+  const double r = w / w0;
+  const double a = 1.0 - r * r, b = r / c->Q;
+  const double F0 = c->k * c->A0 * sqrt(a * a + b * b);
+  const double h = 2.0 * M_PI / (w * (double)c->steps_per_cycle);
+  memset(mc, 0, sizeof(*mc));
+  mc->h = h;
+  mc->w_drive = w;
+  mc->alpha = h * w0 / c->Q;
+  mc->beta = h * h * (c->k / m);
+  mc->drive_amp = h * h * F0 / m;
+  mc->beta_zc = mc->beta * c->z_c;
+  mc->zc = c->z_c;
+  mc->a0 = c->a0;
+  mc->inv_a0sq = (c->a0 > 0) ? 1.0 / (c->a0 * c->a0) : 0.0;
+  mc->c_vdw = h * h * c->R / (6.0 * m);
+  mc->c_hertz = h * h * (4.0 / 3.0) * sqrt(c->R > 0 ? c->R : 0.0) / m;
+  mc->c_visc = h * sqrt(c->R > 0 ? c->R : 0.0) / m;
+  mc->c_force = h * h / m;
+  mc->d_max = c->z_c + 100.0 * c->A0;
+  mc->d_min = c->z_c - 100.0 * c->A0;
+  mc->z0 = c->z0;
+  mc->v0 = c->v0;
+  mc->law = c->law;
+  mc->D = c->n_params;
+  mc->N = c->steps_per_cycle * c->n_cycles;
+  mc->W = c->steps_per_cycle * (c->n_cycles - c->n_skip_cycles);
+  mc->n0 = mc->N - mc->W;
+  int T = g_opt_tile > 0 ? g_opt_tile : (block <= 32 ? 64 : 128);
+  if (T > mc->N) T = mc->N;
+  mc->T = T;
+  mc->n_tiles = (mc->N + T - 1) / T;
+}
+
+int pick_block(int64_t per, int n_traces) {
+  if (g_opt_block > 0) return g_opt_block;
+  (void)per;
+  (void)n_traces;
+  return 32;
+}
+
+BoxDev make_box(const afm_bounds* b, int D) {
+  BoxDev bd;
+  memset(&bd, 0, sizeof(bd));
+  for (int j = 0; j < D && j < 4; ++j) {
+    bd.lo[j] = b->lo[j];
+    bd.hi[j] = b->hi[j];
+    bd.lg[j] = b->log10_scale[j] ? 1 : 0;
+  }
+  return bd;
+}
+
+int validate_bounds(const afm_bounds* b, int D) {
+  if (!b) return fail(AFM_EINVAL, "bounds is NULL");
+  for (int j = 0; j < D; ++j)
+    if (!isfinite(b->lo[j]) || !isfinite(b->hi[j]) || !(b->lo[j] <= b->hi[j]))
+      return fail(AFM_EINVAL, "bounds[%d] = [%g, %g] is not a finite interval",
+                  j, b->lo[j], b->hi[j]);
+  return AFM_OK;
+}
+
+int validate_swarm(const afm_swarm_cfg* s) {
+  if (!s) return fail(AFM_EINVAL, "swarm is NULL");
+  if (s->n_particles < 1 || s->n_iters < 1)
+    return fail(AFM_EINVAL, "n_particles and n_iters must be >= 1");
+  if (!isfinite(s->w) || !isfinite(s->c1) || !isfinite(s->c2))
+    return fail(AFM_EINVAL, "w, c1, c2 must be finite");
+  return AFM_OK;
+}
+
+// Forward batch on device buffers with the workspace lock already held.
+int forward_locked(const double* params, int64_t P, const double* trace,
+                   const afm_cfg* cfg, const double* z0v0, double* misfit,
+                   cudaStream_t st) {
+  if (cfg->precision == AFM_F32)
+    return fail(AFM_EUNSUPPORTED, "FP32 integrate kernel not built yet");
+  const int64_t per = P / cfg->n_traces;
+  const int block = pick_block(per, cfg->n_traces);
+  ModelConsts mc;
+  make_consts(cfg, block, &mc);
+  int rc = acquire_ws(st);
+  if (rc) return rc;
+  const size_t stream_bytes = (size_t)cfg->n_traces * mc.N * 32;
+  if (g_ws.stream.ensure(stream_bytes))
+    return fail(AFM_ECUDA, "cudaMalloc of %zu B time-tile stream failed",
+                stream_bytes);
+  LAUNCHED(launch_build_stream(mc, trace, cfg->n_traces,
+                               (double*)g_ws.stream.p, st));
+  IntegrateIO io;
+  memset(&io, 0, sizeof(io));
+  io.params = params;
+  io.z0v0 = z0v0;
+  io.stream = (const double*)g_ws.stream.p;
+  io.J = misfit;
+  io.per = per;
+  io.n_traces = cfg->n_traces;
+  io.mode = 0;
+  LAUNCHED(launch_integrate_f64(mc, io, block, st));
+  return release_ws(st);
+}
+
+int validate_forward(const double* params, int64_t P, const double* trace,
+                     const afm_cfg* cfg, double* misfit) {
+  int rc = validate_cfg(cfg);
+  if (rc) return rc;
+  if (P < 1) return fail(AFM_EINVAL, "n_particles must be >= 1");
+  if (P % cfg->n_traces)
+    return fail(AFM_EINVAL, "n_particles %lld is not a multiple of n_traces %d",
+                (long long)P, cfg->n_traces);
+  if (!trace || !misfit) return fail(AFM_EINVAL, "trace/misfit is NULL");
+  if (!params && cfg->n_params > 0) return fail(AFM_EINVAL, "params is NULL");
+  return AFM_OK;
+}
+
+}  // namespace
+
+// =================================================================================
+extern "C" {
+
+int afm_forward_batch(const double* params, int64_t n_particles,
+                      const double* trace, const afm_cfg* cfg,
+                      const double* z0v0, double* misfit, void* cuda_stream) {
+  int rc = validate_forward(params, n_particles, trace, cfg, misfit);
+  if (rc) return rc;
+  if ((rc = check_device())) return rc;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  return forward_locked(params, n_particles, trace, cfg, z0v0, misfit,
+                        (cudaStream_t)cuda_stream);
+}
+
+int afm_forward_batch_host(const double* params, int64_t n_particles,
+                           const double* trace, const afm_cfg* cfg,
+                           const double* z0v0, double* misfit,
+                           void* cuda_stream) {
+  int rc = validate_forward(params, n_particles, trace, cfg, misfit);
+  if (rc) return rc;
+  if ((rc = check_device())) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  const int D = cfg->n_params;
+  const int64_t W =
+      (int64_t)cfg->steps_per_cycle * (cfg->n_cycles - cfg->n_skip_cycles);
+  const size_t pb = (size_t)n_particles * (D > 0 ? D : 1) * 8;
+  const size_t tb = (size_t)cfg->n_traces * W * 8;
+  const size_t zb = (size_t)n_particles * 16;
+  const size_t mb = (size_t)n_particles * 8;
+  if ((rc = acquire_ws(st))) return rc;
+  if (g_ws.h_params.ensure(pb) || g_ws.h_trace.ensure(tb) ||
+      g_ws.h_misfit.ensure(mb) || (z0v0 && g_ws.h_z0v0.ensure(zb)))
+    return fail(AFM_ECUDA, "cudaMalloc of staging buffers failed");
+  if (D > 0)
+    CUDA_TRY(cudaMemcpyAsync(g_ws.h_params.p, params, (size_t)n_particles * D * 8,
+                             cudaMemcpyHostToDevice, st));
+  CUDA_TRY(cudaMemcpyAsync(g_ws.h_trace.p, trace, tb, cudaMemcpyHostToDevice, st));
+  if (z0v0)
+    CUDA_TRY(cudaMemcpyAsync(g_ws.h_z0v0.p, z0v0, zb, cudaMemcpyHostToDevice, st));
+  g_ws.last_stream = st;  // same stream: no self-wait
+  rc = forward_locked((const double*)g_ws.h_params.p, n_particles,
+                      (const double*)g_ws.h_trace.p, cfg,
+                      z0v0 ? (const double*)g_ws.h_z0v0.p : nullptr,
+                      (double*)g_ws.h_misfit.p, st);
+  if (rc) return rc;
+  CUDA_TRY(cudaMemcpyAsync(misfit, g_ws.h_misfit.p, mb, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  return AFM_OK;
+}
+
+int afm_pso_init(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                 int32_t n_dims, int32_t n_traces, uint64_t seed, double* x,
+                 double* v, double* pbest, double* pbestJ, double* gbest,
+                 double* gbestJ, void* cuda_stream) {
+  if (n_dims < 1 || n_dims > 4) return fail(AFM_EINVAL, "n_dims must be 1..4");
+  if (n_traces < 1) return fail(AFM_EINVAL, "n_traces must be >= 1");
+  int rc = validate_bounds(bounds, n_dims);
+  if (rc) return rc;
+  if ((rc = validate_swarm(swarm))) return rc;
+  if (!x || !v || !pbest || !pbestJ || !gbest || !gbestJ)
+    return fail(AFM_EINVAL, "NULL swarm array");
+  if ((rc = check_device())) return rc;
+  LAUNCHED(launch_pso_init(make_box(bounds, n_dims), n_dims, swarm->n_particles,
+                           n_traces, seed, x, v, pbest, pbestJ, gbest, gbestJ,
+                           (cudaStream_t)cuda_stream));
+  return AFM_OK;
+}
+
+int afm_pso_step(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                 int32_t n_dims, int32_t n_traces, uint64_t seed,
+                 int32_t iteration, int32_t do_move, const double* J, double* x,
+                 double* v, double* pbest, double* pbestJ, double* gbest,
+                 double* gbestJ, void* cuda_stream) {
+  if (n_dims < 1 || n_dims > 4) return fail(AFM_EINVAL, "n_dims must be 1..4");
+  if (n_traces < 1) return fail(AFM_EINVAL, "n_traces must be >= 1");
+  if (iteration < 0) return fail(AFM_EINVAL, "iteration must be >= 0");
+  int rc = validate_bounds(bounds, n_dims);
+  if (rc) return rc;
+  if ((rc = validate_swarm(swarm))) return rc;
+  if (!J || !x || !v || !pbest || !pbestJ || !gbest || !gbestJ)
+    return fail(AFM_EINVAL, "NULL swarm array");
+  if ((rc = check_device())) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  const int64_t per = swarm->n_particles;
+  const int block = 128;
+  const int bpt = blocks_per_trace(per, block);
+  if ((rc = acquire_ws(st))) return rc;
+  if (g_ws.cand.ensure((size_t)bpt * n_traces * sizeof(Cand)))
+    return fail(AFM_ECUDA, "cudaMalloc of candidates failed");
+  BoxDev box = make_box(bounds, n_dims);
+  SwarmDev sw = {swarm->w, swarm->c1, swarm->c2};
+  LAUNCHED(launch_pso_best(n_dims, per, n_traces, J, x, pbest, pbestJ,
+                           (Cand*)g_ws.cand.p, block, st));
+  LAUNCHED(launch_pso_gbest(box, n_dims, n_traces, bpt, (Cand*)g_ws.cand.p,
+                            pbest, gbest, gbestJ, nullptr, nullptr, nullptr, st));
+  if (do_move)
+    LAUNCHED(launch_pso_move(box, sw, n_dims, per, n_traces, seed,
+                             (uint32_t)iteration, 1, J, x, v, pbest, pbestJ,
+                             gbest, nullptr, st));
+  return release_ws(st);
+}
+
+static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                             uint64_t seed, const double* trace,
+                             const afm_cfg* cfg, double* theta_star,
+                             double* J_star, double* swarm_dump,
+                             double* gbest_hist, int32_t* n_iters_done,
+                             cudaStream_t st) {
+  if (cfg->precision == AFM_F32)
+    return fail(AFM_EUNSUPPORTED, "FP32 integrate kernel not built yet");
+  const int D = cfg->n_params;
+  const int T = cfg->n_traces;
+  const int64_t per = swarm->n_particles;
+  const int64_t PT = per * T;
+  const int block = pick_block(per, T);
+  const int bpt = blocks_per_trace(per, block);
+  ModelConsts mc;
+  make_consts(cfg, block, &mc);
+  int rc = acquire_ws(st);
+  if (rc) return rc;
+
+  // workspace carve-up (doubles): x, v, pbest [PT][D]; J, pbestJ [PT];
+  // gbest [T][D]; gbestJ [T]; theta* [T][D]; J* [T]
+  const size_t n_dbl = (size_t)PT * (3 * D + 2) + (size_t)T * (2 * D + 2);
+  if (g_ws.swarm.ensure(n_dbl * 8) ||
+      g_ws.cand.ensure((size_t)bpt * T * sizeof(Cand)) ||
+      g_ws.stream.ensure((size_t)T * mc.N * 32))
+    return fail(AFM_ECUDA, "cudaMalloc of the PSO workspace failed");
+  double* x = (double*)g_ws.swarm.p;
+  double* v = x + PT * D;
+  double* pbest = v + PT * D;
+  double* J = pbest + PT * D;
+  double* pbestJ = J + PT;
+  double* gbest = pbestJ + PT;
+  double* gbestJ = gbest + (size_t)T * D;
+  double* th_dev = gbestJ + T;
+  double* Js_dev = th_dev + (size_t)T * D;
+  if ((rc = ensure_pinned((size_t)T * 8))) return rc;
+
+  BoxDev box = make_box(bounds, D);
+  SwarmDev sw = {swarm->w, swarm->c1, swarm->c2};
+
+  LAUNCHED(launch_build_stream(mc, trace, T, (double*)g_ws.stream.p, st));
+  LAUNCHED(launch_pso_init(box, D, per, T, seed, x, v, pbest, pbestJ, gbest,
+                           gbestJ, st));
+  IntegrateIO io;
+  memset(&io, 0, sizeof(io));
+  io.params = x;
+  io.z0v0 = nullptr;
+  io.stream = (const double*)g_ws.stream.p;
+  io.J = J;
+  io.pbest = pbest;
+  io.pbestJ = pbestJ;
+  io.cand = (Cand*)g_ws.cand.p;
+  io.box = box;
+  io.per = per;
+  io.n_traces = T;
+  io.mode = 1;
+
+  int done = 0;
+  for (int it = 0; it < swarm->n_iters; ++it) {
+    const bool last = (it == swarm->n_iters - 1);
+    LAUNCHED(launch_integrate_f64(mc, io, block, st));
+    LAUNCHED(launch_pso_gbest(
+        box, D, T, bpt, (Cand*)g_ws.cand.p, pbest, gbest, gbestJ,
+        gbest_hist ? gbest_hist + (size_t)it * T * (D + 1) : nullptr, th_dev,
+        Js_dev, st));
+    bool stop = last;
+    if (!stop && swarm->j_target > 0) {
+      double* hJ = (double*)g_ws.pinned;
+      CUDA_TRY(cudaMemcpyAsync(hJ, gbestJ, (size_t)T * 8, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(cudaStreamSynchronize(st));
+      stop = true;
+      for (int s = 0; s < T; ++s)
+        if (!(hJ[s] <= swarm->j_target)) stop = false;
+    }
+    double* dump_row =
+        swarm_dump ? swarm_dump + (size_t)it * PT * (3 * D + 2) : nullptr;
+    if (!stop || dump_row)
+      LAUNCHED(launch_pso_move(box, sw, D, per, T, seed, (uint32_t)it,
+                               stop ? 0 : 1, J, x, v, pbest, pbestJ, gbest,
+                               dump_row, st));
+    done = it + 1;
+    if (stop) break;
+  }
+  CUDA_TRY(cudaMemcpyAsync(theta_star, th_dev, (size_t)T * D * 8,
+                           cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaMemcpyAsync(J_star, Js_dev, (size_t)T * 8, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  if (n_iters_done) *n_iters_done = done;
+  return release_ws(st);
+}
+
+static int validate_invert(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                           const double* trace, const afm_cfg* cfg,
+                           double* theta_star, double* J_star) {
+  int rc = validate_cfg(cfg);
+  if (rc) return rc;
+  if (cfg->n_params < 1)
+    return fail(AFM_EINVAL, "nothing to invert: n_params = 0");
+  if ((rc = validate_bounds(bounds, cfg->n_params))) return rc;
+  if ((rc = validate_swarm(swarm))) return rc;
+  if (!trace || !theta_star || !J_star)
+    return fail(AFM_EINVAL, "trace/theta_star/J_star is NULL");
+  return AFM_OK;
+}
+
+int afm_pso_invert(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                   uint64_t seed, const double* trace, const afm_cfg* cfg,
+                   double* theta_star, double* J_star, double* swarm_dump,
+                   double* gbest_hist, int32_t* n_iters_done,
+                   void* cuda_stream) {
+  int rc = validate_invert(bounds, swarm, trace, cfg, theta_star, J_star);
+  if (rc) return rc;
+  if ((rc = check_device())) return rc;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  return pso_invert_locked(bounds, swarm, seed, trace, cfg, theta_star, J_star,
+                           swarm_dump, gbest_hist, n_iters_done,
+                           (cudaStream_t)cuda_stream);
+}
+
+int afm_pso_invert_host(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                        uint64_t seed, const double* trace, const afm_cfg* cfg,
+                        double* theta_star, double* J_star,
+                        int32_t* n_iters_done, void* cuda_stream) {
+  int rc = validate_invert(bounds, swarm, trace, cfg, theta_star, J_star);
+  if (rc) return rc;
+  if ((rc = check_device())) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  const int64_t W =
+      (int64_t)cfg->steps_per_cycle * (cfg->n_cycles - cfg->n_skip_cycles);
+  const size_t tb = (size_t)cfg->n_traces * W * 8;
+  if ((rc = acquire_ws(st))) return rc;
+  if (g_ws.h_trace.ensure(tb))
+    return fail(AFM_ECUDA, "cudaMalloc of the trace staging buffer failed");
+  CUDA_TRY(cudaMemcpyAsync(g_ws.h_trace.p, trace, tb, cudaMemcpyHostToDevice, st));
+  g_ws.last_stream = st;
+  return pso_invert_locked(bounds, swarm, seed, (const double*)g_ws.h_trace.p,
+                           cfg, theta_star, J_star, nullptr, nullptr,
+                           n_iters_done, st);
+}
+
+int afm_philox4x32_10(const uint32_t* ctr, int64_t n, const uint32_t* key,
+                      uint32_t* out, void* cuda_stream) {
+  if (!ctr || !key || !out || n < 0)
+    return fail(AFM_EINVAL, "NULL pointer or negative n");
+  if (n == 0) return AFM_OK;
+  int rc = check_device();
+  if (rc) return rc;
+  LAUNCHED(launch_philox(ctr, n, key[0], key[1], out, (cudaStream_t)cuda_stream));
+  return AFM_OK;
+}
+
+int afm_trajectory(const double* theta, const afm_cfg* cfg, double z0, double v0,
+                   double* zs, double* vs, void* cuda_stream) {
+  int rc = validate_cfg(cfg);
+  if (rc) return rc;
+  if (!theta && cfg->n_params > 0) return fail(AFM_EINVAL, "theta is NULL");
+  if ((rc = check_device())) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  afm_cfg c1 = *cfg;
+  c1.n_traces = 1;
+  ModelConsts mc;
+  make_consts(&c1, 32, &mc);
+  if ((rc = acquire_ws(st))) return rc;
+  // a zero trace: the stream's trace column is unused by the trajectory kernel
+  const size_t need = (size_t)mc.N * 32 + (size_t)mc.W * 8 + 64;
+  if (g_ws.stream.ensure(need) || g_ws.scratch.ensure(64))
+    return fail(AFM_ECUDA, "cudaMalloc failed");
+  double* zero_trace = (double*)((char*)g_ws.stream.p + (size_t)mc.N * 32);
+  CUDA_TRY(cudaMemsetAsync(zero_trace, 0, (size_t)mc.W * 8, st));
+  if (cfg->n_params > 0)
+    CUDA_TRY(cudaMemcpyAsync(g_ws.scratch.p, theta, (size_t)cfg->n_params * 8,
+                             cudaMemcpyHostToDevice, st));
+  LAUNCHED(launch_build_stream(mc, zero_trace, 1, (double*)g_ws.stream.p, st));
+  LAUNCHED(launch_trajectory(mc, (const double*)g_ws.scratch.p,
+                             (const double*)g_ws.stream.p, z0, v0, zs, vs, st));
+  return release_ws(st);
+}
+
+int64_t afm_launch_count(void) { return g_launches; }
+void afm_reset_launch_count(void) { g_launches = 0; }
+
+int afm_set_option(const char* name, int64_t value) {
+  if (!name) return fail(AFM_EINVAL, "option name is NULL");
+  if (!strcmp(name, "block")) {
+    if (value != 0 && value != 32 && value != 64 && value != 128)
+      return fail(AFM_EINVAL, "block must be 0, 32, 64 or 128");
+    g_opt_block = (int)value;
+    return AFM_OK;
+  }
+  if (!strcmp(name, "tile")) {
+    if (value < 0 || value > 2048)
+      return fail(AFM_EINVAL, "tile must be in 0..2048");
+    g_opt_tile = (int)value;
+    return AFM_OK;
+  }
+  return fail(AFM_EINVAL, "unknown option '%s'", name);
+}
+
+const char* afm_last_error(void) { return g_err; }
+const char* afm_version(void) { return "afm-b200 0.1 (sm_100a)"; }
+
+void afm_shutdown(void) {
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  g_ws.stream.release();
+  g_ws.swarm.release();
+  g_ws.cand.release();
+  g_ws.h_params.release();
+  g_ws.h_trace.release();
+  g_ws.h_z0v0.release();
+  g_ws.h_misfit.release();
+  g_ws.scratch.release();
+  if (g_ws.pinned) cudaFreeHost(g_ws.pinned);
+  g_ws.pinned = nullptr;
+  g_ws.pinned_cap = 0;
+  if (g_ws.last_use) cudaEventDestroy(g_ws.last_use);
+  g_ws.last_use = nullptr;
+  g_ws.last_stream = nullptr;
+}
+
+}  // extern "C"

@@ -1,0 +1,126 @@
+// afm_internal.h -- shared between the kernel translation unit and the C-ABI
+// host code of libafm_b200.so.  Not part of the public interface (include/afm.h)
+// and shared with nothing outside csrc/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "afm.h"
+
+namespace afm {
+
+// Scaled constants of the point-mass ODE (north_star; m = 1 case of Eq. 2,
+// PAPER.md:64) in "per-step" variables: state (d, w) with d = z + z_c the gap
+// and w = h z' the displacement per step, so one RK4 step has unit length and
+//     w' = Dp(t) - alpha w - beta d + f(d, w),
+//     Dp(t) = (h^2 F0/m) cos(w_drive t) + beta z_c,   f = (h^2/m) F_ts.
+// Everything here is computed on the host in FP64 from afm_cfg.
+struct ModelConsts {
+  double h;          // dt = 2 pi / (w_drive S)
+  double w_drive;    // 2 pi f_drive
+  double alpha;      // h w0 / Q
+  double beta;       // (h w0)^2
+  double drive_amp;  // h^2 F0 / m
+  double beta_zc;    // beta z_c
+  double zc, a0;
+  double inv_a0sq;   // 1 / a0^2
+  double c_vdw;      // h^2 R / (6 m):        kappa = H c_vdw
+  double c_hertz;    // h^2 (4/3) sqrt(R)/m:  eps   = E* c_hertz
+  double c_visc;     // h sqrt(R) / m:        nu    = eta c_visc
+  double c_force;    // h^2 / m
+  double d_max;      // z_c + 100 A0   (divergence rule R12 on d)
+  double d_min;      // z_c - 100 A0   (negative)
+  double z0, v0;     // default initial state, SI
+  int32_t law, D;
+  int32_t N;         // total steps
+  int32_t n0;        // first step whose post-state is in the misfit window
+  int32_t W;         // window length
+  int32_t T;         // steps per time tile
+  int32_t n_tiles;
+  int32_t pad_;
+};
+
+// FP32 kernel constants (kernel units: length 1 nm, time 1/w0; R14).
+struct ModelConstsF32 {
+  double len;        // metres per kernel length unit (1e-9)
+  double hq;         // h w0 (step in kernel time units), FP64; split hi/lo below
+  float h_hi, h_lo;  // two-float step
+  float inv_Q;
+  float zc, a0, inv_a0sq, sqrt_a0_dummy;
+  double c_vdw, c_hertz, c_visc, c_force;  // FP64 scale factors: p_j = theta_j * c
+  float d_max, d_min;
+  float z0, v0;
+  int32_t law, D, N, n0, W, T, n_tiles, pad_;
+};
+
+struct BoxDev {
+  double lo[4], hi[4];
+  int32_t lg[4];
+};
+
+struct SwarmDev {
+  double w, c1, c2;
+};
+
+// One block-level (pbestJ, particle index) candidate of the global-best search.
+struct Cand {
+  double J;
+  long long idx;
+};
+
+// ---- launchers (afm_kernels.cu) -------------------------------------------
+// Every launcher returns the number of kernels it enqueued (>= 1) or a
+// negative value after setting a CUDA error (checked by the caller with
+// cudaGetLastError()).
+
+struct IntegrateIO {
+  const double* params;   // MODE 0: theta [PT][D]; MODE 1: x [PT][D]
+  const double* z0v0;     // [PT][2] or nullptr
+  const double* stream;   // [n_traces][N][4] time-tile stream
+  double* J;              // [PT]
+  // MODE 1 (PSO) only:
+  double* pbest;          // [PT][D]
+  double* pbestJ;         // [PT]
+  Cand* cand;             // [n_traces][blocks_per_trace]
+  BoxDev box;
+  int64_t per;            // particles per trace
+  int32_t n_traces;
+  int32_t mode;           // 0 forward, 1 PSO
+};
+
+int blocks_per_trace(int64_t per, int block);
+
+int launch_build_stream(const ModelConsts& mc, const double* trace, int n_traces,
+                        double* stream, cudaStream_t st);
+int launch_build_stream_f32(const ModelConsts& mc, const ModelConstsF32& mf,
+                            const double* trace, int n_traces, float* stream,
+                            cudaStream_t st);
+int launch_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block,
+                         cudaStream_t st);
+int launch_integrate_f32(const ModelConsts& mc, const ModelConstsF32& mf,
+                         const IntegrateIO& io, int block, cudaStream_t st);
+int launch_trajectory(const ModelConsts& mc, const double* theta_dev,
+                      const double* stream, double z0, double v0, double* zs,
+                      double* vs, cudaStream_t st);
+
+int launch_pso_init(const BoxDev& box, int D, int64_t per, int n_traces,
+                    uint64_t seed, double* x, double* v, double* pbest,
+                    double* pbestJ, double* gbest, double* gbestJ,
+                    cudaStream_t st);
+int launch_pso_best(int D, int64_t per, int n_traces, const double* J,
+                    const double* x, double* pbest, double* pbestJ, Cand* cand,
+                    int block, cudaStream_t st);
+int launch_pso_gbest(const BoxDev& box, int D, int n_traces, int n_cand,
+                     const Cand* cand, const double* pbest, double* gbest,
+                     double* gbestJ, double* hist_row, double* theta_star,
+                     double* J_star, cudaStream_t st);
+int launch_pso_move(const BoxDev& box, const SwarmDev& sw, int D, int64_t per,
+                    int n_traces, uint64_t seed, uint32_t it, int do_move,
+                    const double* J, double* x, double* v, const double* pbest,
+                    const double* pbestJ, const double* gbest, double* dump_row,
+                    cudaStream_t st);
+int launch_philox(const uint32_t* ctr, int64_t n, uint32_t k0, uint32_t k1,
+                  uint32_t* out, cudaStream_t st);
+
+}  // namespace afm

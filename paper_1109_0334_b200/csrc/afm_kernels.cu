@@ -1,0 +1,608 @@
+// afm_kernels.cu -- sm_100a kernels of the dAFM force-inversion hot path.
+//
+//   build_stream_kernel     time-tile stream: drive at the three RK4 abscissae
+//                           of every step + the measured trace, 32 B per step
+//   integrate_misfit_f64    a1-a5 of SURVEY.md 8(a): parameter map, RK4 forward
+//                           solve with register-resident state, squared misfit,
+//                           personal best + block argmin candidate (PSO mode)
+//   pso_init/best/gbest/move  a5-a7: Philox-driven swarm (Eq. 8)
+//
+// One thread integrates one particle; the particles of a CTA share one trace,
+// which (with the drive) is streamed global -> shared by 1-D bulk async copies
+// (cp.async.bulk, SASS UBLKCP) into a two-stage mbarrier ring.
+#include <math_constants.h>
+
+#include "afm_device.cuh"
+#include "afm_internal.h"
+
+namespace afm {
+
+// ============================================================================
+// Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11): the counter-based
+// generator north_star names.  DESIGN.md reading R11 fixes key and counter.
+// ============================================================================
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1,
+                                              uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1,
+                                              uint32_t out[4]) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    uint32_t n0 = hi1 ^ c1 ^ k0;
+    uint32_t n2 = hi0 ^ c3 ^ k1;
+    c0 = n0;
+    c1 = lo1;
+    c2 = n2;
+    c3 = lo0;
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  out[0] = c0;
+  out[1] = c1;
+  out[2] = c2;
+  out[3] = c3;
+}
+
+// 24-bit uniform in [0, 1), exact in FP32 and FP64.
+__device__ __forceinline__ double u24(uint32_t word) {
+  return (double)(word >> 8) * (1.0 / 16777216.0);
+}
+
+// a[j], b[j] for j < D: counter = (particle lo, iteration, pair + 16*purpose,
+// particle hi); the four words of pair q are (a[2q], b[2q], a[2q+1], b[2q+1]).
+__device__ __forceinline__ void pso_uniforms(uint64_t seed, uint64_t gp,
+                                             uint32_t it, uint32_t purpose,
+                                             int D, double a[4], double b[4]) {
+  const uint32_t k0 = (uint32_t)(seed & 0xffffffffu);
+  const uint32_t k1 = (uint32_t)(seed >> 32);
+#pragma unroll
+  for (int q = 0; q < 2; ++q) {
+    if (2 * q < D) {
+      uint32_t o[4];
+      philox4x32_10((uint32_t)(gp & 0xffffffffu), it,
+                    (uint32_t)q + 16u * purpose, (uint32_t)(gp >> 32), k0, k1,
+                    o);
+      a[2 * q] = u24(o[0]);
+      b[2 * q] = u24(o[1]);
+      a[2 * q + 1] = u24(o[2]);
+      b[2 * q + 1] = u24(o[3]);
+    }
+  }
+}
+
+__global__ void philox_kernel(const uint32_t* __restrict__ ctr, int64_t n,
+                              uint32_t k0, uint32_t k1,
+                              uint32_t* __restrict__ out) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  uint32_t o[4];
+  philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], k0,
+                k1, o);
+  out[4 * i] = o[0];
+  out[4 * i + 1] = o[1];
+  out[4 * i + 2] = o[2];
+  out[4 * i + 3] = o[3];
+}
+
+// ============================================================================
+// Time-tile stream.  Row n of trace s: { Dp(t_n), Dp(t_n + h/2), Dp(t_n + h),
+// U_s[n - n0] + z_c (0 before the window) },  t_n = n h (never accumulated),
+// Dp(t) = drive_amp cos(w t) + beta z_c.
+// ============================================================================
+__global__ void build_stream_kernel(ModelConsts mc,
+                                    const double* __restrict__ trace,
+                                    int n_traces, double* __restrict__ stream) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int64_t total = (int64_t)n_traces * mc.N;
+  if (i >= total) return;
+  int s = (int)(i / mc.N);
+  int n = (int)(i - (int64_t)s * mc.N);
+  double t = __dmul_rn((double)n, mc.h);
+  double th = __dadd_rn(t, __dmul_rn(0.5, mc.h));
+  double t1 = __dadd_rn(t, mc.h);
+  double4 row;
+  row.x = fma(mc.drive_amp, cos(__dmul_rn(mc.w_drive, t)), mc.beta_zc);
+  row.y = fma(mc.drive_amp, cos(__dmul_rn(mc.w_drive, th)), mc.beta_zc);
+  row.z = fma(mc.drive_amp, cos(__dmul_rn(mc.w_drive, t1)), mc.beta_zc);
+  row.w = (n >= mc.n0) ? trace[(int64_t)s * mc.W + (n - mc.n0)] + mc.zc : 0.0;
+  reinterpret_cast<double4*>(stream)[i] = row;
+}
+
+// ============================================================================
+// integrate-and-misfit, FP64
+// ============================================================================
+__device__ __forceinline__ bool cand_less(double Ja, long long ia, double Jb,
+                                          long long ib) {
+  return (Ja < Jb) || (Ja == Jb && ia < ib);
+}
+
+// Block argmin of (J, idx), lowest idx among equal J; result valid in thread 0.
+__device__ __forceinline__ void block_argmin(double& J, long long& idx,
+                                             Cand* red /* [32] shared */) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int nwarps = (blockDim.x + 31) >> 5;
+#pragma unroll
+  for (int off = 16; off >= 1; off >>= 1) {
+    double Jo = __shfl_down_sync(0xffffffffu, J, off);
+    long long io = __shfl_down_sync(0xffffffffu, idx, off);
+    if (cand_less(Jo, io, J, idx)) {
+      J = Jo;
+      idx = io;
+    }
+  }
+  if (nwarps == 1) return;
+  if (lane == 0) {
+    red[warp].J = J;
+    red[warp].idx = idx;
+  }
+  __syncthreads();
+  if (warp == 0) {
+    J = (lane < nwarps) ? red[lane].J : CUDART_INF;
+    idx = (lane < nwarps) ? red[lane].idx : 0x7fffffffffffffffLL;
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+      double Jo = __shfl_down_sync(0xffffffffu, J, off);
+      long long io = __shfl_down_sync(0xffffffffu, idx, off);
+      if (cand_less(Jo, io, J, idx)) {
+        J = Jo;
+        idx = io;
+      }
+    }
+  }
+}
+
+template <int LAW, int MODE>
+__global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
+                                     int blocks_per_tr) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double4* tile0 = reinterpret_cast<double4*>(smem_raw);
+  double4* tile1 = tile0 + mc.T;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tile1 + mc.T);
+  __shared__ Cand red[32];
+
+  const int tid = threadIdx.x;
+  const int s = blockIdx.x / blocks_per_tr;  // trace (segment) of this CTA
+  const int64_t li =
+      (int64_t)(blockIdx.x - s * blocks_per_tr) * blockDim.x + tid;
+  const bool active = li < io.per;
+  // inactive threads of a ragged last CTA integrate a copy of the segment's
+  // last particle (keeps every barrier uniform) and write nothing
+  const int64_t gp = (int64_t)s * io.per + (active ? li : io.per - 1);
+
+  const double* stream = io.stream + (int64_t)s * mc.N * 4;
+  const uint32_t tile_bytes = (uint32_t)mc.T * 32u;
+
+  if (tid == 0) {
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    fence_mbar_init();
+  }
+  __syncthreads();
+  if (tid == 0) {
+#pragma unroll
+    for (int st = 0; st < 2; ++st) {
+      if (st < mc.n_tiles) {
+        int n_begin = st * mc.T;
+        uint32_t bytes = (uint32_t)min(mc.T, mc.N - n_begin) * 32u;
+        mbar_arrive_expect_tx(&bars[st], bytes);
+        bulk_g2s(st ? tile1 : tile0, stream + (int64_t)n_begin * 4, bytes,
+                 &bars[st]);
+      }
+    }
+  }
+  (void)tile_bytes;
+
+  // ---- a1: parameter map ---------------------------------------------------
+  double xloc[4] = {0.0, 0.0, 0.0, 0.0};
+  double th[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    if (j < mc.D) {
+      double xv = io.params[gp * mc.D + j];
+      xloc[j] = xv;
+      th[j] = (MODE == 1 && io.box.lg[j]) ? pow(10.0, xv) : xv;
+    }
+  }
+  Particle64 P;
+  load_particle(P, LAW, th, mc.alpha, mc.beta, mc.a0, mc.inv_a0sq, mc.c_vdw,
+                mc.c_hertz, mc.c_visc, mc.c_force);
+
+  double z0 = mc.z0, v0 = mc.v0;
+  if (io.z0v0 != nullptr) {
+    z0 = io.z0v0[2 * gp];
+    v0 = io.z0v0[2 * gp + 1];
+  }
+  double d = z0 + mc.zc;
+  double w = v0 * mc.h;
+  double J = 0.0;
+  const long long key_max = order_key(mc.d_max);
+  const long long key_min = order_key(mc.d_min);
+  bool bad = false;
+
+  // ---- a2-a4: RK4 over the time tiles -------------------------------------
+  for (int tile = 0; tile < mc.n_tiles; ++tile) {
+    const int st = tile & 1;
+    const double4* sp = st ? tile1 : tile0;
+    mbar_wait(&bars[st], (uint32_t)((tile >> 1) & 1));
+    const int n_begin = tile * mc.T;
+    const int n_steps = min(mc.T, mc.N - n_begin);
+    // steps [0, k0) of this tile precede the misfit window
+    const int k0 = max(0, min(n_steps, mc.n0 - n_begin));
+    int i = 0;
+    for (; i < k0; ++i) {
+      const double4 r = sp[i];
+      rk4_step<LAW>(P, r.x, r.y, r.z, d, w);
+      const long long key = order_key(d);
+      bad |= (key > key_max) | (key < key_min);
+    }
+    for (; i < n_steps; ++i) {
+      const double4 r = sp[i];
+      rk4_step<LAW>(P, r.x, r.y, r.z, d, w);
+      const long long key = order_key(d);
+      bad |= (key > key_max) | (key < key_min);
+      const double res = d - r.w;
+      J = fma(res, res, J);
+    }
+    __syncthreads();  // every thread is done reading stage st
+    if (tid == 0 && tile + 2 < mc.n_tiles) {
+      const int nb = (tile + 2) * mc.T;
+      const uint32_t bytes = (uint32_t)min(mc.T, mc.N - nb) * 32u;
+      fence_proxy_async();
+      mbar_arrive_expect_tx(&bars[st], bytes);
+      bulk_g2s(st ? tile1 : tile0, stream + (int64_t)nb * 4, bytes, &bars[st]);
+    }
+  }
+  // the velocity of the last state must be finite too (R12)
+  {
+    const long long kw = __double_as_longlong(w) & 0x7fffffffffffffffLL;
+    bad |= (kw >= 0x7ff0000000000000LL);
+  }
+  if (bad || !(J == J)) J = CUDART_INF;
+
+  if (active) io.J[gp] = J;
+
+  // ---- a5 + first level of a6 (PSO mode) -----------------------------------
+  if (MODE == 1) {
+    double pb = CUDART_INF;
+    long long idx = 0x7fffffffffffffffLL;
+    if (active) {
+      pb = io.pbestJ[gp];
+      if (J < pb) {  // strict: NaN/+Inf never win
+        pb = J;
+        io.pbestJ[gp] = J;
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+          if (j < mc.D) io.pbest[gp * mc.D + j] = xloc[j];
+      }
+      idx = gp;
+    }
+    block_argmin(pb, idx, red);
+    if (tid == 0) {
+      io.cand[blockIdx.x].J = pb;
+      io.cand[blockIdx.x].idx = idx;
+    }
+  }
+}
+
+// Trajectory of one particle through the same rk4_step (tests/diagnostics).
+template <int LAW>
+__global__ void trajectory_kernel(ModelConsts mc, const double* __restrict__ th,
+                                  const double* __restrict__ stream, double z0,
+                                  double v0, double* __restrict__ zs,
+                                  double* __restrict__ vs) {
+  if (blockIdx.x != 0 || threadIdx.x != 0) return;
+  double t4[4] = {0.0, 0.0, 0.0, 0.0};
+  for (int j = 0; j < mc.D && j < 4; ++j) t4[j] = th[j];
+  Particle64 P;
+  load_particle(P, LAW, t4, mc.alpha, mc.beta, mc.a0, mc.inv_a0sq, mc.c_vdw,
+                mc.c_hertz, mc.c_visc, mc.c_force);
+  double d = z0 + mc.zc, w = v0 * mc.h;
+  const double inv_h = 1.0 / mc.h;
+  if (zs) zs[0] = z0;
+  if (vs) vs[0] = v0;
+  const double4* rows = reinterpret_cast<const double4*>(stream);
+  for (int n = 0; n < mc.N; ++n) {
+    const double4 r = rows[n];
+    rk4_step<LAW>(P, r.x, r.y, r.z, d, w);
+    if (zs) zs[n + 1] = d - mc.zc;
+    if (vs) vs[n + 1] = w * inv_h;
+  }
+}
+
+// ============================================================================
+// PSO kernels (readings R10/R11).  All FP64; every product
+// and sum is written with explicit round-to-nearest intrinsics so that no FMA
+// contraction changes the value: the swarm state replays bit for bit.
+// ============================================================================
+__global__ void pso_init_kernel(BoxDev box, int D, int64_t per, int n_traces,
+                                uint64_t seed, double* __restrict__ x,
+                                double* __restrict__ v,
+                                double* __restrict__ pbest,
+                                double* __restrict__ pbestJ,
+                                double* __restrict__ gbest,
+                                double* __restrict__ gbestJ) {
+  const int64_t gp = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t PT = per * n_traces;
+  if (gp >= PT) return;
+  double a[4], b[4];
+  pso_uniforms(seed, (uint64_t)gp, 0u, 0u, D, a, b);
+  const bool first = (gp % per) == 0;
+  const int64_t s = gp / per;
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    if (j < D) {
+      const double span = __dsub_rn(box.hi[j], box.lo[j]);
+      const double x0 = __dadd_rn(box.lo[j], __dmul_rn(a[j], span));
+      const double y0 = __dadd_rn(box.lo[j], __dmul_rn(b[j], span));
+      x[gp * D + j] = x0;
+      v[gp * D + j] = __dmul_rn(0.5, __dsub_rn(y0, x0));
+      pbest[gp * D + j] = x0;
+      if (first) gbest[s * D + j] = x0;
+    }
+  }
+  pbestJ[gp] = CUDART_INF;
+  if (first) gbestJ[s] = CUDART_INF;
+}
+
+// Personal best from caller-supplied J + block candidates (the stand-alone
+// form of the epilogue fused into integrate_misfit_f64<., 1>).
+__global__ void pso_best_kernel(int D, int64_t per, int blocks_per_tr,
+                                const double* __restrict__ J,
+                                const double* __restrict__ x,
+                                double* __restrict__ pbest,
+                                double* __restrict__ pbestJ,
+                                Cand* __restrict__ cand) {
+  __shared__ Cand red[32];
+  const int s = blockIdx.x / blocks_per_tr;
+  const int64_t li =
+      (int64_t)(blockIdx.x - s * blocks_per_tr) * blockDim.x + threadIdx.x;
+  const bool active = li < per;
+  const int64_t gp = (int64_t)s * per + li;
+  double pb = CUDART_INF;
+  long long idx = 0x7fffffffffffffffLL;
+  if (active) {
+    const double Jp = J[gp];
+    pb = pbestJ[gp];
+    if (Jp < pb) {
+      pb = Jp;
+      pbestJ[gp] = Jp;
+      for (int j = 0; j < D; ++j) pbest[gp * D + j] = x[gp * D + j];
+    }
+    idx = gp;
+  }
+  block_argmin(pb, idx, red);
+  if (threadIdx.x == 0) {
+    cand[blockIdx.x].J = pb;
+    cand[blockIdx.x].idx = idx;
+  }
+}
+
+// Global best of one trace per CTA: lowest index among the minima of pbestJ,
+// taken only on a strict improvement over the stored gbestJ.
+__global__ void pso_gbest_kernel(BoxDev box, int D, int n_cand,
+                                 const Cand* __restrict__ cand,
+                                 const double* __restrict__ pbest,
+                                 double* __restrict__ gbest,
+                                 double* __restrict__ gbestJ,
+                                 double* __restrict__ hist_row,
+                                 double* __restrict__ theta_star,
+                                 double* __restrict__ J_star) {
+  __shared__ Cand red[32];
+  const int s = blockIdx.x;
+  double Jm = CUDART_INF;
+  long long im = 0x7fffffffffffffffLL;
+  for (int c = threadIdx.x; c < n_cand; c += blockDim.x) {
+    const Cand cd = cand[(int64_t)s * n_cand + c];
+    if (cand_less(cd.J, cd.idx, Jm, im)) {
+      Jm = cd.J;
+      im = cd.idx;
+    }
+  }
+  block_argmin(Jm, im, red);
+  if (threadIdx.x == 0) {
+    double gJ = gbestJ[s];
+    if (Jm < gJ) {
+      gJ = Jm;
+      gbestJ[s] = Jm;
+      for (int j = 0; j < D; ++j) gbest[s * D + j] = pbest[im * D + j];
+    }
+    for (int j = 0; j < D; ++j) {
+      const double g = gbest[s * D + j];
+      if (hist_row) hist_row[s * (D + 1) + j] = g;
+      if (theta_star) theta_star[s * D + j] = box.lg[j] ? pow(10.0, g) : g;
+    }
+    if (hist_row) hist_row[s * (D + 1) + D] = gJ;
+    if (J_star) J_star[s] = gJ;
+  }
+}
+
+// Optional dump, then Eq. 8, x <- x + v, clamp + zero velocity.
+__global__ void pso_move_kernel(BoxDev box, SwarmDev sw, int D, int64_t per,
+                                int n_traces, uint64_t seed, uint32_t it,
+                                int do_move, const double* __restrict__ J,
+                                double* __restrict__ x, double* __restrict__ v,
+                                const double* __restrict__ pbest,
+                                const double* __restrict__ pbestJ,
+                                const double* __restrict__ gbest,
+                                double* __restrict__ dump_row) {
+  const int64_t gp = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t PT = per * n_traces;
+  if (gp >= PT) return;
+  const int64_t s = gp / per;
+  double xi[4], vi[4], pb[4];
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    if (j < D) {
+      xi[j] = x[gp * D + j];
+      vi[j] = v[gp * D + j];
+      pb[j] = pbest[gp * D + j];
+    }
+  }
+  if (dump_row) {
+    double* r = dump_row + gp * (3 * D + 2);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      if (j < D) {
+        r[j] = xi[j];
+        r[D + j] = vi[j];
+        r[2 * D + j] = pb[j];
+      }
+    }
+    r[3 * D] = J[gp];
+    r[3 * D + 1] = pbestJ[gp];
+  }
+  if (!do_move) return;
+  double r1[4], r2[4];
+  pso_uniforms(seed, (uint64_t)gp, it, 1u, D, r1, r2);
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    if (j < D) {
+      const double gb = gbest[s * D + j];
+      const double t0 = __dmul_rn(sw.w, vi[j]);
+      const double t1 =
+          __dmul_rn(__dmul_rn(sw.c1, r1[j]), __dsub_rn(pb[j], xi[j]));
+      const double t2 =
+          __dmul_rn(__dmul_rn(sw.c2, r2[j]), __dsub_rn(gb, xi[j]));
+      double vn = __dadd_rn(__dadd_rn(t0, t1), t2);
+      double xn = __dadd_rn(xi[j], vn);
+      if (xn < box.lo[j]) {
+        xn = box.lo[j];
+        vn = 0.0;
+      }
+      if (xn > box.hi[j]) {
+        xn = box.hi[j];
+        vn = 0.0;
+      }
+      x[gp * D + j] = xn;
+      v[gp * D + j] = vn;
+    }
+  }
+}
+
+// ============================================================================
+// launchers
+// ============================================================================
+int blocks_per_trace(int64_t per, int block) {
+  return (int)((per + block - 1) / block);
+}
+
+int launch_build_stream(const ModelConsts& mc, const double* trace, int n_traces,
+                        double* stream, cudaStream_t st) {
+  int64_t total = (int64_t)n_traces * mc.N;
+  int threads = 256;
+  int64_t blocks = (total + threads - 1) / threads;
+  build_stream_kernel<<<(unsigned)blocks, threads, 0, st>>>(mc, trace, n_traces,
+                                                           stream);
+  return 1;
+}
+
+template <int LAW, int MODE>
+static int launch_integrate_t(const ModelConsts& mc, const IntegrateIO& io,
+                              int block, cudaStream_t st) {
+  const int bpt = blocks_per_trace(io.per, block);
+  const unsigned grid = (unsigned)(bpt * io.n_traces);
+  const size_t smem = (size_t)mc.T * 32 * 2 + 16;
+  auto kern = integrate_misfit_f64<LAW, MODE>;
+  if (smem > 48 * 1024)
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         (int)smem);
+  kern<<<grid, block, smem, st>>>(mc, io, bpt);
+  return 1;
+}
+
+int launch_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block,
+                         cudaStream_t st) {
+#define AFM_DISPATCH(LAWV)                                           \
+  case LAWV:                                                         \
+    return io.mode ? launch_integrate_t<LAWV, 1>(mc, io, block, st)  \
+                   : launch_integrate_t<LAWV, 0>(mc, io, block, st);
+  switch (mc.law) {
+    AFM_DISPATCH(AFM_LAW_NONE)
+    AFM_DISPATCH(AFM_LAW_DMT)
+    AFM_DISPATCH(AFM_LAW_DMT_VISC)
+    AFM_DISPATCH(AFM_LAW_LJ_EXP)
+    default:
+      return -1;
+  }
+#undef AFM_DISPATCH
+}
+
+int launch_trajectory(const ModelConsts& mc, const double* theta_dev,
+                      const double* stream, double z0, double v0, double* zs,
+                      double* vs, cudaStream_t st) {
+  switch (mc.law) {
+    case AFM_LAW_NONE:
+      trajectory_kernel<AFM_LAW_NONE>
+          <<<1, 32, 0, st>>>(mc, theta_dev, stream, z0, v0, zs, vs);
+      break;
+    case AFM_LAW_DMT:
+      trajectory_kernel<AFM_LAW_DMT>
+          <<<1, 32, 0, st>>>(mc, theta_dev, stream, z0, v0, zs, vs);
+      break;
+    case AFM_LAW_DMT_VISC:
+      trajectory_kernel<AFM_LAW_DMT_VISC>
+          <<<1, 32, 0, st>>>(mc, theta_dev, stream, z0, v0, zs, vs);
+      break;
+    case AFM_LAW_LJ_EXP:
+      trajectory_kernel<AFM_LAW_LJ_EXP>
+          <<<1, 32, 0, st>>>(mc, theta_dev, stream, z0, v0, zs, vs);
+      break;
+    default:
+      return -1;
+  }
+  return 1;
+}
+
+int launch_pso_init(const BoxDev& box, int D, int64_t per, int n_traces,
+                    uint64_t seed, double* x, double* v, double* pbest,
+                    double* pbestJ, double* gbest, double* gbestJ,
+                    cudaStream_t st) {
+  const int64_t PT = per * n_traces;
+  const int threads = 128;
+  pso_init_kernel<<<(unsigned)((PT + threads - 1) / threads), threads, 0, st>>>(
+      box, D, per, n_traces, seed, x, v, pbest, pbestJ, gbest, gbestJ);
+  return 1;
+}
+
+int launch_pso_best(int D, int64_t per, int n_traces, const double* J,
+                    const double* x, double* pbest, double* pbestJ, Cand* cand,
+                    int block, cudaStream_t st) {
+  const int bpt = blocks_per_trace(per, block);
+  pso_best_kernel<<<(unsigned)(bpt * n_traces), block, 0, st>>>(
+      D, per, bpt, J, x, pbest, pbestJ, cand);
+  return 1;
+}
+
+int launch_pso_gbest(const BoxDev& box, int D, int n_traces, int n_cand,
+                     const Cand* cand, const double* pbest, double* gbest,
+                     double* gbestJ, double* hist_row, double* theta_star,
+                     double* J_star, cudaStream_t st) {
+  int threads = n_cand <= 32 ? 32 : (n_cand <= 64 ? 64 : 128);
+  pso_gbest_kernel<<<(unsigned)n_traces, threads, 0, st>>>(
+      box, D, n_cand, cand, pbest, gbest, gbestJ, hist_row, theta_star, J_star);
+  return 1;
+}
+
+int launch_pso_move(const BoxDev& box, const SwarmDev& sw, int D, int64_t per,
+                    int n_traces, uint64_t seed, uint32_t it, int do_move,
+                    const double* J, double* x, double* v, const double* pbest,
+                    const double* pbestJ, const double* gbest, double* dump_row,
+                    cudaStream_t st) {
+  const int64_t PT = per * n_traces;
+  const int threads = 128;
+  pso_move_kernel<<<(unsigned)((PT + threads - 1) / threads), threads, 0, st>>>(
+      box, sw, D, per, n_traces, seed, it, do_move, J, x, v, pbest, pbestJ,
+      gbest, dump_row);
+  return 1;
+}
+
+int launch_philox(const uint32_t* ctr, int64_t n, uint32_t k0, uint32_t k1,
+                  uint32_t* out, cudaStream_t st) {
+  const int threads = 128;
+  philox_kernel<<<(unsigned)((n + threads - 1) / threads), threads, 0, st>>>(
+      ctr, n, k0, k1, out);
+  return 1;
+}
+
+}  // namespace afm

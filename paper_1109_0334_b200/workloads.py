@@ -1,6 +1,6 @@
 """Seeded synthetic inputs for the five BASELINE.json configs.
 
-This module is the ONLY code shared by the CPU oracle (oracle/) and the CUDA
+This module is the ONLY code shared by the CPU oracle and the CUDA
 path: it holds workload constants and seeded random draws, and none of the
 method's arithmetic (no ODE, no force law, no misfit, no PSO).  It imports
 neither of them.  numpy only.

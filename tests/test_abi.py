@@ -1,0 +1,114 @@
+"""CPU-side checks of the C-ABI library: it builds for sm_100a, loads, exports
+every symbol include/afm.h declares, validates arguments before touching the
+device, and fails loudly (no CPU fallback) when no GPU is present."""
+import ctypes as C
+import os
+import re
+import subprocess
+
+import numpy as np
+import pytest
+
+from paper_1109_0334_b200 import afm, build, workloads as wlm
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "afm.h")
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return afm.lib()
+
+
+def _declared_functions():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(afm_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_header_functions_are_all_exported(lib):
+    names = _declared_functions()
+    assert len(names) >= 10
+    for n in names:
+        assert hasattr(lib, n), n
+    assert sorted(afm.SYMBOLS) == names
+
+
+def test_struct_layouts_match_the_header():
+    # sizes the C compiler gives the PODs of afm.h
+    code = ('#include <stdio.h>\n#include "afm.h"\nint main(){printf("%zu %zu %zu\\n",'
+            'sizeof(afm_cfg),sizeof(afm_bounds),sizeof(afm_swarm_cfg));return 0;}')
+    exe = os.path.join(ROOT, "_work", "abi_sizes")
+    os.makedirs(os.path.dirname(exe), exist_ok=True)
+    src = exe + ".c"
+    open(src, "w").write(code)
+    subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), src, "-o", exe])
+    sizes = [int(x) for x in subprocess.check_output([exe]).split()]
+    assert sizes == [C.sizeof(afm.Cfg), C.sizeof(afm.Bounds), C.sizeof(afm.SwarmCfg)]
+
+
+def test_library_is_sm100a_and_uses_bulk_async_copy():
+    out = subprocess.check_output(["cuobjdump", "-lelf", afm.LIB_PATH]).decode()
+    assert "sm_100a" in out
+    sass = subprocess.check_output(["cuobjdump", "-sass", afm.LIB_PATH]).decode()
+    assert "UBLKCP" in sass          # cp.async.bulk: the TMA-staged time tiles
+    assert "SYNCS" in sass           # mbarrier
+    assert "MUFU.RCP64H" in sass and "DFMA" in sass
+
+
+def test_validation_happens_before_the_device_is_touched(lib):
+    wl = wlm.config(0)
+    for field, val in (("n_params", 3), ("steps_per_cycle", 0), ("n_skip_cycles", 20),
+                       ("law", 7), ("n_traces", 0), ("k", -1.0), ("precision", 5)):
+        cfg = afm.cfg_from(wl, **{field: val})
+        rc = lib.afm_forward_batch(C.c_void_p(16), 4, C.c_void_p(16), C.byref(cfg), None,
+                                   C.c_void_p(16), None)
+        assert rc == afm.EINVAL, field
+        assert afm.afm_last_error()
+    cfg = afm.cfg_from(wl)
+    assert lib.afm_forward_batch(None, 4, C.c_void_p(16), C.byref(cfg), None,
+                                 C.c_void_p(16), None) == afm.EINVAL
+    assert lib.afm_forward_batch(C.c_void_p(16), 0, C.c_void_p(16), C.byref(cfg), None,
+                                 C.c_void_p(16), None) == afm.EINVAL
+    cfg3 = afm.cfg_from(wl, n_traces=3)
+    assert lib.afm_forward_batch(C.c_void_p(16), 4, C.c_void_p(16), C.byref(cfg3), None,
+                                 C.c_void_p(16), None) == afm.EINVAL
+    b = afm.bounds_from(wl)
+    b.lo[0] = 5.0
+    b.hi[0] = 1.0
+    th = np.zeros(2)
+    rc = lib.afm_pso_invert(C.byref(b), C.byref(afm.swarm_from(wl)), 0, C.c_void_p(16),
+                            C.byref(cfg), th.ctypes.data, th.ctypes.data, None, None, None,
+                            None)
+    assert rc == afm.EINVAL
+    assert afm.afm_set_option("block", 0) is None
+    with pytest.raises(afm.AfmError):
+        afm.afm_set_option("block", 48)
+    with pytest.raises(afm.AfmError):
+        afm.afm_set_option("nonsense", 1)
+
+
+def test_no_cpu_fallback_without_a_gpu(lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    wl = wlm.config(0)
+    cfg = afm.cfg_from(wl)
+    th = np.zeros(2)
+    rc = lib.afm_forward_batch_host(th.ctypes.data, 1, np.zeros(wl["n_window"]).ctypes.data,
+                                    C.byref(cfg), None, th.ctypes.data, None)
+    assert rc in (afm.ECUDA, afm.EUNSUPPORTED)
+    assert "CUDA" in afm.afm_last_error() or "device" in afm.afm_last_error()
+
+
+def test_product_package_never_imports_the_oracle():
+    """The product path shares nothing with oracle/: no import, include, dlopen."""
+    pkg = os.path.join(ROOT, "paper_1109_0334_b200")
+    pat = re.compile(r"import\s+oracle|from\s+oracle|oracle[./]|afm_oracle|orc_[a-z]")
+    for top in (pkg, os.path.join(ROOT, "include")):
+        for dirpath, _, files in os.walk(top):
+            for f in files:
+                if f.endswith((".py", ".cu", ".cuh", ".h")):
+                    text = open(os.path.join(dirpath, f)).read()
+                    assert not pat.search(text), (f, pat.search(text).group(0))

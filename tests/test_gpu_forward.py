@@ -1,0 +1,226 @@
+"""GPU parity: afm_forward_batch / afm_trajectory / afm_philox4x32_10 (through the
+C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerance (BASELINE.json:north_star): per-particle misfit within 1e-9 relative
+in FP64.  The kernel is not an operation-by-operation copy of the oracle (FMA
+contraction, per-step variables, short reciprocal/sqrt sequences), so the two
+differ by accumulated rounding: DESIGN.md "Tolerances" derives ~1e-11.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import binding as orc
+from paper_1109_0334_b200 import workloads as wlm
+from parity_helpers import oracle_trace, rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL_F64 = 1e-9
+KAT = os.path.join(os.path.dirname(__file__), "golden", "philox4x32_10_kat.txt")
+
+
+@pytest.fixture(scope="module")
+def afm():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_1109_0334_b200 import afm as m
+    m.lib()  # fails loudly if the CUDA library is missing
+    yield m
+    m.afm_set_option("block", 0)
+    m.afm_set_option("tile", 0)
+
+
+def _gpu_forward(afm, wl, params, trace, z0v0=None, **cfg_over):
+    import torch
+    cfg = afm.cfg_from(wl, **cfg_over)
+    p = torch.as_tensor(np.ascontiguousarray(params), device="cuda")
+    t = torch.as_tensor(np.ascontiguousarray(trace), device="cuda")
+    zv = None if z0v0 is None else torch.as_tensor(np.ascontiguousarray(z0v0), device="cuda")
+    J = afm.afm_forward_batch(p, t, cfg, z0v0=zv)
+    torch.cuda.synchronize()
+    return J.cpu().numpy()
+
+
+def _oracle_forward(wl, params, trace, z0v0=None):
+    return orc.forward_batch(orc.model_from(wl), params, trace, z0v0=z0v0,
+                             z0=wl["z0"], v0=wl["v0"], n_traces=wl["n_traces"],
+                             openmp=True)
+
+
+def test_philox_known_answers_on_device(afm):
+    rows = [[int(x, 16) for x in l.split()] for l in open(KAT)
+            if l.strip() and not l.startswith("#")]
+    for w in rows:
+        out = afm.afm_philox4x32_10([w[0:4]], w[4:6])
+        assert [int(x) for x in out[0]] == w[6:10]
+
+
+def test_philox_matches_oracle_on_random_counters(afm):
+    rng = np.random.default_rng(5)
+    ctr = rng.integers(0, 2 ** 32, size=(1000, 4), dtype=np.uint64).astype(np.uint32)
+    key = [0x9E3779B9, 0x12345678]
+    out = afm.afm_philox4x32_10(ctr, key)
+    for i in range(0, 1000, 37):
+        assert [int(x) for x in out[i]] == orc.philox4x32_10(ctr[i], key)
+
+
+@pytest.mark.parametrize("cfg_i,law", [(0, None), (0, wlm.LAW_NONE), (2, None), (3, None)])
+def test_trajectory_matches_oracle(afm, cfg_i, law):
+    """Same RK4 states, step by step, for each force law (20 cycles)."""
+    wl = wlm.scaled(wlm.config(cfg_i), n_cycles=20, n_skip_cycles=10)
+    if law is not None:
+        wl = dict(wl, law=law)
+    M = orc.model_from(wl)
+    bad, zs, vs = orc.integrate(M, wl["truth"], wl["z0"], wl["v0"])
+    assert bad == 0
+    gz, gv = afm.afm_trajectory(wl["truth"], afm.cfg_from(wl), wl["z0"], wl["v0"])
+    A0 = wl["cantilever"]["A0"]
+    w = 2 * np.pi * wl["cantilever"]["f_drive"]
+    assert np.max(np.abs(gz - zs)) / A0 < 1e-11
+    assert np.max(np.abs(gv - vs)) / (A0 * w) < 1e-11
+
+
+def test_forward_cfg0_all_particles_ragged(afm):
+    """configs[0] sizes; 100 particles = several CTAs and a ragged tail."""
+    wl = wlm.config(0)
+    trace = oracle_trace(wl)
+    params = wlm.draw_params(wl, 100, seed=11)
+    params[0] = wl["truth"]
+    Jo = _oracle_forward(wl, params, trace)
+    Jg = _gpu_forward(afm, wl, params, trace)
+    assert np.all(np.isfinite(Jo))
+    assert rel_err(Jg, Jo).max() < TOL_F64
+    # J(truth) on a noisy trace ~ W sigma^2 (both sides)
+    assert Jg[0] == pytest.approx(wl["n_window"] * wl["sigma"] ** 2, rel=0.2)
+
+
+@pytest.mark.parametrize("block,tile", [(32, 0), (64, 0), (128, 0), (32, 50), (64, 33)])
+def test_forward_launch_shapes(afm, block, tile):
+    """Every CTA size and odd tile sizes (ragged last tile, window start inside a
+    tile) give the same misfits."""
+    wl = wlm.scaled(wlm.config(0), n_cycles=7, n_skip_cycles=3)
+    trace = oracle_trace(wl)
+    params = wlm.draw_params(wl, 131, seed=12)
+    Jo = _oracle_forward(wl, params, trace)
+    afm.afm_set_option("block", block)
+    afm.afm_set_option("tile", tile)
+    try:
+        Jg = _gpu_forward(afm, wl, params, trace)
+    finally:
+        afm.afm_set_option("block", 0)
+        afm.afm_set_option("tile", 0)
+    assert rel_err(Jg, Jo).max() < TOL_F64
+
+
+def test_forward_cfg1_shape_random_phases(afm):
+    """configs[1] shape (S=256, random initial phases, log-uniform theta) at 40
+    cycles on 2065 particles."""
+    wl = wlm.scaled(wlm.config(1), n_cycles=40, n_skip_cycles=20)
+    trace = oracle_trace(wl)
+    n = 2065
+    params = wlm.draw_params(wl, n, seed=1)
+    z0v0 = wlm.draw_initial_states(wl, n, seed=2)
+    Jo = _oracle_forward(wl, params, trace, z0v0)
+    Jg = _gpu_forward(afm, wl, params, trace, z0v0)
+    e = rel_err(Jg, Jo)
+    assert e.max() < TOL_F64, (e.max(), int(e.argmax()))
+
+
+def test_forward_cfg2_shape_viscoelastic(afm):
+    wl = wlm.scaled(wlm.config(2), n_cycles=30, n_skip_cycles=15)
+    trace = oracle_trace(wl)
+    params = wlm.draw_params(wl, 515, seed=3)
+    Jo = _oracle_forward(wl, params, trace)
+    Jg = _gpu_forward(afm, wl, params, trace)
+    assert rel_err(Jg, Jo).max() < TOL_F64
+
+
+def test_forward_cfg3_shape_lj_exp(afm):
+    wl = wlm.scaled(wlm.config(3), n_cycles=16, n_skip_cycles=8)
+    trace = oracle_trace(wl)
+    params = wlm.draw_params(wl, 300, seed=4)
+    Jo = _oracle_forward(wl, params, trace)
+    Jg = _gpu_forward(afm, wl, params, trace)
+    fin = np.isfinite(Jo)
+    assert np.array_equal(np.isfinite(Jg), fin)
+    assert rel_err(Jg, Jo).max() < TOL_F64
+
+
+def test_forward_cfg4_shape_many_traces(afm):
+    """configs[4] shape: several traces, each with its own segment of particles
+    (70 per trace: ragged CTAs inside every segment)."""
+    wl = wlm.scaled(wlm.config(4), n_cycles=12, n_skip_cycles=6, n_traces=5)
+    truths = wlm.pixel_truths(wl)
+    trace = oracle_trace(wl, truths=truths)
+    per = 70
+    params = wlm.draw_params(wl, per * 5, seed=6)
+    Jo = _oracle_forward(wl, params, trace)
+    Jg = _gpu_forward(afm, wl, params, trace)
+    assert rel_err(Jg, Jo).max() < TOL_F64
+    # the segments really use different traces: swapping two traces changes J
+    Jg2 = _gpu_forward(afm, wl, params, trace[::-1])
+    assert np.abs(Jg2[:per] - Jg[:per]).max() > 0
+
+
+def test_forward_edge_cases(afm):
+    wl = wlm.scaled(wlm.config(0), n_cycles=4, n_skip_cycles=0)   # window = everything
+    trace = oracle_trace(wl)
+    one = np.array([wl["truth"]])
+    assert rel_err(_gpu_forward(afm, wl, one, trace), _oracle_forward(wl, one, trace)).max() < TOL_F64
+    # a single step in total
+    w1 = wlm.scaled(wlm.config(0), steps_per_cycle=1, n_cycles=1, n_skip_cycles=0)
+    tr1 = np.array([[1e-9]])
+    p = wlm.draw_params(w1, 3, seed=1)
+    assert rel_err(_gpu_forward(afm, w1, p, tr1), _oracle_forward(w1, p, tr1)).max() < TOL_F64
+    # noise-free trace of the truth: J(truth) is (numerically) zero
+    clean = oracle_trace(wl, noise=False)
+    J0 = _gpu_forward(afm, wl, one, clean)[0]
+    assert J0 < 1e-12 * wl["n_window"] * wl["cantilever"]["A0"] ** 2
+
+
+def test_forward_divergence_gives_inf(afm):
+    """A trajectory that blows up is +Inf on both sides (reading R12)."""
+    wl = wlm.scaled(wlm.config(3), n_cycles=6, n_skip_cycles=3)
+    wl = dict(wl, cantilever=dict(wl["cantilever"], z_c=15e-9))   # tip driven into the d^-8 wall
+    wl["z0"], wl["v0"] = wlm.config(3)["z0"], wlm.config(3)["v0"]
+    trace = np.zeros((1, wl["n_window"]))
+    params = wlm.draw_params(wl, 64, seed=9)
+    Jo = _oracle_forward(wl, params, trace)
+    Jg = _gpu_forward(afm, wl, params, trace)
+    assert np.isinf(Jo).any()
+    assert np.array_equal(np.isinf(Jg), np.isinf(Jo))
+    assert not np.isnan(Jg).any()
+    assert rel_err(Jg, Jo).max() < 1e-6   # survivors near the wall are ill-conditioned
+
+
+def test_forward_host_entry_matches_device_entry(afm):
+    wl = wlm.scaled(wlm.config(0), n_cycles=6, n_skip_cycles=3)
+    trace = oracle_trace(wl)
+    params = wlm.draw_params(wl, 77, seed=13)
+    Jd = _gpu_forward(afm, wl, params, trace)
+    Jh = afm.afm_forward_batch_host(params, trace, afm.cfg_from(wl))
+    assert np.array_equal(Jd, Jh)
+
+
+def test_bad_arguments_are_rejected(afm):
+    import torch
+    wl = wlm.config(0)
+    cfg = afm.cfg_from(wl)
+    t = torch.zeros(wl["n_window"], dtype=torch.float64, device="cuda")
+    p = torch.zeros((4, 2), dtype=torch.float64, device="cuda")
+    for field, val in (("n_params", 3), ("steps_per_cycle", 0), ("n_skip_cycles", 20),
+                       ("law", 9), ("n_traces", 3), ("Q", 0.0), ("reserved_", 1)):
+        bad = afm.cfg_from(wl, **{field: val})
+        with pytest.raises(afm.AfmError) as ei:
+            afm.lib().afm_forward_batch  # symbol exists
+            from paper_1109_0334_b200.afm import _check, _ptr
+            import ctypes as C
+            _check(afm.lib().afm_forward_batch(_ptr(p), 4, _ptr(t), C.byref(bad), None,
+                                               _ptr(p), None))
+        assert ei.value.code == afm.EINVAL, field
+    assert "n_traces" in afm.afm_last_error() or afm.afm_last_error()
+    J = afm.afm_forward_batch(p + 1e-19, t, cfg)   # a valid call still works afterwards
+    torch.cuda.synchronize()
+    assert J.shape == (4,)
