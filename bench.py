@@ -1,0 +1,373 @@
+#!/usr/bin/env python
+"""bench.py -- RK4 particle-steps/s of the dAFM force-inversion hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--precision f64|f32] [--no-extras]
+
+Workload (config.workload): BASELINE.json configs[1] -- 65,536 DMT parameter sets,
+200 cycles x 256 RK4 steps, random initial phases, misfit over the last 100
+cycles against a 25,600-sample noisy trace.  One "step" is one pass of the whole
+hot path over that batch: afm_forward_batch (a1-a4: parameter map, RK4, misfit)
+followed by afm_pso_step (a5-a7: personal best, global best, Eq. 8 move) on a
+65,536-particle swarm holding the same coordinates.  Inputs are synthetic
+(paper_1109_0334_b200.workloads, seeded), resident in HBM for `value`, and
+start in pinned host memory for `e2e` (afm_forward_batch_host: H2D of theta,
+z0v0 and trace, D2H of the misfits, inside the timed region).
+
+N > 1 (torchrun): every rank runs its own batch of the same shape (different
+seeds); there is no data-path collective; scaling is
+weak; value = all ranks' particle-steps / max-over-ranks time.
+
+--impl reference times the CPU oracle (oracle/, single thread) on a bounded
+sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1109_0334_b200 import workloads as wlm  # noqa: E402
+
+METRIC = "rk4_particle_steps_per_sec"
+UNIT = "particle-steps/s"
+
+# Algorithmic flops per particle-step, SURVEY.md 8(d) / DESIGN.md "Roofline":
+# oracle-form arithmetic, add/mul/compare = 1, FMA = 2, div = sqrt = exp = 1.
+FLOPS_PER_STEP = {wlm.LAW_DMT: 57.0, wlm.LAW_DMT_VISC: 57.0, wlm.LAW_LJ_EXP: 93.0,
+                  wlm.LAW_NONE: 49.0}
+# FP64 FMA peak of the lane model: 148 SMs x 64 lanes x 2 flops x clock
+N_SM, FP64_LANES, FP32_LANES = 148, 64, 128
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    sm_max = 1965.0
+    src = "fallback clock 1965 MHz"
+    if os.path.exists(path):
+        try:
+            sm_max = float(json.load(open(path)).get("sm_max_mhz", sm_max))
+            src = "MEASURED_PEAKS.json sm_max_mhz"
+        except Exception:
+            pass
+    return dict(fp64_tflops=N_SM * FP64_LANES * 2 * sm_max * 1e6 / 1e12,
+                fp32_tflops=N_SM * FP32_LANES * 2 * sm_max * 1e6 / 1e12,
+                clock_mhz=sm_max, clock_source=src)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "50"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+                pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return dict(sm_mhz=float(np.median(sm)) if sm else None,
+                    sm_max_mhz=float(max(mx)) if mx else None,
+                    power_w_max=float(max(pw)) if pw else None,
+                    samples=len(sm), reasons=sorted(reasons))
+
+
+def _oracle_trace(wl):
+    """The oracle's own trace (no oracle input ever comes from the CUDA path)."""
+    from oracle import binding as orc
+    bad, win = orc.window(orc.model_from(wl), wl["truth"], wl["z0"], wl["v0"])
+    return win[None, :] + wlm.trace_noise(wl, n_traces=1)
+
+
+def _oracle_sample(wl, n_sample, seed_params, seed_states, trace):
+    """Time the oracle as it stands (single thread) on n_sample particles."""
+    from oracle import binding as orc
+    M = orc.model_from(wl)
+    params = wlm.draw_params(wl, n_sample, seed=seed_params)
+    z0v0 = wlm.draw_initial_states(wl, n_sample, seed=seed_states)
+    t0 = time.perf_counter()
+    J = orc.forward_batch(M, params, trace, z0v0=z0v0, openmp=False)
+    dt = time.perf_counter() - t0
+    return dt, J
+
+
+def _make_trace(wl):
+    """The measured trace of the GPU arm: built by the GPU path itself from the
+    ground truth + seeded noise (afm_trajectory); nothing here touches oracle/."""
+    from paper_1109_0334_b200 import afm
+    zs, _ = afm.afm_trajectory(wl["truth"], afm.cfg_from(wl, n_traces=1), wl["z0"], wl["v0"])
+    clean = zs[-wl["n_window"]:]
+    return clean[None, :] + wlm.trace_noise(wl, n_traces=1)
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on a bounded sample of configs[1]."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from oracle import binding as orc
+    wl = wlm.config(1)
+    trace = _oracle_trace(wl)
+    n_sample = args.ref_particles
+    for _ in range(args.warmup):
+        _oracle_sample(wl, 4, 1, 2, trace)
+    times = []
+    for _ in range(args.steps):
+        dt, _ = _oracle_sample(wl, n_sample, 1, 2, trace)
+        times.append(dt)
+    total = float(sum(times))
+    value = n_sample * wl["n_steps"] * args.steps / total
+    sample = "%d of 65536 particles x %d RK4 steps per step, single thread" % (
+        n_sample, wl["n_steps"])
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[1] forward batch, DMT, FP64 (bounded sample)",
+                   "particles_per_step": n_sample, "rk4_steps": wl["n_steps"]},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": sample, "host_cores": os.cpu_count()},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0,
+                "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1109_0334_b200 import afm
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    afm.lib()
+    prec = afm.F32 if args.precision == "f32" else afm.F64
+
+    wl = wlm.config(1)
+    P = wl["swarm"]["n_particles"]
+    D = wl["n_params"]
+    N = wl["n_steps"]
+    cfg = afm.cfg_from(wl, precision=prec)
+    trace_np = _make_trace(wl)
+    coords_np = wlm.draw_coords(wl, P, seed=1 + 100 * rank)
+    params_np = wlm.theta_of_coords(wl, coords_np)
+    z0v0_np = wlm.draw_initial_states(wl, P, seed=2 + 100 * rank)
+
+    dev = torch.device("cuda", local)
+    params = torch.as_tensor(params_np, device=dev)
+    trace = torch.as_tensor(trace_np, device=dev)
+    z0v0 = torch.as_tensor(z0v0_np, device=dev)
+    misfit = torch.empty(P, dtype=torch.float64, device=dev)
+    bounds = afm.bounds_from(wl)
+    swarm = afm.swarm_from(wl)
+    state = afm.afm_pso_init(bounds, swarm, D, 1, wl["pso_seed"])
+    state["x"].copy_(torch.as_tensor(coords_np, device=dev))
+    state["pbest"].copy_(state["x"])
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)  # > 126 MB L2
+
+    def step(it):
+        afm.afm_forward_batch(params, trace, cfg, z0v0=z0v0, misfit=misfit)
+        afm.afm_pso_step(bounds, swarm, D, 1, wl["pso_seed"], it, True, misfit, state)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for i in range(args.warmup):
+        step(i)
+    barrier()
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True),
+           torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    afm.afm_reset_launch_count()
+    barrier()
+    for i in range(args.steps):
+        flush.zero_()                      # L2 flush between timed iterations (untimed)
+        ev[i][0].record()
+        afm.afm_forward_batch(params, trace, cfg, z0v0=z0v0, misfit=misfit)
+        ev[i][1].record()
+        afm.afm_pso_step(bounds, swarm, D, 1, wl["pso_seed"], args.warmup + i, True,
+                         misfit, state)
+        ev[i][2].record()
+    barrier()
+    launches = afm.afm_launch_count()
+    step_ms = [e[0].elapsed_time(e[2]) for e in ev]
+    fwd_ms = [e[0].elapsed_time(e[1]) for e in ev]
+    total_ms = float(sum(step_ms))
+    clocks = sampler.stop() if sampler else None
+
+    # ---- e2e: host buffers in, host misfits out, through the C ABI ----------
+    h_params = torch.as_tensor(params_np).pin_memory()
+    h_trace = torch.as_tensor(trace_np).pin_memory()
+    h_z0v0 = torch.as_tensor(z0v0_np).pin_memory()
+    h_out = torch.empty(P, dtype=torch.float64).pin_memory()
+    hp, ht, hz, ho = (h_params.numpy(), h_trace.numpy(), h_z0v0.numpy(), h_out.numpy())
+    afm.afm_forward_batch_host(hp, ht, cfg, z0v0=hz, misfit=ho)
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        afm.afm_forward_batch_host(hp, ht, cfg, z0v0=hz, misfit=ho)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    finite = int(np.isfinite(ho).sum())
+
+    t = torch.tensor([total_ms, e2e_s * 1e3, float(sum(fwd_ms))], dtype=torch.float64,
+                     device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms, e2e_ms, fwd_total_ms = [float(x) for x in t.cpu()]
+
+    units = float(P) * N * args.steps * world
+    value = units / (total_ms * 1e-3)
+    e2e_value = units / (e2e_ms * 1e-3)
+
+    if rank == 0:
+        pk = _peaks()
+        kern_ms = fwd_total_ms / args.steps
+        flops = FLOPS_PER_STEP[wl["law"]] * P * N
+        achieved = flops / (kern_ms * 1e-3) / 1e12
+        peak = pk["fp32_tflops"] if prec == afm.F32 else pk["fp64_tflops"]
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if prec == afm.F32 else "f64", "data": "synthetic",
+            "config": {"workload": "configs[1]: 65536 DMT theta x 200 cycles x 256 RK4 "
+                                   "steps, misfit over last 100 cycles (per GPU)",
+                       "particles_per_gpu": P, "rk4_steps": N, "window": wl["n_window"],
+                       "step": "afm_forward_batch + afm_pso_step",
+                       "l2": "256 MB buffer zeroed between timed iterations"},
+            "e2e": {"value": e2e_value, "unit": UNIT,
+                    "h2d_bytes_per_step": int(hp.nbytes + ht.nbytes + hz.nbytes),
+                    "d2h_bytes_per_step": int(ho.nbytes),
+                    "api": "afm_forward_batch_host", "finite_misfits": finite},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "roofline": {"bound": "alu", "kernel": "integrate_misfit_%s" % args.precision,
+                         "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                         "frac": achieved / peak, "traffic": None,
+                         "flops_per_particle_step": FLOPS_PER_STEP[wl["law"]],
+                         "kernel_ms": kern_ms,
+                         "peak_source": "lane model 148 SM x %d lanes x 2 x %s (%s)" % (
+                             FP32_LANES if prec == afm.F32 else FP64_LANES,
+                             pk["clock_mhz"], pk["clock_source"])},
+        }
+        if not args.no_extras and world == 1:
+            out["extras"] = extras(afm, torch, dev)
+            n_s = args.cpu_particles
+            dt, _ = _oracle_sample(wl, n_s, 1, 2, _oracle_trace(wl))
+            out["cpu_baseline"] = {
+                "value": n_s * N / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+                "sample": "%d of 65536 particles x %d RK4 steps, single thread, %.1f s"
+                          % (n_s, N, dt),
+                "host_cores": os.cpu_count()}
+        print(json.dumps(out))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def extras(afm, torch, dev):
+    """Secondary figures of BASELINE.json:metric: forward-batch latency and
+    inversion wall time (host clock, call to return) of configs[0] and [2]."""
+    ex = {}
+    for ci in (0, 2):
+        wl = wlm.config(ci)
+        cfg = afm.cfg_from(wl)
+        zs, _ = afm.afm_trajectory(wl["truth"], cfg, wl["z0"], wl["v0"])
+        trace = torch.as_tensor(zs[-wl["n_window"]:][None, :] + wlm.trace_noise(wl),
+                                device=dev)
+        b, s = afm.bounds_from(wl), afm.swarm_from(wl)
+        afm.afm_pso_invert(b, s, wl["pso_seed"], trace, cfg)       # warm-up
+        t0 = time.perf_counter()
+        r = afm.afm_pso_invert(b, s, wl["pso_seed"], trace, cfg)
+        ms = (time.perf_counter() - t0) * 1e3
+        units = wl["swarm"]["n_particles"] * wl["swarm"]["n_iters"] * wl["n_steps"]
+        ex["cfg%d_inversion_ms" % ci] = ms
+        ex["cfg%d_particle_steps_per_s" % ci] = units / (ms * 1e-3)
+        ex["cfg%d_theta_star_rel_err_vs_truth" % ci] = [
+            float(abs(a - t) / abs(t)) for a, t in zip(r["theta_star"][0], wl["truth"])]
+    return ex
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--cpu-particles", type=int, default=3072,
+                    help="oracle sample size of the cpu_baseline leg")
+    ap.add_argument("--ref-particles", type=int, default=512,
+                    help="oracle sample size per step of --impl reference")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

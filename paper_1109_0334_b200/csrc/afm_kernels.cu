@@ -216,9 +216,11 @@ __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
   double d = z0 + mc.zc;
   double w = v0 * mc.h;
   double J = 0.0;
+  const long long a0_bits = __double_as_longlong(mc.a0);
   const long long key_max = order_key(mc.d_max);
   const long long key_min = order_key(mc.d_min);
   bool bad = false;
+  int mode = 0;  // warp-uniform: 0 = speculate free flight, 1 = general
 
   // ---- a2-a4: RK4 over the time tiles -------------------------------------
   for (int tile = 0; tile < mc.n_tiles; ++tile) {
@@ -229,20 +231,15 @@ __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
     const int n_steps = min(mc.T, mc.N - n_begin);
     // steps [0, k0) of this tile precede the misfit window
     const int k0 = max(0, min(n_steps, mc.n0 - n_begin));
-    int i = 0;
-    for (; i < k0; ++i) {
+    for (int i = 0; i < n_steps; ++i) {
       const double4 r = sp[i];
-      rk4_step<LAW>(P, r.x, r.y, r.z, d, w);
+      rk4_step<LAW>(P, r.x, r.y, r.z, a0_bits, d, w, mode);
       const long long key = order_key(d);
       bad |= (key > key_max) | (key < key_min);
-    }
-    for (; i < n_steps; ++i) {
-      const double4 r = sp[i];
-      rk4_step<LAW>(P, r.x, r.y, r.z, d, w);
-      const long long key = order_key(d);
-      bad |= (key > key_max) | (key < key_min);
-      const double res = d - r.w;
-      J = fma(res, res, J);
+      if (i >= k0) {  // warp-uniform: inside the misfit window
+        const double res = d - r.w;
+        J = fma(res, res, J);
+      }
     }
     __syncthreads();  // every thread is done reading stage st
     if (tid == 0 && tile + 2 < mc.n_tiles) {
@@ -291,22 +288,26 @@ __global__ void trajectory_kernel(ModelConsts mc, const double* __restrict__ th,
                                   const double* __restrict__ stream, double z0,
                                   double v0, double* __restrict__ zs,
                                   double* __restrict__ vs) {
-  if (blockIdx.x != 0 || threadIdx.x != 0) return;
+  // one warp, every lane integrates the same particle (rk4_step votes across
+  // the full warp); lane 0 writes
+  const bool writer = (threadIdx.x == 0);
   double t4[4] = {0.0, 0.0, 0.0, 0.0};
   for (int j = 0; j < mc.D && j < 4; ++j) t4[j] = th[j];
   Particle64 P;
   load_particle(P, LAW, t4, mc.alpha, mc.beta, mc.a0, mc.inv_a0sq, mc.c_vdw,
                 mc.c_hertz, mc.c_visc, mc.c_force);
   double d = z0 + mc.zc, w = v0 * mc.h;
+  const long long a0_bits = __double_as_longlong(mc.a0);
   const double inv_h = 1.0 / mc.h;
-  if (zs) zs[0] = z0;
-  if (vs) vs[0] = v0;
+  int mode = 0;
+  if (zs && writer) zs[0] = z0;
+  if (vs && writer) vs[0] = v0;
   const double4* rows = reinterpret_cast<const double4*>(stream);
   for (int n = 0; n < mc.N; ++n) {
     const double4 r = rows[n];
-    rk4_step<LAW>(P, r.x, r.y, r.z, d, w);
-    if (zs) zs[n + 1] = d - mc.zc;
-    if (vs) vs[n + 1] = w * inv_h;
+    rk4_step<LAW>(P, r.x, r.y, r.z, a0_bits, d, w, mode);
+    if (zs && writer) zs[n + 1] = d - mc.zc;
+    if (vs && writer) vs[n + 1] = w * inv_h;
   }
 }
 

@@ -181,18 +181,24 @@ def test_forward_edge_cases(afm):
 
 
 def test_forward_divergence_gives_inf(afm):
-    """A trajectory that blows up is +Inf on both sides (reading R12)."""
-    wl = wlm.scaled(wlm.config(3), n_cycles=6, n_skip_cycles=3)
-    wl = dict(wl, cantilever=dict(wl["cantilever"], z_c=15e-9))   # tip driven into the d^-8 wall
-    wl["z0"], wl["v0"] = wlm.config(3)["z0"], wlm.config(3)["v0"]
-    trace = np.zeros((1, wl["n_window"]))
-    params = wlm.draw_params(wl, 64, seed=9)
+    """A trajectory that blows up is +Inf on both sides (reading R12).  Particles
+    at the edge of blowing up are ill-conditioned: they are compared only where
+    the oracle's own verdict survives a 1e-13 relative change of theta
+    (SURVEY.md 8(c) c-15 protocol)."""
+    base = wlm.scaled(wlm.config(3), n_cycles=6, n_skip_cycles=3)
+    trace = np.zeros((1, base["n_window"]))
+    params = wlm.draw_params(base, 64, seed=9)
+    # tip driven into the d^-8 wall: most diverge, some survive
+    wl = dict(base, cantilever=dict(base["cantilever"], z_c=15e-9))
     Jo = _oracle_forward(wl, params, trace)
+    Jo2 = _oracle_forward(wl, params * (1 + 1e-13), trace)
     Jg = _gpu_forward(afm, wl, params, trace)
-    assert np.isinf(Jo).any()
-    assert np.array_equal(np.isinf(Jg), np.isinf(Jo))
+    assert np.isinf(Jo).any() and np.isfinite(Jo).any()
     assert not np.isnan(Jg).any()
-    assert rel_err(Jg, Jo).max() < 1e-6   # survivors near the wall are ill-conditioned
+    robust = (np.isinf(Jo) == np.isinf(Jo2)) & (rel_err(Jo2, Jo) < 1e-12)
+    assert robust.sum() > 32 and np.isinf(Jo[robust]).sum() > 8
+    assert np.array_equal(np.isinf(Jg)[robust], np.isinf(Jo)[robust])
+    assert rel_err(Jg, Jo)[robust].max() < TOL_F64
 
 
 def test_forward_host_entry_matches_device_entry(afm):
