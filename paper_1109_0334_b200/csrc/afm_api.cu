@@ -52,6 +52,7 @@ int fail(int code, const char* fmt, ...) {
 // ---- options -----------------------------------------------------------------
 int g_opt_block = 0;  // 0 = auto
 int g_opt_tile = 0;   // 0 = auto
+int g_opt_ppt = 0;    // 0 = auto
 
 // ---- grow-only device workspace ------------------------------------------------
 struct Buffer {
@@ -199,6 +200,7 @@ void make_consts(const afm_cfg* c, int block, ModelConsts* mc) {
   mc->c_force = h * h / m;
   mc->d_max = c->z_c + 100.0 * c->A0;
   mc->d_min = c->z_c - 100.0 * c->A0;
+  mc->d_safe = fmax(0.0, 100.0 * c->A0 - fabs(c->z_c));
   mc->z0 = c->z0;
   mc->v0 = c->v0;
   mc->law = c->law;
@@ -217,6 +219,18 @@ int pick_block(int64_t per, int n_traces) {
   (void)per;
   (void)n_traces;
   return 32;
+}
+
+// Particles per thread: two interleaved chains once the batch would put at
+// least two one-particle warps on every SM sub-partition (148 x 4 of them).
+int pick_ppt(int64_t per, int n_traces) {
+  if (g_opt_ppt > 0) return g_opt_ppt;
+  // measured on B200: with >= 3 warps per SM
+  // sub-partition the issue port is already the limit and a second chain per
+  // thread only lowers the free-flight hit rate, so one particle per thread
+  (void)per;
+  (void)n_traces;
+  return 1;
 }
 
 BoxDev make_box(const afm_bounds* b, int D) {
@@ -256,6 +270,7 @@ int forward_locked(const double* params, int64_t P, const double* trace,
     return fail(AFM_EUNSUPPORTED, "FP32 integrate kernel not built yet");
   const int64_t per = P / cfg->n_traces;
   const int block = pick_block(per, cfg->n_traces);
+  const int ppt = pick_ppt(per, cfg->n_traces);
   ModelConsts mc;
   make_consts(cfg, block, &mc);
   int rc = acquire_ws(st);
@@ -275,7 +290,7 @@ int forward_locked(const double* params, int64_t P, const double* trace,
   io.per = per;
   io.n_traces = cfg->n_traces;
   io.mode = 0;
-  LAUNCHED(launch_integrate_f64(mc, io, block, st));
+  LAUNCHED(launch_integrate_f64(mc, io, block, ppt, st));
   return release_ws(st);
 }
 
@@ -411,7 +426,8 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
   const int64_t per = swarm->n_particles;
   const int64_t PT = per * T;
   const int block = pick_block(per, T);
-  const int bpt = blocks_per_trace(per, block);
+  const int ppt = pick_ppt(per, T);
+  const int bpt = blocks_per_trace(per, block * ppt);
   ModelConsts mc;
   make_consts(cfg, block, &mc);
   int rc = acquire_ws(st);
@@ -458,7 +474,7 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
   int done = 0;
   for (int it = 0; it < swarm->n_iters; ++it) {
     const bool last = (it == swarm->n_iters - 1);
-    LAUNCHED(launch_integrate_f64(mc, io, block, st));
+    LAUNCHED(launch_integrate_f64(mc, io, block, ppt, st));
     LAUNCHED(launch_pso_gbest(
         box, D, T, bpt, (Cand*)g_ws.cand.p, pbest, gbest, gbestJ,
         gbest_hist ? gbest_hist + (size_t)it * T * (D + 1) : nullptr, th_dev,
@@ -587,6 +603,11 @@ int afm_set_option(const char* name, int64_t value) {
     if (value != 0 && value != 32 && value != 64 && value != 128)
       return fail(AFM_EINVAL, "block must be 0, 32, 64 or 128");
     g_opt_block = (int)value;
+    return AFM_OK;
+  }
+  if (!strcmp(name, "ppt")) {
+    if (value < 0 || value > 2) return fail(AFM_EINVAL, "ppt must be 0, 1 or 2");
+    g_opt_ppt = (int)value;
     return AFM_OK;
   }
   if (!strcmp(name, "tile")) {

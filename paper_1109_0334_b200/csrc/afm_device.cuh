@@ -114,81 +114,62 @@ __device__ __forceinline__ bool ge_pos(double d, long long a0_bits) {
   return __double_as_longlong(d) >= a0_bits;
 }
 
-// g(s, d, w): the acceleration term in per-step variables.
-template <int LAW>
-__device__ __forceinline__ double accel(const Particle64& P, double s, double d,
-                                        double w, long long a0_bits) {
-  double base = fma(P.nbeta, d, fma(P.nalpha, w, s));
-  if (LAW == AFM_LAW_NONE) {
-    return base;
-  } else if (LAW == AFM_LAW_DMT || LAW == AFM_LAW_DMT_VISC) {
-    // at d == a0 both branches give -kappa/a0^2 (the law is continuous), so
-    // the contact branch only ever sees a0 - d > 0.
-    if (ge_pos(d, a0_bits)) {
-      double r = rcp_fast(d * d);
-      return fma(P.c0, r, base);
-    } else {
-      double del = P.a0 - d;
-      double sq = sqrt_fast(del);
-      double f = fma(P.c1 * del, sq, P.c2);
-      if (LAW == AFM_LAW_DMT_VISC) f = fma(P.c3 * sq, w, f);
-      return base + f;
-    }
-  } else {  // AFM_LAW_LJ_EXP
-    double r = rcp_fast(d * d);
-    double r2 = r * r;
-    double r4 = r2 * r2;
-    double f = fma(P.c0, r4, P.c1 * r);
-    double ex = exp(d * P.c3);
-    f = fma(P.c2, ex, f);
-    return base + f;
-  }
-}
+// g(s, d, w) = s - alpha w - beta d + f(d, w): the acceleration term in
+// per-step variables.  The stage velocity w is the last operand to arrive, so
+// everything else is folded first and w enters through one final FMA.
 
-// The same term on the free-flight (d >= a0) side of the DMT laws, no branch.
+// Free-flight (d >= a0) side of the DMT laws, and the whole of law NONE when
+// c0 = 0 is skipped by the caller.
 __device__ __forceinline__ double accel_free(const Particle64& P, double s,
                                              double d, double w) {
-  double base = fma(P.nbeta, d, fma(P.nalpha, w, s));
-  return fma(P.c0, rcp_fast(d * d), base);
+  const double part = fma(P.c0, rcp_fast(d * d), fma(P.nbeta, d, s));
+  return fma(P.nalpha, w, part);
 }
 
 // DMT laws, both sides evaluated and selected per lane (straight-line code: the
 // reciprocal and the square-root chains overlap).  A lane on the other side
 // feeds its unused chain a harmless argument (rsqrt of a negative number is NaN
-// and is never selected).
+// and is never selected).  The free-flight value is computed exactly as in
+// accel_free, so a lane's result does not depend on which form ran.
 template <int LAW>
 __device__ __forceinline__ double accel_both(const Particle64& P, double s,
                                              double d, double w,
                                              long long a0_bits) {
-  const double base = fma(P.nbeta, d, fma(P.nalpha, w, s));
-  const double g_free = fma(P.c0, rcp_fast(d * d), base);
+  const double b0 = fma(P.nbeta, d, s);
+  const double g_free = fma(P.nalpha, w, fma(P.c0, rcp_fast(d * d), b0));
   const double del = P.a0 - d;
   const double sq = sqrt_fast(del);
-  double f = fma(P.c1 * del, sq, P.c2);
-  if (LAW == AFM_LAW_DMT_VISC) f = fma(P.c3 * sq, w, f);
-  const double g_contact = base + f;
+  const double part = fma(P.c1 * del, sq, P.c2 + b0);
+  // viscous term -nu sqrt(delta) w joins the -alpha w term: one coefficient
+  const double cw = (LAW == AFM_LAW_DMT_VISC) ? fma(P.c3, sq, P.nalpha) : P.nalpha;
+  const double g_contact = fma(cw, w, part);
   return ge_pos(d, a0_bits) ? g_free : g_contact;
 }
 
-// Stage acceleration with a warp-uniform choice of code: all lanes in free
-// flight -> the short form; otherwise both sides + select.  `touched` records
-// (warp-uniformly) that some lane was in contact.
+// Laws without a contact switch.
 template <int LAW>
-__device__ __forceinline__ double accel_warp(const Particle64& P, double s,
-                                             double d, double w,
-                                             long long a0_bits, bool& touched) {
-  if (LAW == AFM_LAW_DMT || LAW == AFM_LAW_DMT_VISC) {
-    if (__all_sync(0xffffffffu, ge_pos(d, a0_bits))) return accel_free(P, s, d, w);
-    touched = true;
-    return accel_both<LAW>(P, s, d, w, a0_bits);
-  } else {
-    return accel<LAW>(P, s, d, w, a0_bits);
+__device__ __forceinline__ double accel_smooth(const Particle64& P, double s,
+                                               double d, double w) {
+  const double b0 = fma(P.nbeta, d, s);
+  if (LAW == AFM_LAW_LJ_EXP) {
+    const double r = rcp_fast(d * d);
+    const double r2 = r * r;
+    const double r4 = r2 * r2;
+    double f = fma(P.c0, r4, fma(P.c1, r, b0));
+    f = fma(P.c2, exp(d * P.c3), f);
+    return fma(P.nalpha, w, f);
   }
+  return fma(P.nalpha, w, b0);  // AFM_LAW_NONE
 }
 
+template <int LAW>
+struct IsDmt {
+  static constexpr bool value = (LAW == AFM_LAW_DMT || LAW == AFM_LAW_DMT_VISC);
+};
+
 // One classical RK4 step (tableau c = (0, 1/2, 1/2, 1),
-// b = (1/6, 1/3, 1/3, 1/6)) of unit length in per-step variables.  With
-// k_jd = stage velocity and k_j = stage acceleration:
+// b = (1/6, 1/3, 1/3, 1/6)) of unit length in per-step variables, for the PPT
+// particles of one thread.  With k_jd = stage velocity, k_j = stage acceleration:
 //   k_1d = w, k_2d = w + k1/2, k_3d = w + k2/2, k_4d = w + k3
 //   d' = d + (k_1d + 2 k_2d + 2 k_3d + k_4d)/6 = d + w + (k1 + k2 + k3)/6
 //   w' = w + (k1 + 2 k2 + 2 k3 + k4)/6
@@ -199,61 +180,129 @@ __device__ __forceinline__ double accel_warp(const Particle64& P, double s,
 // position does not depend on stage 1's force, stage 4's not on stage 3's).
 // `mode` is a warp-uniform state: in mode 0 the step is first taken
 // speculatively on the free-flight side and kept only if every stage position
-// of every lane of the warp really was >= a0 (tested on the high words:
+// of every particle of the warp really was >= a0 (tested on the high words:
 // conservative by < 2^-20 relative; the exact test lives in the general path);
 // a failed speculation redoes the step in the general form and switches to
 // mode 1, which skips the speculation until a whole step passes without
-// contact.  Every path evaluates the same arithmetic for a given lane and
-// stage, so which path ran never changes a result.
-template <int LAW>
-__device__ __forceinline__ void rk4_step(const Particle64& P, double s0,
-                                         double sh, double s1,
-                                         long long a0_bits, double& d,
-                                         double& w, int& mode) {
-  const double sixth = 1.0 / 6.0;
-  const double dw = d + w;
-  const double d2 = fma(0.5, w, d);
-  if ((LAW == AFM_LAW_DMT || LAW == AFM_LAW_DMT_VISC) && mode == 0) {
-    const double k1 = accel_free(P, s0, d, w);
-    const double w2 = fma(0.5, k1, w);
-    const double k2 = accel_free(P, sh, d2, w2);
-    const double w3 = fma(0.5, k2, w);
-    const double d3 = fma(0.5, w2, d);
-    const double k3 = accel_free(P, sh, d3, w3);
-    const double d4 = d + w3;
-    const double k4 = accel_free(P, s1, d4, w + k3);
-    const int a0_hi = (int)(a0_bits >> 32);
-    const int m = min(min(__double2hiint(d), __double2hiint(d2)),
-                      min(__double2hiint(d3), __double2hiint(d4)));
-    if (__all_sync(0xffffffffu, m > a0_hi)) {
-      const double t23 = k2 + k3;
-      const double s3 = k1 + t23;
-      d = fma(s3, sixth, dw);
-      w = fma((s3 + t23) + k4, sixth, w);
-      return;
-    }
-    mode = 1;
-  }
-  bool touched = false;
-  const double k1 = accel_warp<LAW>(P, s0, d, w, a0_bits, touched);
-  const double w2 = fma(0.5, k1, w);
-  const double k2 = accel_warp<LAW>(P, sh, d2, w2, a0_bits, touched);
-  const double w3 = fma(0.5, k2, w);
-  const double k3 = accel_warp<LAW>(P, sh, fma(0.5, w2, d), w3, a0_bits, touched);
-  const double k4 = accel_warp<LAW>(P, s1, d + w3, w + k3, a0_bits, touched);
-  const double t23 = k2 + k3;
-  const double s3 = k1 + t23;
-  d = fma(s3, sixth, dw);
-  w = fma((s3 + t23) + k4, sixth, w);
-  if (!touched) mode = 0;
-}
-
+// contact.  The general form evaluates both sides of the law in every stage
+// and selects per lane.  A given particle and stage sees the same arithmetic
+// whichever path ran, so the path never changes a result.
 // Monotone integer key of a double (total order equal to the numeric order
 // for non-NaN; +NaN above +Inf, -NaN below -Inf), for the divergence test on
 // the ALU pipe instead of two FP64 compares.
 __device__ __forceinline__ long long order_key(double x) {
   long long b = __double_as_longlong(x);
   return b ^ ((b >> 63) & 0x7fffffffffffffffLL);
+}
+
+// Divergence rule R12 on d = z + z_c, every step: |z| > 100 A0 or non-finite.
+// Cheap sound filter first (ALU pipe, high word only): |d| below the double
+// whose high word is `safe_hi` implies |z| <= 100 A0; only a suspect value
+// takes the exact two-sided test.
+struct DivergeTest {
+  long long key_min, key_max;  // order_key(z_c -+ 100 A0)
+  int safe_hi;                 // high word of max(0, 100 A0 - |z_c|)
+};
+__device__ __forceinline__ bool diverged_step(double d, const DivergeTest& T) {
+  const int hi = __double2hiint(d) & 0x7fffffff;
+  if (__builtin_expect(hi >= T.safe_hi, 0)) {
+    const long long key = order_key(d);
+    return (key > T.key_max) | (key < T.key_min);
+  }
+  return false;
+}
+
+template <int LAW, int PPT>
+__device__ __forceinline__ void rk4_step(const Particle64 (&P)[PPT], double s0,
+                                         double sh, double s1,
+                                         long long a0_bits, double (&d)[PPT],
+                                         double (&w)[PPT], int& mode,
+                                         bool (&bad)[PPT],
+                                         const DivergeTest& T) {
+  const double sixth = 1.0 / 6.0;
+  double dw[PPT], d2[PPT];
+#pragma unroll
+  for (int q = 0; q < PPT; ++q) {
+    dw[q] = d[q] + w[q];
+    d2[q] = fma(0.5, w[q], d[q]);
+  }
+  if (!IsDmt<LAW>::value) {
+#pragma unroll
+    for (int q = 0; q < PPT; ++q) {
+      const double k1 = accel_smooth<LAW>(P[q], s0, d[q], w[q]);
+      const double w2 = fma(0.5, k1, w[q]);
+      const double k2 = accel_smooth<LAW>(P[q], sh, d2[q], w2);
+      const double w3 = fma(0.5, k2, w[q]);
+      const double k3 = accel_smooth<LAW>(P[q], sh, fma(0.5, w2, d[q]), w3);
+      const double k4 = accel_smooth<LAW>(P[q], s1, d[q] + w3, w[q] + k3);
+      const double t23 = k2 + k3;
+      const double s3 = k1 + t23;
+      d[q] = fma(s3, sixth, dw[q]);
+      w[q] = fma((s3 + t23) + k4, sixth, w[q]);
+      bad[q] |= diverged_step(d[q], T);
+    }
+    return;
+  }
+  if (mode == 0) {
+    double dn[PPT], wn[PPT];
+    int m = 0x7fffffff;
+    unsigned hmax = 0u;
+#pragma unroll
+    for (int q = 0; q < PPT; ++q) {
+      const double k1 = accel_free(P[q], s0, d[q], w[q]);
+      const double w2 = fma(0.5, k1, w[q]);
+      const double k2 = accel_free(P[q], sh, d2[q], w2);
+      const double w3 = fma(0.5, k2, w[q]);
+      const double d3 = fma(0.5, w2, d[q]);
+      const double k3 = accel_free(P[q], sh, d3, w3);
+      const double d4 = d[q] + w3;
+      const double k4 = accel_free(P[q], s1, d4, w[q] + k3);
+      m = min(m, min(min(__double2hiint(d[q]), __double2hiint(d2[q])),
+                     min(__double2hiint(d3), __double2hiint(d4))));
+      const double t23 = k2 + k3;
+      const double s3 = k1 + t23;
+      dn[q] = fma(s3, sixth, dw[q]);
+      wn[q] = fma((s3 + t23) + k4, sixth, w[q]);
+      hmax = max(hmax, (unsigned)__double2hiint(dn[q]));
+    }
+    // kept only if no stage touched the sample and the new gap is a positive
+    // number below the divergence filter (unsigned compare: a negative or NaN
+    // high word is huge) -- so a kept step needs no divergence test
+    if (__all_sync(0xffffffffu, (m > (int)(a0_bits >> 32)) &
+                                    (hmax < (unsigned)T.safe_hi))) {
+#pragma unroll
+      for (int q = 0; q < PPT; ++q) {
+        d[q] = dn[q];
+        w[q] = wn[q];
+      }
+      return;
+    }
+    mode = 1;
+  }
+  // general form: every stage evaluates both sides of the law and selects per
+  // lane -- straight-line code, no vote between the stages, so the four
+  // reciprocal and four square-root chains overlap like in the fast form
+  int m = 0x7fffffff;
+#pragma unroll
+  for (int q = 0; q < PPT; ++q) {
+    const double k1 = accel_both<LAW>(P[q], s0, d[q], w[q], a0_bits);
+    const double w2 = fma(0.5, k1, w[q]);
+    const double k2 = accel_both<LAW>(P[q], sh, d2[q], w2, a0_bits);
+    const double w3 = fma(0.5, k2, w[q]);
+    const double d3 = fma(0.5, w2, d[q]);
+    const double k3 = accel_both<LAW>(P[q], sh, d3, w3, a0_bits);
+    const double d4 = d[q] + w3;
+    const double k4 = accel_both<LAW>(P[q], s1, d4, w[q] + k3, a0_bits);
+    m = min(m, min(min(__double2hiint(d[q]), __double2hiint(d2[q])),
+                   min(__double2hiint(d3), __double2hiint(d4))));
+    const double t23 = k2 + k3;
+    const double s3 = k1 + t23;
+    d[q] = fma(s3, sixth, dw[q]);
+    w[q] = fma((s3 + t23) + k4, sixth, w[q]);
+    bad[q] |= diverged_step(d[q], T);
+  }
+  // back to speculation once a whole step stayed clear of the sample
+  if (__all_sync(0xffffffffu, m > (int)(a0_bits >> 32))) mode = 0;
 }
 
 // Scaled law coefficients from physical parameters theta.

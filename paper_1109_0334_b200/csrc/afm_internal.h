@@ -31,6 +31,7 @@ struct ModelConsts {
   double c_force;    // h^2 / m
   double d_max;      // z_c + 100 A0   (divergence rule R12 on d)
   double d_min;      // z_c - 100 A0   (negative)
+  double d_safe;     // max(0, 100 A0 - |z_c|): |d| < d_safe => not diverged
   double z0, v0;     // default initial state, SI
   int32_t law, D;
   int32_t N;         // total steps
@@ -97,7 +98,7 @@ int launch_build_stream_f32(const ModelConsts& mc, const ModelConstsF32& mf,
                             const double* trace, int n_traces, float* stream,
                             cudaStream_t st);
 int launch_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block,
-                         cudaStream_t st);
+                         int ppt, cudaStream_t st);
 int launch_integrate_f32(const ModelConsts& mc, const ModelConstsF32& mf,
                          const IntegrateIO& io, int block, cudaStream_t st);
 int launch_trajectory(const ModelConsts& mc, const double* theta_dev,

@@ -152,7 +152,38 @@ __device__ __forceinline__ void block_argmin(double& J, long long& idx,
   }
 }
 
-template <int LAW, int MODE>
+// T steps of one time tile, [i0, i1), with (WIN) or without the misfit sum.
+template <int LAW, int PPT, bool WIN>
+__device__ __forceinline__ void run_steps(const double4* sp, int i0, int i1,
+                                          const Particle64 (&P)[PPT],
+                                          long long a0_bits,
+                                          const DivergeTest& T,
+                                          double (&d)[PPT], double (&w)[PPT],
+                                          double (&J)[PPT], bool (&bad)[PPT],
+                                          int& mode) {
+  if (i0 >= i1) return;
+  double4 r = sp[i0];
+#pragma unroll 2
+  for (int i = i0; i < i1; ++i) {
+    // next row fetched one step ahead; the fetch past the last row of a tile
+    // lands in the other stage or the padding and is discarded
+    const double4 rn = sp[i + 1];
+    rk4_step<LAW, PPT>(P, r.x, r.y, r.z, a0_bits, d, w, mode, bad, T);
+    if (WIN) {
+#pragma unroll
+      for (int q = 0; q < PPT; ++q) {
+        const double res = d[q] - r.w;
+        J[q] = fma(res, res, J[q]);
+      }
+    }
+    r = rn;
+  }
+}
+
+// PPT particles per thread: particle q of a thread is local index
+// base + q * blockDim.x + tid (coalesced).  PPT = 2 interleaves two independent
+// dependency chains per thread for the throughput-bound batches.
+template <int LAW, int MODE, int PPT>
 __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
                                      int blocks_per_tr) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -163,15 +194,20 @@ __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
 
   const int tid = threadIdx.x;
   const int s = blockIdx.x / blocks_per_tr;  // trace (segment) of this CTA
-  const int64_t li =
-      (int64_t)(blockIdx.x - s * blocks_per_tr) * blockDim.x + tid;
-  const bool active = li < io.per;
-  // inactive threads of a ragged last CTA integrate a copy of the segment's
-  // last particle (keeps every barrier uniform) and write nothing
-  const int64_t gp = (int64_t)s * io.per + (active ? li : io.per - 1);
+  const int64_t base =
+      (int64_t)(blockIdx.x - s * blocks_per_tr) * blockDim.x * PPT + tid;
+  bool active[PPT];
+  int64_t gp[PPT];
+#pragma unroll
+  for (int q = 0; q < PPT; ++q) {
+    const int64_t li = base + (int64_t)q * blockDim.x;
+    active[q] = li < io.per;
+    // an inactive slot of a ragged last CTA integrates a copy of the segment's
+    // last particle (keeps every vote and barrier uniform) and writes nothing
+    gp[q] = (int64_t)s * io.per + (active[q] ? li : io.per - 1);
+  }
 
   const double* stream = io.stream + (int64_t)s * mc.N * 4;
-  const uint32_t tile_bytes = (uint32_t)mc.T * 32u;
 
   if (tid == 0) {
     mbar_init(&bars[0], 1);
@@ -191,35 +227,41 @@ __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
       }
     }
   }
-  (void)tile_bytes;
 
   // ---- a1: parameter map ---------------------------------------------------
-  double xloc[4] = {0.0, 0.0, 0.0, 0.0};
-  double th[4] = {0.0, 0.0, 0.0, 0.0};
+  double xloc[PPT][4];
+  Particle64 P[PPT];
+  double d[PPT], w[PPT], J[PPT];
+  bool bad[PPT];
 #pragma unroll
-  for (int j = 0; j < 4; ++j) {
-    if (j < mc.D) {
-      double xv = io.params[gp * mc.D + j];
-      xloc[j] = xv;
-      th[j] = (MODE == 1 && io.box.lg[j]) ? pow(10.0, xv) : xv;
+  for (int q = 0; q < PPT; ++q) {
+    double th[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      xloc[q][j] = 0.0;
+      if (j < mc.D) {
+        const double xv = io.params[gp[q] * mc.D + j];
+        xloc[q][j] = xv;
+        th[j] = (MODE == 1 && io.box.lg[j]) ? pow(10.0, xv) : xv;
+      }
     }
+    load_particle(P[q], LAW, th, mc.alpha, mc.beta, mc.a0, mc.inv_a0sq,
+                  mc.c_vdw, mc.c_hertz, mc.c_visc, mc.c_force);
+    double z0 = mc.z0, v0 = mc.v0;
+    if (io.z0v0 != nullptr) {
+      z0 = io.z0v0[2 * gp[q]];
+      v0 = io.z0v0[2 * gp[q] + 1];
+    }
+    d[q] = z0 + mc.zc;
+    w[q] = v0 * mc.h;
+    J[q] = 0.0;
+    bad[q] = false;
   }
-  Particle64 P;
-  load_particle(P, LAW, th, mc.alpha, mc.beta, mc.a0, mc.inv_a0sq, mc.c_vdw,
-                mc.c_hertz, mc.c_visc, mc.c_force);
-
-  double z0 = mc.z0, v0 = mc.v0;
-  if (io.z0v0 != nullptr) {
-    z0 = io.z0v0[2 * gp];
-    v0 = io.z0v0[2 * gp + 1];
-  }
-  double d = z0 + mc.zc;
-  double w = v0 * mc.h;
-  double J = 0.0;
   const long long a0_bits = __double_as_longlong(mc.a0);
-  const long long key_max = order_key(mc.d_max);
-  const long long key_min = order_key(mc.d_min);
-  bool bad = false;
+  DivergeTest T;
+  T.key_max = order_key(mc.d_max);
+  T.key_min = order_key(mc.d_min);
+  T.safe_hi = __double2hiint(mc.d_safe);
   int mode = 0;  // warp-uniform: 0 = speculate free flight, 1 = general
 
   // ---- a2-a4: RK4 over the time tiles -------------------------------------
@@ -231,16 +273,8 @@ __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
     const int n_steps = min(mc.T, mc.N - n_begin);
     // steps [0, k0) of this tile precede the misfit window
     const int k0 = max(0, min(n_steps, mc.n0 - n_begin));
-    for (int i = 0; i < n_steps; ++i) {
-      const double4 r = sp[i];
-      rk4_step<LAW>(P, r.x, r.y, r.z, a0_bits, d, w, mode);
-      const long long key = order_key(d);
-      bad |= (key > key_max) | (key < key_min);
-      if (i >= k0) {  // warp-uniform: inside the misfit window
-        const double res = d - r.w;
-        J = fma(res, res, J);
-      }
-    }
+    run_steps<LAW, PPT, false>(sp, 0, k0, P, a0_bits, T, d, w, J, bad, mode);
+    run_steps<LAW, PPT, true>(sp, k0, n_steps, P, a0_bits, T, d, w, J, bad, mode);
     __syncthreads();  // every thread is done reading stage st
     if (tid == 0 && tile + 2 < mc.n_tiles) {
       const int nb = (tile + 2) * mc.T;
@@ -250,30 +284,34 @@ __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
       bulk_g2s(st ? tile1 : tile0, stream + (int64_t)nb * 4, bytes, &bars[st]);
     }
   }
-  // the velocity of the last state must be finite too (R12)
-  {
-    const long long kw = __double_as_longlong(w) & 0x7fffffffffffffffLL;
-    bad |= (kw >= 0x7ff0000000000000LL);
-  }
-  if (bad || !(J == J)) J = CUDART_INF;
 
-  if (active) io.J[gp] = J;
+  double pb = CUDART_INF;
+  long long idx = 0x7fffffffffffffffLL;
+#pragma unroll
+  for (int q = 0; q < PPT; ++q) {
+    // the velocity of the last state must be finite too (R12)
+    const long long kw = __double_as_longlong(w[q]) & 0x7fffffffffffffffLL;
+    bad[q] |= (kw >= 0x7ff0000000000000LL);
+    if (bad[q] || !(J[q] == J[q])) J[q] = CUDART_INF;
+    if (active[q]) io.J[gp[q]] = J[q];
 
-  // ---- a5 + first level of a6 (PSO mode) -----------------------------------
-  if (MODE == 1) {
-    double pb = CUDART_INF;
-    long long idx = 0x7fffffffffffffffLL;
-    if (active) {
-      pb = io.pbestJ[gp];
-      if (J < pb) {  // strict: NaN/+Inf never win
-        pb = J;
-        io.pbestJ[gp] = J;
+    // ---- a5 + first level of a6 (PSO mode) ---------------------------------
+    if (MODE == 1 && active[q]) {
+      double pq = io.pbestJ[gp[q]];
+      if (J[q] < pq) {  // strict: NaN/+Inf never win
+        pq = J[q];
+        io.pbestJ[gp[q]] = J[q];
 #pragma unroll
         for (int j = 0; j < 4; ++j)
-          if (j < mc.D) io.pbest[gp * mc.D + j] = xloc[j];
+          if (j < mc.D) io.pbest[gp[q] * mc.D + j] = xloc[q][j];
       }
-      idx = gp;
+      if (cand_less(pq, gp[q], pb, idx)) {
+        pb = pq;
+        idx = gp[q];
+      }
     }
+  }
+  if (MODE == 1) {
     block_argmin(pb, idx, red);
     if (tid == 0) {
       io.cand[blockIdx.x].J = pb;
@@ -293,21 +331,26 @@ __global__ void trajectory_kernel(ModelConsts mc, const double* __restrict__ th,
   const bool writer = (threadIdx.x == 0);
   double t4[4] = {0.0, 0.0, 0.0, 0.0};
   for (int j = 0; j < mc.D && j < 4; ++j) t4[j] = th[j];
-  Particle64 P;
-  load_particle(P, LAW, t4, mc.alpha, mc.beta, mc.a0, mc.inv_a0sq, mc.c_vdw,
+  Particle64 P[1];
+  load_particle(P[0], LAW, t4, mc.alpha, mc.beta, mc.a0, mc.inv_a0sq, mc.c_vdw,
                 mc.c_hertz, mc.c_visc, mc.c_force);
-  double d = z0 + mc.zc, w = v0 * mc.h;
+  double d[1] = {z0 + mc.zc}, w[1] = {v0 * mc.h};
   const long long a0_bits = __double_as_longlong(mc.a0);
   const double inv_h = 1.0 / mc.h;
   int mode = 0;
+  bool bad[1] = {false};
+  DivergeTest T;
+  T.key_max = order_key(mc.d_max);
+  T.key_min = order_key(mc.d_min);
+  T.safe_hi = __double2hiint(mc.d_safe);
   if (zs && writer) zs[0] = z0;
   if (vs && writer) vs[0] = v0;
   const double4* rows = reinterpret_cast<const double4*>(stream);
   for (int n = 0; n < mc.N; ++n) {
     const double4 r = rows[n];
-    rk4_step<LAW>(P, r.x, r.y, r.z, a0_bits, d, w, mode);
-    if (zs && writer) zs[n + 1] = d - mc.zc;
-    if (vs && writer) vs[n + 1] = w * inv_h;
+    rk4_step<LAW, 1>(P, r.x, r.y, r.z, a0_bits, d, w, mode, bad, T);
+    if (zs && writer) zs[n + 1] = d[0] - mc.zc;
+    if (vs && writer) vs[n + 1] = w[0] * inv_h;
   }
 }
 
@@ -498,13 +541,13 @@ int launch_build_stream(const ModelConsts& mc, const double* trace, int n_traces
   return 1;
 }
 
-template <int LAW, int MODE>
+template <int LAW, int MODE, int PPT>
 static int launch_integrate_t(const ModelConsts& mc, const IntegrateIO& io,
                               int block, cudaStream_t st) {
-  const int bpt = blocks_per_trace(io.per, block);
+  const int bpt = blocks_per_trace(io.per, block * PPT);
   const unsigned grid = (unsigned)(bpt * io.n_traces);
-  const size_t smem = (size_t)mc.T * 32 * 2 + 16;
-  auto kern = integrate_misfit_f64<LAW, MODE>;
+  const size_t smem = (size_t)mc.T * 32 * 2 + 64;  // + barriers + over-read pad
+  auto kern = integrate_misfit_f64<LAW, MODE, PPT>;
   if (smem > 48 * 1024)
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                          (int)smem);
@@ -513,11 +556,14 @@ static int launch_integrate_t(const ModelConsts& mc, const IntegrateIO& io,
 }
 
 int launch_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block,
-                         cudaStream_t st) {
-#define AFM_DISPATCH(LAWV)                                           \
-  case LAWV:                                                         \
-    return io.mode ? launch_integrate_t<LAWV, 1>(mc, io, block, st)  \
-                   : launch_integrate_t<LAWV, 0>(mc, io, block, st);
+                         int ppt, cudaStream_t st) {
+#define AFM_DISPATCH(LAWV)                                                      \
+  case LAWV:                                                                    \
+    if (ppt == 2)                                                               \
+      return io.mode ? launch_integrate_t<LAWV, 1, 2>(mc, io, block, st)        \
+                     : launch_integrate_t<LAWV, 0, 2>(mc, io, block, st);       \
+    return io.mode ? launch_integrate_t<LAWV, 1, 1>(mc, io, block, st)          \
+                   : launch_integrate_t<LAWV, 0, 1>(mc, io, block, st);
   switch (mc.law) {
     AFM_DISPATCH(AFM_LAW_NONE)
     AFM_DISPATCH(AFM_LAW_DMT)
