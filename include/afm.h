@@ -199,6 +199,14 @@ int afm_philox4x32_10(const uint32_t* ctr, int64_t n, const uint32_t* key,
 int afm_trajectory(const double* theta, const afm_cfg* cfg, double z0,
                    double v0, double* zs, double* vs, void* cuda_stream);
 
+/* Register-only FMA throughput of the device (the measured
+ * denominator reported beside the lane-model peak).  Runs a kernel of
+ * independent dependent-FMA chains for about `seconds` (0 < seconds <= 10) in
+ * the given afm_precision and writes the sustained rate, counting 2 flops per
+ * FMA, to *tflops (host).  Synchronous.  Not part of the hot path. */
+int afm_fma_peak(int32_t precision, double seconds, double* tflops,
+                 void* cuda_stream);
+
 /* Kernel launches enqueued by this library on the calling thread since the
  * last reset (bench.py's gpu_launches). */
 int64_t afm_launch_count(void);

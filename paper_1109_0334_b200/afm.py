@@ -24,7 +24,7 @@ OK, EINVAL, ECUDA, EUNSUPPORTED = 0, -1, -2, -3
 SYMBOLS = (
     "afm_forward_batch", "afm_forward_batch_host", "afm_pso_invert",
     "afm_pso_invert_host", "afm_pso_step", "afm_pso_init",
-    "afm_philox4x32_10", "afm_trajectory", "afm_launch_count",
+    "afm_philox4x32_10", "afm_trajectory", "afm_fma_peak", "afm_launch_count",
     "afm_reset_launch_count", "afm_set_option", "afm_last_error",
     "afm_version", "afm_shutdown",
 )
@@ -94,9 +94,10 @@ def lib():
         L.afm_philox4x32_10.argtypes = [dp, i64, C.POINTER(C.c_uint32), dp, vp]
         L.afm_trajectory.argtypes = [dp, C.POINTER(Cfg), C.c_double, C.c_double,
                                      dp, dp, vp]
+        L.afm_fma_peak.argtypes = [i32, C.c_double, C.POINTER(C.c_double), vp]
         for name in ("afm_forward_batch", "afm_forward_batch_host", "afm_pso_invert",
                      "afm_pso_invert_host", "afm_pso_step", "afm_pso_init",
-                     "afm_philox4x32_10", "afm_trajectory"):
+                     "afm_philox4x32_10", "afm_trajectory", "afm_fma_peak"):
             getattr(L, name).restype = C.c_int
         L.afm_launch_count.restype = i64
         L.afm_launch_count.argtypes = []
@@ -317,6 +318,14 @@ def afm_trajectory(theta, cfg, z0, v0, stream=None):
                                 _ptr(zs), _ptr(vs), _stream_ptr(stream)))
     torch.cuda.synchronize()
     return zs.cpu().numpy(), vs.cpu().numpy()
+
+
+def afm_fma_peak(precision, seconds=0.2, stream=None):
+    """Measured register-only FMA rate in TFLOP/s (2 flops per FMA)."""
+    out = C.c_double(0.0)
+    _check(lib().afm_fma_peak(int(precision), float(seconds), C.byref(out),
+                              _stream_ptr(stream)))
+    return out.value
 
 
 def afm_launch_count():

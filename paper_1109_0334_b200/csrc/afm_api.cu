@@ -214,6 +214,49 @@ void make_consts(const afm_cfg* c, int block, ModelConsts* mc) {
   mc->n_tiles = (mc->N + T - 1) / T;
 }
 
+// FP32 kernel constants (kernel units: 1 nm, one step; everything /6).
+void make_consts_f32(const afm_cfg* c, ModelConstsF32* mf) {
+  const double w0 = 2.0 * M_PI * c->f0;
+  const double w = 2.0 * M_PI * c->f_drive;
+  const double r = w / w0;
+  const double a = 1.0 - r * r, b = r / c->Q;
+  const double h = 2.0 * M_PI / (w * (double)c->steps_per_cycle);
+  const double len = 1e-9;
+  const double hq = h * w0;
+  memset(mf, 0, sizeof(*mf));
+  mf->len = len;
+  mf->h = h;
+  mf->w_drive = w;
+  mf->a6 = hq / c->Q / 6.0;
+  mf->b6 = hq * hq / 6.0;
+  mf->drive6 = mf->b6 * (c->A0 * sqrt(a * a + b * b)) / len;
+  mf->b6_zc = mf->b6 * c->z_c / len;
+  mf->zc = c->z_c / len;
+  mf->a0 = c->a0 / len;
+  const double sqR = sqrt(c->R > 0 ? c->R : 0.0);
+  mf->c_vdw = mf->b6 * c->R / (6.0 * c->k * len * len * len);
+  mf->c_hertz = mf->b6 * (4.0 / 3.0) * sqR * sqrt(len) / c->k;
+  mf->c_visc = mf->b6 * sqR * sqrt(len) / (h * c->k);
+  mf->c_rep = mf->b6 / (c->k * pow(len, 9.0));
+  mf->c_att = mf->b6 / (c->k * len * len * len);
+  mf->c_fad = mf->b6 / (c->k * len);
+  mf->c_lam = 1.4426950408889634 * len;
+  mf->d_max = (c->z_c + 100.0 * c->A0) / len;
+  mf->d_min = (c->z_c - 100.0 * c->A0) / len;
+  mf->d_safe = fmax(0.0, 100.0 * c->A0 - fabs(c->z_c)) / len;
+  mf->z0 = c->z0;
+  mf->v0 = c->v0;
+  mf->law = c->law;
+  mf->D = c->n_params;
+  mf->N = c->steps_per_cycle * c->n_cycles;
+  mf->W = c->steps_per_cycle * (c->n_cycles - c->n_skip_cycles);
+  mf->n0 = mf->N - mf->W;
+  int T = g_opt_tile > 0 ? g_opt_tile : 128;
+  if (T > mf->N) T = mf->N;
+  mf->T = T;
+  mf->n_tiles = (mf->N + T - 1) / T;
+}
+
 int pick_block(int64_t per, int n_traces) {
   if (g_opt_block > 0) return g_opt_block;
   (void)per;
@@ -266,21 +309,26 @@ int validate_swarm(const afm_swarm_cfg* s) {
 int forward_locked(const double* params, int64_t P, const double* trace,
                    const afm_cfg* cfg, const double* z0v0, double* misfit,
                    cudaStream_t st) {
-  if (cfg->precision == AFM_F32)
-    return fail(AFM_EUNSUPPORTED, "FP32 integrate kernel not built yet");
+  const bool f32 = (cfg->precision == AFM_F32);
   const int64_t per = P / cfg->n_traces;
   const int block = pick_block(per, cfg->n_traces);
   const int ppt = pick_ppt(per, cfg->n_traces);
   ModelConsts mc;
+  ModelConstsF32 mf;
   make_consts(cfg, block, &mc);
+  make_consts_f32(cfg, &mf);
   int rc = acquire_ws(st);
   if (rc) return rc;
-  const size_t stream_bytes = (size_t)cfg->n_traces * mc.N * 32;
-  if (g_ws.stream.ensure(stream_bytes))
+  const size_t stream_bytes = (size_t)cfg->n_traces * mc.N * (f32 ? 16 : 32);
+  if (g_ws.stream.ensure(stream_bytes + 64))
     return fail(AFM_ECUDA, "cudaMalloc of %zu B time-tile stream failed",
                 stream_bytes);
-  LAUNCHED(launch_build_stream(mc, trace, cfg->n_traces,
-                               (double*)g_ws.stream.p, st));
+  if (f32)
+    LAUNCHED(launch_build_stream_f32(mf, trace, cfg->n_traces,
+                                     (float*)g_ws.stream.p, st));
+  else
+    LAUNCHED(launch_build_stream(mc, trace, cfg->n_traces,
+                                 (double*)g_ws.stream.p, st));
   IntegrateIO io;
   memset(&io, 0, sizeof(io));
   io.params = params;
@@ -290,6 +338,10 @@ int forward_locked(const double* params, int64_t P, const double* trace,
   io.per = per;
   io.n_traces = cfg->n_traces;
   io.mode = 0;
+  if (f32) {
+    LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
+    return release_ws(st);
+  }
   LAUNCHED(launch_integrate_f64(mc, io, block, ppt, st));
   return release_ws(st);
 }
@@ -419,8 +471,7 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
                              double* J_star, double* swarm_dump,
                              double* gbest_hist, int32_t* n_iters_done,
                              cudaStream_t st) {
-  if (cfg->precision == AFM_F32)
-    return fail(AFM_EUNSUPPORTED, "FP32 integrate kernel not built yet");
+  const bool f32 = (cfg->precision == AFM_F32);
   const int D = cfg->n_params;
   const int T = cfg->n_traces;
   const int64_t per = swarm->n_particles;
@@ -429,7 +480,9 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
   const int ppt = pick_ppt(per, T);
   const int bpt = blocks_per_trace(per, block * ppt);
   ModelConsts mc;
+  ModelConstsF32 mf;
   make_consts(cfg, block, &mc);
+  make_consts_f32(cfg, &mf);
   int rc = acquire_ws(st);
   if (rc) return rc;
 
@@ -438,7 +491,7 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
   const size_t n_dbl = (size_t)PT * (3 * D + 2) + (size_t)T * (2 * D + 2);
   if (g_ws.swarm.ensure(n_dbl * 8) ||
       g_ws.cand.ensure((size_t)bpt * T * sizeof(Cand)) ||
-      g_ws.stream.ensure((size_t)T * mc.N * 32))
+      g_ws.stream.ensure((size_t)T * mc.N * 32 + 64))
     return fail(AFM_ECUDA, "cudaMalloc of the PSO workspace failed");
   double* x = (double*)g_ws.swarm.p;
   double* v = x + PT * D;
@@ -454,7 +507,10 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
   BoxDev box = make_box(bounds, D);
   SwarmDev sw = {swarm->w, swarm->c1, swarm->c2};
 
-  LAUNCHED(launch_build_stream(mc, trace, T, (double*)g_ws.stream.p, st));
+  if (f32)
+    LAUNCHED(launch_build_stream_f32(mf, trace, T, (float*)g_ws.stream.p, st));
+  else
+    LAUNCHED(launch_build_stream(mc, trace, T, (double*)g_ws.stream.p, st));
   LAUNCHED(launch_pso_init(box, D, per, T, seed, x, v, pbest, pbestJ, gbest,
                            gbestJ, st));
   IntegrateIO io;
@@ -474,7 +530,10 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
   int done = 0;
   for (int it = 0; it < swarm->n_iters; ++it) {
     const bool last = (it == swarm->n_iters - 1);
-    LAUNCHED(launch_integrate_f64(mc, io, block, ppt, st));
+    if (f32)
+      LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
+    else
+      LAUNCHED(launch_integrate_f64(mc, io, block, ppt, st));
     LAUNCHED(launch_pso_gbest(
         box, D, T, bpt, (Cand*)g_ws.cand.p, pbest, gbest, gbestJ,
         gbest_hist ? gbest_hist + (size_t)it * T * (D + 1) : nullptr, th_dev,
@@ -591,6 +650,42 @@ int afm_trajectory(const double* theta, const afm_cfg* cfg, double z0, double v0
   LAUNCHED(launch_build_stream(mc, zero_trace, 1, (double*)g_ws.stream.p, st));
   LAUNCHED(launch_trajectory(mc, (const double*)g_ws.scratch.p,
                              (const double*)g_ws.stream.p, z0, v0, zs, vs, st));
+  return release_ws(st);
+}
+
+int afm_fma_peak(int32_t precision, double seconds, double* tflops,
+                 void* cuda_stream) {
+  if (!tflops) return fail(AFM_EINVAL, "tflops is NULL");
+  if (precision != AFM_F64 && precision != AFM_F32)
+    return fail(AFM_EINVAL, "unknown precision %d", precision);
+  if (!(seconds > 0) || seconds > 10)
+    return fail(AFM_EINVAL, "seconds must be in (0, 10]");
+  int rc = check_device();
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  if ((rc = acquire_ws(st))) return rc;
+  if (g_ws.scratch.ensure(64)) return fail(AFM_ECUDA, "cudaMalloc failed");
+  int dev = 0, sms = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const int threads = 256, blocks = sms * 8;
+  const double per_iter = 2.0 * 8 * 16 * (double)threads * blocks;  // flops
+  // calibrate the iteration count on a short launch, then time `seconds`
+  int iters = 2000;
+  float ms = 0.f;
+  int n = launch_fma_peak(precision, iters, blocks, threads, g_ws.scratch.p, &ms, st);
+  if (n < 0) return fail(AFM_ECUDA, "cudaEventCreate failed");
+  g_launches += n;
+  CUDA_TRY(cudaGetLastError());
+  double want = seconds * 1e3 / (ms > 1e-3 ? ms : 1e-3) * iters;
+  if (want > 2.0e8) want = 2.0e8;
+  iters = want < 2000 ? 2000 : (int)want;
+  n = launch_fma_peak(precision, iters, blocks, threads, g_ws.scratch.p, &ms, st);
+  if (n < 0) return fail(AFM_ECUDA, "cudaEventCreate failed");
+  g_launches += n;
+  CUDA_TRY(cudaGetLastError());
+  *tflops = per_iter * iters / (ms * 1e-3) / 1e12;
   return release_ws(st);
 }
 

@@ -1,0 +1,100 @@
+// afm_device_common.cuh -- pieces shared by the FP64 and FP32 integrate kernels:
+// the PTX wrappers of the TMA-staged (cp.async.bulk + mbarrier) time-tile ring
+// and the block argmin of the global-best search.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include <stdint.h>
+
+#include "afm_internal.h"
+
+namespace afm {
+
+// ---- mbarrier / bulk-copy PTX (sm_90+; SASS: SYNCS.*, UBLKCP) ---------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)),
+               "r"(count)
+               : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() {
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() {
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar,
+                                                      uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(
+                   smem_u32(bar)),
+               "r"(bytes)
+               : "memory");
+}
+// 1-D bulk async copy global -> shared, completion counted on an mbarrier.
+// dst, src 16-byte aligned, bytes a multiple of 16.
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src,
+                                         uint32_t bytes, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes "
+      "[%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar))
+      : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "AFM_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra AFM_DONE;\n"
+      "bra AFM_WAIT;\n"
+      "AFM_DONE:\n"
+      "}" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+
+__device__ __forceinline__ bool cand_less(double Ja, long long ia, double Jb,
+                                          long long ib) {
+  return (Ja < Jb) || (Ja == Jb && ia < ib);
+}
+
+// Block argmin of (J, idx), lowest idx among equal J; result valid in thread 0.
+__device__ __forceinline__ void block_argmin(double& J, long long& idx,
+                                             Cand* red /* [32] shared */) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int nwarps = (blockDim.x + 31) >> 5;
+#pragma unroll
+  for (int off = 16; off >= 1; off >>= 1) {
+    double Jo = __shfl_down_sync(0xffffffffu, J, off);
+    long long io = __shfl_down_sync(0xffffffffu, idx, off);
+    if (cand_less(Jo, io, J, idx)) {
+      J = Jo;
+      idx = io;
+    }
+  }
+  if (nwarps == 1) return;
+  if (lane == 0) {
+    red[warp].J = J;
+    red[warp].idx = idx;
+  }
+  __syncthreads();
+  if (warp == 0) {
+    J = (lane < nwarps) ? red[lane].J : CUDART_INF;
+    idx = (lane < nwarps) ? red[lane].idx : 0x7fffffffffffffffLL;
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+      double Jo = __shfl_down_sync(0xffffffffu, J, off);
+      long long io = __shfl_down_sync(0xffffffffu, idx, off);
+      if (cand_less(Jo, io, J, idx)) {
+        J = Jo;
+        idx = io;
+      }
+    }
+  }
+}
+
+}  // namespace afm

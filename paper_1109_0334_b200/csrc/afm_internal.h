@@ -42,16 +42,24 @@ struct ModelConsts {
   int32_t pad_;
 };
 
-// FP32 kernel constants (kernel units: length 1 nm, time 1/w0; R14).
+// FP32 kernel constants (R14; afm_device_f32.cuh).  Kernel units:
+// length 1 nm, one RK4 step = unit time; every acceleration coefficient is
+// pre-scaled by 1/6 (b6 = beta/6, a6 = alpha/6).  Computed on the host in FP64.
 struct ModelConstsF32 {
   double len;        // metres per kernel length unit (1e-9)
-  double hq;         // h w0 (step in kernel time units), FP64; split hi/lo below
-  float h_hi, h_lo;  // two-float step
-  float inv_Q;
-  float zc, a0, inv_a0sq, sqrt_a0_dummy;
-  double c_vdw, c_hertz, c_visc, c_force;  // FP64 scale factors: p_j = theta_j * c
-  float d_max, d_min;
-  float z0, v0;
+  double h;          // step, seconds
+  double w_drive;
+  double a6, b6;     // alpha/6, beta/6 in FP64 (split hi/lo by the kernel)
+  double drive6;     // b6 * (F0/k) / len: drive amplitude of the scaled stream
+  double b6_zc;      // b6 * z_c / len
+  double zc, a0;     // nm
+  double c_vdw;      // c0 = -theta0 c_vdw, c2 = c0 / a0^2        (DMT)
+  double c_hertz;    // c1 = theta1 c_hertz
+  double c_visc;     // c3 = -theta2 c_visc
+  double c_rep, c_att, c_fad;  // LJ+exp: c0 = theta0 c_rep, c1 = -theta1 c_att, c2 = -theta2 c_fad
+  double c_lam;      // c3 = -c_lam / theta3  (log2(e) len)
+  double d_max, d_min, d_safe;  // nm
+  double z0, v0;     // default initial state, SI
   int32_t law, D, N, n0, W, T, n_tiles, pad_;
 };
 
@@ -78,7 +86,7 @@ struct Cand {
 struct IntegrateIO {
   const double* params;   // MODE 0: theta [PT][D]; MODE 1: x [PT][D]
   const double* z0v0;     // [PT][2] or nullptr
-  const double* stream;   // [n_traces][N][4] time-tile stream
+  const double* stream;   // [n_traces][N][4] time-tile stream (FP32 kernel: float4 rows)
   double* J;              // [PT]
   // MODE 1 (PSO) only:
   double* pbest;          // [PT][D]
@@ -94,13 +102,12 @@ int blocks_per_trace(int64_t per, int block);
 
 int launch_build_stream(const ModelConsts& mc, const double* trace, int n_traces,
                         double* stream, cudaStream_t st);
-int launch_build_stream_f32(const ModelConsts& mc, const ModelConstsF32& mf,
-                            const double* trace, int n_traces, float* stream,
-                            cudaStream_t st);
+int launch_build_stream_f32(const ModelConstsF32& mf, const double* trace,
+                            int n_traces, float* stream, cudaStream_t st);
 int launch_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block,
                          int ppt, cudaStream_t st);
-int launch_integrate_f32(const ModelConsts& mc, const ModelConstsF32& mf,
-                         const IntegrateIO& io, int block, cudaStream_t st);
+int launch_integrate_f32(const ModelConstsF32& mf, const IntegrateIO& io,
+                         int block, int ppt, cudaStream_t st);
 int launch_trajectory(const ModelConsts& mc, const double* theta_dev,
                       const double* stream, double z0, double v0, double* zs,
                       double* vs, cudaStream_t st);
@@ -121,6 +128,8 @@ int launch_pso_move(const BoxDev& box, const SwarmDev& sw, int D, int64_t per,
                     const double* J, double* x, double* v, const double* pbest,
                     const double* pbestJ, const double* gbest, double* dump_row,
                     cudaStream_t st);
+int launch_fma_peak(int precision, int iters, int blocks, int threads,
+                    void* sink, float* ms, cudaStream_t st);
 int launch_philox(const uint32_t* ctr, int64_t n, uint32_t k0, uint32_t k1,
                   uint32_t* out, cudaStream_t st);
 

@@ -112,46 +112,6 @@ __global__ void build_stream_kernel(ModelConsts mc,
 // ============================================================================
 // integrate-and-misfit, FP64
 // ============================================================================
-__device__ __forceinline__ bool cand_less(double Ja, long long ia, double Jb,
-                                          long long ib) {
-  return (Ja < Jb) || (Ja == Jb && ia < ib);
-}
-
-// Block argmin of (J, idx), lowest idx among equal J; result valid in thread 0.
-__device__ __forceinline__ void block_argmin(double& J, long long& idx,
-                                             Cand* red /* [32] shared */) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int nwarps = (blockDim.x + 31) >> 5;
-#pragma unroll
-  for (int off = 16; off >= 1; off >>= 1) {
-    double Jo = __shfl_down_sync(0xffffffffu, J, off);
-    long long io = __shfl_down_sync(0xffffffffu, idx, off);
-    if (cand_less(Jo, io, J, idx)) {
-      J = Jo;
-      idx = io;
-    }
-  }
-  if (nwarps == 1) return;
-  if (lane == 0) {
-    red[warp].J = J;
-    red[warp].idx = idx;
-  }
-  __syncthreads();
-  if (warp == 0) {
-    J = (lane < nwarps) ? red[lane].J : CUDART_INF;
-    idx = (lane < nwarps) ? red[lane].idx : 0x7fffffffffffffffLL;
-#pragma unroll
-    for (int off = 16; off >= 1; off >>= 1) {
-      double Jo = __shfl_down_sync(0xffffffffu, J, off);
-      long long io = __shfl_down_sync(0xffffffffu, idx, off);
-      if (cand_less(Jo, io, J, idx)) {
-        J = Jo;
-        idx = io;
-      }
-    }
-  }
-}
-
 // T steps of one time tile, [i0, i1), with (WIN) or without the misfit sum.
 template <int LAW, int PPT, bool WIN>
 __device__ __forceinline__ void run_steps(const double4* sp, int i0, int i1,
