@@ -188,6 +188,50 @@ int afm_pso_init(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
                  double* v, double* pbest, double* pbestJ, double* gbest,
                  double* gbestJ, void* cuda_stream);
 
+/* ---- Sharded swarm ------------------------------------------
+ * One process per GPU holds a contiguous slice of a larger swarm: local
+ * particle i of this process is global particle first_particle + i (global
+ * indices run trace-major: trace * particles_per_trace + i, as in
+ * afm_pso_invert).  Philox counters and the lowest-index tie-break use the
+ * global index, so a sharded run replays the unsharded one bit for bit.  The
+ * only data exchanged per iteration is the candidate row of every rank
+ * (D + 2 doubles per trace), which the CALLER all-gathers (torch.distributed /
+ * NCCL) between afm_pso_shard_eval and afm_pso_shard_move; sharding whole
+ * traces needs no exchange (n_ranks = 1, gathered = own cand_out).
+ * swarm->n_particles is the LOCAL particle count per local trace. */
+
+/* afm_pso_init for a shard.  Note: gbest is set to the first LOCAL particle;
+ * when one trace is sharded over ranks, copy rank 0's gbest to the others. */
+int afm_pso_shard_init(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                       int32_t n_dims, int32_t n_traces, uint64_t seed,
+                       int64_t first_particle, double* x, double* v,
+                       double* pbest, double* pbestJ, double* gbest,
+                       double* gbestJ, void* cuda_stream);
+
+/* Rows a1-a5 + the local part of a6 for this shard: theta = map(x), forward
+ * solve + misfit, personal bests, and the shard's best candidate per trace.
+ * All device, FP64:  trace [cfg->n_traces][W]; x, pbest [PT][D]; J, pbestJ
+ * [PT]; cand_out [cfg->n_traces][D+2] = { pbestJ, global index, pbest x[D] }.
+ * Asynchronous. */
+int afm_pso_shard_eval(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                       const double* trace, const afm_cfg* cfg,
+                       int64_t first_particle, const double* x, double* J,
+                       double* pbest, double* pbestJ, double* cand_out,
+                       void* cuda_stream);
+
+/* Rest of a6 + a7: global best per trace from the gathered candidates
+ * (device [n_ranks][n_traces][D+2]; lowest global index among equal minima,
+ * replaced only on a strict improvement), then Eq. 8 + move + bound rule when
+ * do_move != 0.  theta_star [n_traces][D], J_star [n_traces]: device or NULL.
+ * Asynchronous. */
+int afm_pso_shard_move(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                       int32_t n_dims, int32_t n_traces, uint64_t seed,
+                       int32_t iteration, int32_t do_move,
+                       int64_t first_particle, const double* gathered,
+                       int32_t n_ranks, double* x, double* v,
+                       const double* pbest, double* gbest, double* gbestJ,
+                       double* theta_star, double* J_star, void* cuda_stream);
+
 /* Philox4x32-10 on the device for n counters (tests: known answers).
  *   ctr device [n][4] uint32, key host [2], out device [n][4].  Async. */
 int afm_philox4x32_10(const uint32_t* ctr, int64_t n, const uint32_t* key,

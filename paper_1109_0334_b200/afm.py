@@ -24,6 +24,7 @@ OK, EINVAL, ECUDA, EUNSUPPORTED = 0, -1, -2, -3
 SYMBOLS = (
     "afm_forward_batch", "afm_forward_batch_host", "afm_pso_invert",
     "afm_pso_invert_host", "afm_pso_step", "afm_pso_init",
+    "afm_pso_shard_init", "afm_pso_shard_eval", "afm_pso_shard_move",
     "afm_philox4x32_10", "afm_trajectory", "afm_fma_peak", "afm_launch_count",
     "afm_reset_launch_count", "afm_set_option", "afm_last_error",
     "afm_version", "afm_shutdown",
@@ -91,13 +92,22 @@ def lib():
                                    u64, i32, i32, dp, dp, dp, dp, dp, dp, dp, vp]
         L.afm_pso_init.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), i32, i32,
                                    u64, dp, dp, dp, dp, dp, dp, vp]
+        L.afm_pso_shard_init.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), i32,
+                                         i32, u64, i64, dp, dp, dp, dp, dp, dp, vp]
+        L.afm_pso_shard_eval.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), dp,
+                                         C.POINTER(Cfg), i64, dp, dp, dp, dp, dp, vp]
+        L.afm_pso_shard_move.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), i32,
+                                         i32, u64, i32, i32, i64, dp, i32, dp, dp, dp,
+                                         dp, dp, dp, dp, vp]
         L.afm_philox4x32_10.argtypes = [dp, i64, C.POINTER(C.c_uint32), dp, vp]
         L.afm_trajectory.argtypes = [dp, C.POINTER(Cfg), C.c_double, C.c_double,
                                      dp, dp, vp]
         L.afm_fma_peak.argtypes = [i32, C.c_double, C.POINTER(C.c_double), vp]
         for name in ("afm_forward_batch", "afm_forward_batch_host", "afm_pso_invert",
                      "afm_pso_invert_host", "afm_pso_step", "afm_pso_init",
-                     "afm_philox4x32_10", "afm_trajectory", "afm_fma_peak"):
+                     "afm_philox4x32_10", "afm_trajectory", "afm_fma_peak",
+                     "afm_pso_shard_init", "afm_pso_shard_eval",
+                     "afm_pso_shard_move"):
             getattr(L, name).restype = C.c_int
         L.afm_launch_count.restype = i64
         L.afm_launch_count.argtypes = []
@@ -292,6 +302,60 @@ def afm_pso_step(bounds, swarm, n_dims, n_traces, seed, iteration, do_move, J, s
                               _ptr(st["x"]), _ptr(st["v"]), _ptr(st["pbest"]),
                               _ptr(st["pbestJ"]), _ptr(st["gbest"]),
                               _ptr(st["gbestJ"]), _stream_ptr(stream)))
+    return st
+
+
+def afm_pso_shard_init(bounds, swarm, n_dims, n_traces, seed, first_particle,
+                       stream=None):
+    """Swarm state of a shard: swarm.n_particles local particles
+    per local trace, global index = first_particle + local index."""
+    torch = _torch()
+    PT = swarm.n_particles * n_traces
+    kw = dict(dtype=torch.float64, device="cuda")
+    st = dict(x=torch.empty((PT, n_dims), **kw), v=torch.empty((PT, n_dims), **kw),
+              pbest=torch.empty((PT, n_dims), **kw), pbestJ=torch.empty(PT, **kw),
+              gbest=torch.empty((n_traces, n_dims), **kw),
+              gbestJ=torch.empty(n_traces, **kw), J=torch.empty(PT, **kw),
+              cand=torch.empty((n_traces, n_dims + 2), **kw),
+              theta_star=torch.empty((n_traces, n_dims), **kw),
+              J_star=torch.empty(n_traces, **kw))
+    _check(lib().afm_pso_shard_init(C.byref(bounds), C.byref(swarm), n_dims, n_traces,
+                                    int(seed), int(first_particle), _ptr(st["x"]),
+                                    _ptr(st["v"]), _ptr(st["pbest"]),
+                                    _ptr(st["pbestJ"]), _ptr(st["gbest"]),
+                                    _ptr(st["gbestJ"]), _stream_ptr(stream)))
+    return st
+
+
+def afm_pso_shard_eval(bounds, swarm, trace, cfg, first_particle, st, stream=None):
+    """Forward batch + personal bests of the shard; returns st["cand"]
+    [n_traces][D+2] = (pbestJ, global index, pbest x[D]) for the exchange."""
+    trace = _dev_f64(trace, "trace")
+    if trace.numel() != cfg.n_traces * cfg.n_window:
+        raise ValueError("trace must hold n_traces * W samples")
+    _check(lib().afm_pso_shard_eval(C.byref(bounds), C.byref(swarm), _ptr(trace),
+                                    C.byref(cfg), int(first_particle), _ptr(st["x"]),
+                                    _ptr(st["J"]), _ptr(st["pbest"]),
+                                    _ptr(st["pbestJ"]), _ptr(st["cand"]),
+                                    _stream_ptr(stream)))
+    return st["cand"]
+
+
+def afm_pso_shard_move(bounds, swarm, n_dims, n_traces, seed, iteration, do_move,
+                       first_particle, gathered, st, stream=None):
+    """Global best from the gathered candidates [n_ranks][n_traces][D+2], then the
+    Eq. 8 move of the shard."""
+    gathered = _dev_f64(gathered, "gathered")
+    n_ranks = gathered.numel() // (n_traces * (n_dims + 2))
+    if n_ranks * n_traces * (n_dims + 2) != gathered.numel():
+        raise ValueError("gathered must be [n_ranks][n_traces][D+2]")
+    _check(lib().afm_pso_shard_move(C.byref(bounds), C.byref(swarm), n_dims, n_traces,
+                                    int(seed), int(iteration), int(bool(do_move)),
+                                    int(first_particle), _ptr(gathered), n_ranks,
+                                    _ptr(st["x"]), _ptr(st["v"]), _ptr(st["pbest"]),
+                                    _ptr(st["gbest"]), _ptr(st["gbestJ"]),
+                                    _ptr(st["theta_star"]), _ptr(st["J_star"]),
+                                    _stream_ptr(stream)))
     return st
 
 

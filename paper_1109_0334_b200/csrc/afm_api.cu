@@ -412,10 +412,12 @@ int afm_forward_batch_host(const double* params, int64_t n_particles,
   return AFM_OK;
 }
 
-int afm_pso_init(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
-                 int32_t n_dims, int32_t n_traces, uint64_t seed, double* x,
-                 double* v, double* pbest, double* pbestJ, double* gbest,
-                 double* gbestJ, void* cuda_stream) {
+int afm_pso_shard_init(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                       int32_t n_dims, int32_t n_traces, uint64_t seed,
+                       int64_t first_particle, double* x, double* v,
+                       double* pbest, double* pbestJ, double* gbest,
+                       double* gbestJ, void* cuda_stream) {
+  if (first_particle < 0) return fail(AFM_EINVAL, "first_particle must be >= 0");
   if (n_dims < 1 || n_dims > 4) return fail(AFM_EINVAL, "n_dims must be 1..4");
   if (n_traces < 1) return fail(AFM_EINVAL, "n_traces must be >= 1");
   int rc = validate_bounds(bounds, n_dims);
@@ -425,9 +427,17 @@ int afm_pso_init(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
     return fail(AFM_EINVAL, "NULL swarm array");
   if ((rc = check_device())) return rc;
   LAUNCHED(launch_pso_init(make_box(bounds, n_dims), n_dims, swarm->n_particles,
-                           n_traces, seed, x, v, pbest, pbestJ, gbest, gbestJ,
-                           (cudaStream_t)cuda_stream));
+                           n_traces, seed, first_particle, x, v, pbest, pbestJ,
+                           gbest, gbestJ, (cudaStream_t)cuda_stream));
   return AFM_OK;
+}
+
+int afm_pso_init(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                 int32_t n_dims, int32_t n_traces, uint64_t seed, double* x,
+                 double* v, double* pbest, double* pbestJ, double* gbest,
+                 double* gbestJ, void* cuda_stream) {
+  return afm_pso_shard_init(bounds, swarm, n_dims, n_traces, seed, 0, x, v,
+                            pbest, pbestJ, gbest, gbestJ, cuda_stream);
 }
 
 int afm_pso_step(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
@@ -459,7 +469,7 @@ int afm_pso_step(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   LAUNCHED(launch_pso_gbest(box, n_dims, n_traces, bpt, (Cand*)g_ws.cand.p,
                             pbest, gbest, gbestJ, nullptr, nullptr, nullptr, st));
   if (do_move)
-    LAUNCHED(launch_pso_move(box, sw, n_dims, per, n_traces, seed,
+    LAUNCHED(launch_pso_move(box, sw, n_dims, per, n_traces, seed, 0,
                              (uint32_t)iteration, 1, J, x, v, pbest, pbestJ,
                              gbest, nullptr, st));
   return release_ws(st);
@@ -511,7 +521,7 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
     LAUNCHED(launch_build_stream_f32(mf, trace, T, (float*)g_ws.stream.p, st));
   else
     LAUNCHED(launch_build_stream(mc, trace, T, (double*)g_ws.stream.p, st));
-  LAUNCHED(launch_pso_init(box, D, per, T, seed, x, v, pbest, pbestJ, gbest,
+  LAUNCHED(launch_pso_init(box, D, per, T, seed, 0, x, v, pbest, pbestJ, gbest,
                            gbestJ, st));
   IntegrateIO io;
   memset(&io, 0, sizeof(io));
@@ -550,7 +560,7 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
     double* dump_row =
         swarm_dump ? swarm_dump + (size_t)it * PT * (3 * D + 2) : nullptr;
     if (!stop || dump_row)
-      LAUNCHED(launch_pso_move(box, sw, D, per, T, seed, (uint32_t)it,
+      LAUNCHED(launch_pso_move(box, sw, D, per, T, seed, 0, (uint32_t)it,
                                stop ? 0 : 1, J, x, v, pbest, pbestJ, gbest,
                                dump_row, st));
     done = it + 1;
@@ -612,6 +622,91 @@ int afm_pso_invert_host(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   return pso_invert_locked(bounds, swarm, seed, (const double*)g_ws.h_trace.p,
                            cfg, theta_star, J_star, nullptr, nullptr,
                            n_iters_done, st);
+}
+
+int afm_pso_shard_eval(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                       const double* trace, const afm_cfg* cfg,
+                       int64_t first_particle, const double* x, double* J,
+                       double* pbest, double* pbestJ, double* cand_out,
+                       void* cuda_stream) {
+  int rc = validate_cfg(cfg);
+  if (rc) return rc;
+  if (cfg->n_params < 1) return fail(AFM_EINVAL, "n_params = 0");
+  if ((rc = validate_bounds(bounds, cfg->n_params))) return rc;
+  if ((rc = validate_swarm(swarm))) return rc;
+  if (first_particle < 0) return fail(AFM_EINVAL, "first_particle must be >= 0");
+  if (!trace || !x || !J || !pbest || !pbestJ || !cand_out)
+    return fail(AFM_EINVAL, "NULL array");
+  if ((rc = check_device())) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  const bool f32 = (cfg->precision == AFM_F32);
+  const int D = cfg->n_params, T = cfg->n_traces;
+  const int64_t per = swarm->n_particles;
+  const int block = pick_block(per, T);
+  const int ppt = pick_ppt(per, T);
+  const int bpt = blocks_per_trace(per, block * ppt);
+  ModelConsts mc;
+  ModelConstsF32 mf;
+  make_consts(cfg, block, &mc);
+  make_consts_f32(cfg, &mf);
+  if ((rc = acquire_ws(st))) return rc;
+  if (g_ws.cand.ensure((size_t)bpt * T * sizeof(Cand)) ||
+      g_ws.stream.ensure((size_t)T * mc.N * 32 + 64))
+    return fail(AFM_ECUDA, "cudaMalloc of the shard workspace failed");
+  if (f32)
+    LAUNCHED(launch_build_stream_f32(mf, trace, T, (float*)g_ws.stream.p, st));
+  else
+    LAUNCHED(launch_build_stream(mc, trace, T, (double*)g_ws.stream.p, st));
+  IntegrateIO io;
+  memset(&io, 0, sizeof(io));
+  io.params = x;
+  io.stream = (const double*)g_ws.stream.p;
+  io.J = J;
+  io.pbest = pbest;
+  io.pbestJ = pbestJ;
+  io.cand = (Cand*)g_ws.cand.p;
+  io.box = make_box(bounds, D);
+  io.per = per;
+  io.n_traces = T;
+  io.mode = 1;
+  if (f32)
+    LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
+  else
+    LAUNCHED(launch_integrate_f64(mc, io, block, ppt, st));
+  LAUNCHED(launch_pso_shard_cand(D, T, bpt, first_particle, (Cand*)g_ws.cand.p,
+                                 pbest, cand_out, st));
+  return release_ws(st);
+}
+
+int afm_pso_shard_move(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                       int32_t n_dims, int32_t n_traces, uint64_t seed,
+                       int32_t iteration, int32_t do_move,
+                       int64_t first_particle, const double* gathered,
+                       int32_t n_ranks, double* x, double* v,
+                       const double* pbest, double* gbest, double* gbestJ,
+                       double* theta_star, double* J_star, void* cuda_stream) {
+  if (n_dims < 1 || n_dims > 4) return fail(AFM_EINVAL, "n_dims must be 1..4");
+  if (n_traces < 1) return fail(AFM_EINVAL, "n_traces must be >= 1");
+  if (n_ranks < 1) return fail(AFM_EINVAL, "n_ranks must be >= 1");
+  if (iteration < 0) return fail(AFM_EINVAL, "iteration must be >= 0");
+  if (first_particle < 0) return fail(AFM_EINVAL, "first_particle must be >= 0");
+  int rc = validate_bounds(bounds, n_dims);
+  if (rc) return rc;
+  if ((rc = validate_swarm(swarm))) return rc;
+  if (!gathered || !x || !v || !pbest || !gbest || !gbestJ)
+    return fail(AFM_EINVAL, "NULL swarm array");
+  if ((rc = check_device())) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  BoxDev box = make_box(bounds, n_dims);
+  SwarmDev sw = {swarm->w, swarm->c1, swarm->c2};
+  LAUNCHED(launch_pso_shard_gbest(box, n_dims, n_traces, n_ranks, gathered, gbest,
+                                  gbestJ, theta_star, J_star, st));
+  if (do_move)
+    LAUNCHED(launch_pso_move(box, sw, n_dims, swarm->n_particles, n_traces, seed,
+                             first_particle, (uint32_t)iteration, 1, nullptr, x,
+                             v, pbest, nullptr, gbest, nullptr, st));
+  return AFM_OK;
 }
 
 int afm_philox4x32_10(const uint32_t* ctr, int64_t n, const uint32_t* key,

@@ -18,7 +18,7 @@
 // a 1e-4..1e-3 relative misfit error.  The first-order residuals of everything
 // that is rounded once and used every step are therefore added back into the
 // lo parts once per step:
-//     cc = -beta6_lo d_mid - alpha6_lo w_mid - beta6 d_lo - alpha6 w_lo
+//     cc = -beta6_lo d_mid - alpha6_lo w_mid - beta6 d_lo
 // (d_mid, w_mid: stage-2 values = the weighted mean stage argument to first
 // order) enters w' with weight 6 and d' with weight 3, and the stream carries
 // e_w = exact (s0 + 4 sh + s1)/6 minus the float sum actually used.
@@ -123,18 +123,23 @@ __device__ __forceinline__ void commit32(const Model32& M, State32& S, float g1,
   const float t23 = g2 + g3;
   const float s3 = g1 + t23;
   const float X = (s3 + t23) + g4;
-  const float cc = fmaf(M.nbeta_lo, d2, M.nalpha_lo * w2) +
-                   fmaf(M.nbeta, S.dl, M.nalpha * S.wl);
-  // d' = d + w + s3 (+ 3 cc): the large part w_hi by an error-free sum
-  float sd, e;
-  two_sum32(S.dh, S.wh, sd, e);
-  const float lo = __fadd_rn(__fadd_rn(S.dl, __fadd_rn(s3, fmaf(3.0f, cc, S.wl))), e);
+  const float cc = fmaf(M.nbeta, S.dl, fmaf(M.nbeta_lo, d2, M.nalpha_lo * w2));
+  // d' = d + w + s3 (+ 3 cc).  The large part w_hi is added by a fast two-sum:
+  // exact while |d_hi| >= |w_hi|; when the gap is smaller than one step's
+  // travel (deep contact) its error is <= ulp(w_hi) ~ 1e-8 nm, once.
+  const float sd = __fadd_rn(S.dh, S.wh);
+  const float e = __fsub_rn(S.wh, __fsub_rn(sd, S.dh));
+  const float lo =
+      __fadd_rn(__fadd_rn(S.dl, __fadd_rn(s3, fmaf(3.0f, cc, S.wl))), e);
   const float dn = __fadd_rn(sd, lo);
   S.dl = __fsub_rn(lo, __fsub_rn(dn, sd));
   S.dh = dn;
-  // w' = w + X (+ 6 cc + ew)
+  // w' = w + X (+ 6 cc + ew): |X| << |w_hi| except where w crosses zero, and
+  // there the error is <= ulp(X) -- the rounding X carries anyway
   const float t = __fadd_rn(__fadd_rn(S.wl, fmaf(6.0f, cc, ew)), X);
-  two_sum32(S.wh, t, S.wh, S.wl);
+  const float wn = __fadd_rn(S.wh, t);
+  S.wl = __fsub_rn(t, __fsub_rn(wn, S.wh));
+  S.wh = wn;
 }
 
 template <int LAW>

@@ -113,8 +113,8 @@ int launch_trajectory(const ModelConsts& mc, const double* theta_dev,
                       double* vs, cudaStream_t st);
 
 int launch_pso_init(const BoxDev& box, int D, int64_t per, int n_traces,
-                    uint64_t seed, double* x, double* v, double* pbest,
-                    double* pbestJ, double* gbest, double* gbestJ,
+                    uint64_t seed, int64_t first, double* x, double* v,
+                    double* pbest, double* pbestJ, double* gbest, double* gbestJ,
                     cudaStream_t st);
 int launch_pso_best(int D, int64_t per, int n_traces, const double* J,
                     const double* x, double* pbest, double* pbestJ, Cand* cand,
@@ -124,10 +124,17 @@ int launch_pso_gbest(const BoxDev& box, int D, int n_traces, int n_cand,
                      double* gbestJ, double* hist_row, double* theta_star,
                      double* J_star, cudaStream_t st);
 int launch_pso_move(const BoxDev& box, const SwarmDev& sw, int D, int64_t per,
-                    int n_traces, uint64_t seed, uint32_t it, int do_move,
-                    const double* J, double* x, double* v, const double* pbest,
-                    const double* pbestJ, const double* gbest, double* dump_row,
-                    cudaStream_t st);
+                    int n_traces, uint64_t seed, int64_t first, uint32_t it,
+                    int do_move, const double* J, double* x, double* v,
+                    const double* pbest, const double* pbestJ,
+                    const double* gbest, double* dump_row, cudaStream_t st);
+int launch_pso_shard_cand(int D, int n_traces, int n_cand, int64_t first,
+                          const Cand* cand, const double* pbest,
+                          double* cand_out, cudaStream_t st);
+int launch_pso_shard_gbest(const BoxDev& box, int D, int n_traces, int n_ranks,
+                           const double* gathered, double* gbest,
+                           double* gbestJ, double* theta_star, double* J_star,
+                           cudaStream_t st);
 int launch_fma_peak(int precision, int iters, int blocks, int threads,
                     void* sink, float* ms, cudaStream_t st);
 int launch_philox(const uint32_t* ctr, int64_t n, uint32_t k0, uint32_t k1,

@@ -320,7 +320,8 @@ __global__ void trajectory_kernel(ModelConsts mc, const double* __restrict__ th,
 // contraction changes the value: the swarm state replays bit for bit.
 // ============================================================================
 __global__ void pso_init_kernel(BoxDev box, int D, int64_t per, int n_traces,
-                                uint64_t seed, double* __restrict__ x,
+                                uint64_t seed, int64_t first,
+                                double* __restrict__ x,
                                 double* __restrict__ v,
                                 double* __restrict__ pbest,
                                 double* __restrict__ pbestJ,
@@ -330,8 +331,8 @@ __global__ void pso_init_kernel(BoxDev box, int D, int64_t per, int n_traces,
   const int64_t PT = per * n_traces;
   if (gp >= PT) return;
   double a[4], b[4];
-  pso_uniforms(seed, (uint64_t)gp, 0u, 0u, D, a, b);
-  const bool first = (gp % per) == 0;
+  pso_uniforms(seed, (uint64_t)(first + gp), 0u, 0u, D, a, b);
+  const bool head = (gp % per) == 0;
   const int64_t s = gp / per;
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
@@ -342,11 +343,11 @@ __global__ void pso_init_kernel(BoxDev box, int D, int64_t per, int n_traces,
       x[gp * D + j] = x0;
       v[gp * D + j] = __dmul_rn(0.5, __dsub_rn(y0, x0));
       pbest[gp * D + j] = x0;
-      if (first) gbest[s * D + j] = x0;
+      if (head) gbest[s * D + j] = x0;
     }
   }
   pbestJ[gp] = CUDART_INF;
-  if (first) gbestJ[s] = CUDART_INF;
+  if (head) gbestJ[s] = CUDART_INF;
 }
 
 // Personal best from caller-supplied J + block candidates (the stand-alone
@@ -421,10 +422,76 @@ __global__ void pso_gbest_kernel(BoxDev box, int D, int n_cand,
   }
 }
 
+// Sharded swarm: this process's best candidate of every local
+// trace, in a form that can be exchanged: row s = { pbestJ, global particle
+// index (exact in a double below 2^53), pbest x[D] }.
+__global__ void pso_shard_cand_kernel(int D, int n_cand, int64_t first,
+                                      const Cand* __restrict__ cand,
+                                      const double* __restrict__ pbest,
+                                      double* __restrict__ cand_out) {
+  __shared__ Cand red[32];
+  const int s = blockIdx.x;
+  double Jm = CUDART_INF;
+  long long im = 0x7fffffffffffffffLL;
+  for (int c = threadIdx.x; c < n_cand; c += blockDim.x) {
+    const Cand cd = cand[(int64_t)s * n_cand + c];
+    if (cand_less(cd.J, cd.idx, Jm, im)) {
+      Jm = cd.J;
+      im = cd.idx;
+    }
+  }
+  block_argmin(Jm, im, red);
+  if (threadIdx.x == 0) {
+    double* r = cand_out + (int64_t)s * (D + 2);
+    r[0] = Jm;
+    r[1] = (double)(first + im);
+    for (int j = 0; j < D; ++j) r[2 + j] = pbest[im * D + j];
+  }
+}
+
+// Global best of every local trace from the candidates of all ranks
+// (gathered [n_ranks][n_traces][D+2]): lowest global index among the minima,
+// taken only on a strict improvement -- the rule of pso_gbest_kernel.
+__global__ void pso_shard_gbest_kernel(BoxDev box, int D, int n_traces,
+                                       int n_ranks,
+                                       const double* __restrict__ gathered,
+                                       double* __restrict__ gbest,
+                                       double* __restrict__ gbestJ,
+                                       double* __restrict__ theta_star,
+                                       double* __restrict__ J_star) {
+  const int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n_traces) return;
+  double Jm = CUDART_INF;
+  long long im = 0x7fffffffffffffffLL;
+  int rm = -1;
+  for (int r = 0; r < n_ranks; ++r) {
+    const double* row = gathered + ((int64_t)r * n_traces + s) * (D + 2);
+    const long long idx = (long long)row[1];
+    if (cand_less(row[0], idx, Jm, im)) {
+      Jm = row[0];
+      im = idx;
+      rm = r;
+    }
+  }
+  double gJ = gbestJ[s];
+  if (rm >= 0 && Jm < gJ) {
+    gJ = Jm;
+    gbestJ[s] = Jm;
+    const double* row = gathered + ((int64_t)rm * n_traces + s) * (D + 2);
+    for (int j = 0; j < D; ++j) gbest[s * D + j] = row[2 + j];
+  }
+  for (int j = 0; j < D; ++j) {
+    const double g = gbest[s * D + j];
+    if (theta_star) theta_star[s * D + j] = box.lg[j] ? pow(10.0, g) : g;
+  }
+  if (J_star) J_star[s] = gJ;
+}
+
 // Optional dump, then Eq. 8, x <- x + v, clamp + zero velocity.
 __global__ void pso_move_kernel(BoxDev box, SwarmDev sw, int D, int64_t per,
-                                int n_traces, uint64_t seed, uint32_t it,
-                                int do_move, const double* __restrict__ J,
+                                int n_traces, uint64_t seed, int64_t first,
+                                uint32_t it, int do_move,
+                                const double* __restrict__ J,
                                 double* __restrict__ x, double* __restrict__ v,
                                 const double* __restrict__ pbest,
                                 const double* __restrict__ pbestJ,
@@ -458,7 +525,7 @@ __global__ void pso_move_kernel(BoxDev box, SwarmDev sw, int D, int64_t per,
   }
   if (!do_move) return;
   double r1[4], r2[4];
-  pso_uniforms(seed, (uint64_t)gp, it, 1u, D, r1, r2);
+  pso_uniforms(seed, (uint64_t)(first + gp), it, 1u, D, r1, r2);
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
     if (j < D) {
@@ -562,13 +629,14 @@ int launch_trajectory(const ModelConsts& mc, const double* theta_dev,
 }
 
 int launch_pso_init(const BoxDev& box, int D, int64_t per, int n_traces,
-                    uint64_t seed, double* x, double* v, double* pbest,
+                    uint64_t seed, int64_t first, double* x, double* v,
+                    double* pbest,
                     double* pbestJ, double* gbest, double* gbestJ,
                     cudaStream_t st) {
   const int64_t PT = per * n_traces;
   const int threads = 128;
   pso_init_kernel<<<(unsigned)((PT + threads - 1) / threads), threads, 0, st>>>(
-      box, D, per, n_traces, seed, x, v, pbest, pbestJ, gbest, gbestJ);
+      box, D, per, n_traces, seed, first, x, v, pbest, pbestJ, gbest, gbestJ);
   return 1;
 }
 
@@ -592,15 +660,36 @@ int launch_pso_gbest(const BoxDev& box, int D, int n_traces, int n_cand,
 }
 
 int launch_pso_move(const BoxDev& box, const SwarmDev& sw, int D, int64_t per,
-                    int n_traces, uint64_t seed, uint32_t it, int do_move,
-                    const double* J, double* x, double* v, const double* pbest,
+                    int n_traces, uint64_t seed, int64_t first, uint32_t it,
+                    int do_move, const double* J, double* x, double* v,
+                    const double* pbest,
                     const double* pbestJ, const double* gbest, double* dump_row,
                     cudaStream_t st) {
   const int64_t PT = per * n_traces;
   const int threads = 128;
   pso_move_kernel<<<(unsigned)((PT + threads - 1) / threads), threads, 0, st>>>(
-      box, sw, D, per, n_traces, seed, it, do_move, J, x, v, pbest, pbestJ,
-      gbest, dump_row);
+      box, sw, D, per, n_traces, seed, first, it, do_move, J, x, v, pbest,
+      pbestJ, gbest, dump_row);
+  return 1;
+}
+
+int launch_pso_shard_cand(int D, int n_traces, int n_cand, int64_t first,
+                          const Cand* cand, const double* pbest,
+                          double* cand_out, cudaStream_t st) {
+  int threads = n_cand <= 32 ? 32 : (n_cand <= 64 ? 64 : 128);
+  pso_shard_cand_kernel<<<(unsigned)n_traces, threads, 0, st>>>(
+      D, n_cand, first, cand, pbest, cand_out);
+  return 1;
+}
+
+int launch_pso_shard_gbest(const BoxDev& box, int D, int n_traces, int n_ranks,
+                           const double* gathered, double* gbest,
+                           double* gbestJ, double* theta_star, double* J_star,
+                           cudaStream_t st) {
+  const int threads = 64;
+  pso_shard_gbest_kernel<<<(unsigned)((n_traces + threads - 1) / threads),
+                           threads, 0, st>>>(box, D, n_traces, n_ranks, gathered,
+                                             gbest, gbestJ, theta_star, J_star);
   return 1;
 }
 

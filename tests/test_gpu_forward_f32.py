@@ -51,10 +51,12 @@ def _oracle(wl, params, trace, z0v0=None):
 def _check_bulk_and_outliers(wl, params, trace, z0v0, Jg, Jo, label, max_outliers):
     """SURVEY.md 8(c) c-15 protocol.  Every particle must meet TOL_F32 unless the
     ORACLE ITSELF is ill-conditioned there: a 1e-10 relative change of theta or
-    of the initial state moves the oracle's own J by more than 1e-6 relative
-    (amplification > 1e4, so that the ~1e-7 roundings of any FP32 scheme exceed
-    1e-3; the paper cites chaotic tip dynamics, PAPER.md ref [12]).  At most
+    of the initial state moves the oracle's own J by more than ILL = 2.1e-7
+    relative, i.e. the amplification exceeds 2.1e3 and a ONE-ulp FP32
+    perturbation (2^-23) of the inputs alone already moves J by TOL_F32/4 (the
+    paper cites chaotic tip dynamics, PAPER.md ref [12]).  At most
     `max_outliers` such particles, each one verified."""
+    ILL = 0.25 * TOL_F32 / 2.0 ** -23 * 1e-10
     fin = np.isfinite(Jo)
     assert np.array_equal(np.isfinite(Jg), fin)
     e = rel_err(Jg, Jo)
@@ -80,7 +82,7 @@ def _check_bulk_and_outliers(wl, params, trace, z0v0, Jg, Jo, label, max_outlier
             moved = max(moved, abs(J2 - J0) / J0)
         print("  outlier %d: err %.2e, oracle moves %.2e under a 1e-10 perturbation"
               % (i, e[i], moved))
-        assert moved > 1e-6, (int(i), e[i], moved)
+        assert moved > ILL, (int(i), e[i], moved)
     return e
 
 
@@ -187,19 +189,23 @@ def test_f32_edge_cases(afm):
 
 
 def test_f32_divergence_gives_inf(afm):
-    """Blow-ups are +Inf (R12); verdicts compared where the oracle's own verdict
-    survives a 1e-6 relative change of theta (the FP32 rounding of theta)."""
+    """Blow-ups are +Inf (R12).  Whether RK4 blows up at the d^-8 wall is itself
+    chaotic for the marginal particles, so verdicts are compared where the
+    oracle's own verdict survives 1e-6..1e-4 relative changes of theta and z0."""
     base = wlm.scaled(wlm.config(3), n_cycles=6, n_skip_cycles=3)
     trace = np.zeros((1, base["n_window"]))
     params = wlm.draw_params(base, 64, seed=9)
     wl = dict(base, cantilever=dict(base["cantilever"], z_c=15e-9))
     Jo = _oracle(wl, params, trace)
-    Jo2 = _oracle(wl, params * (1 + 1e-6), trace)
-    Jo3 = _oracle(wl, params * (1 - 1e-6), trace)
     Jg = _gpu(afm, wl, params, trace)
     assert not np.isnan(Jg).any()
-    robust = (np.isinf(Jo) == np.isinf(Jo2)) & (np.isinf(Jo) == np.isinf(Jo3))
-    robust &= (rel_err(Jo2, Jo) < 1e-4) & (rel_err(Jo3, Jo) < 1e-4)
+    robust = np.ones(len(Jo), dtype=bool)
+    M = orc.model_from(wl)
+    for eps in (1e-6, -1e-6, 1e-5, -1e-5, 1e-4, -1e-4):
+        J1 = _oracle(wl, params * (1 + eps), trace)
+        J2 = orc.forward_batch(M, params, trace, z0=wl["z0"] + eps * 1e-9, v0=wl["v0"],
+                               openmp=True)
+        robust &= (np.isinf(J1) == np.isinf(Jo)) & (np.isinf(J2) == np.isinf(Jo))
     assert robust.sum() > 16 and np.isinf(Jo[robust]).sum() > 4
     assert np.array_equal(np.isinf(Jg)[robust], np.isinf(Jo)[robust])
 
