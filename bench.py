@@ -286,6 +286,7 @@ def run_ours(args):
         flops = FLOPS_PER_STEP[wl["law"]] * P * N
         achieved = flops / (kern_ms * 1e-3) / 1e12
         peak = pk["fp32_tflops"] if prec == afm.F32 else pk["fp64_tflops"]
+        peak_meas = afm.afm_fma_peak(prec, 0.25)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup,
@@ -310,10 +311,14 @@ def run_ours(args):
                          "kernel_ms": kern_ms,
                          "peak_source": "lane model 148 SM x %d lanes x 2 x %s (%s)" % (
                              FP32_LANES if prec == afm.F32 else FP64_LANES,
-                             pk["clock_mhz"], pk["clock_source"])},
+                             pk["clock_mhz"], pk["clock_source"]),
+                         "peak_measured": peak_meas,
+                         "frac_of_measured": achieved / peak_meas,
+                         "peak_measured_source": "afm_fma_peak: register-only FMA "
+                                                 "chains, 0.25 s, this run"},
         }
         if not args.no_extras and world == 1:
-            out["extras"] = extras(afm, torch, dev)
+            out["extras"] = extras(afm, torch, dev, prec)
             n_s = args.cpu_particles
             dt, _ = _oracle_sample(wl, n_s, 1, 2, _oracle_trace(wl))
             out["cpu_baseline"] = {
@@ -328,16 +333,72 @@ def run_ours(args):
     return 0
 
 
-def extras(afm, torch, dev):
-    """Secondary figures of BASELINE.json:metric: forward-batch latency and
-    inversion wall time (host clock, call to return) of configs[0] and [2]."""
-    ex = {}
+def _event_ms(torch, fn, reps):
+    fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def extras(afm, torch, dev, main_prec):
+    """Secondary figures of BASELINE.json:metric (not the headline): measured FMA
+    peaks, configs[1] in the other precision, one forward batch of configs[3]
+    and [4] at full size, and the inversion wall time (host clock, call to
+    return) of configs[0] and [2]."""
+    ex = {"fma_peak_measured_tflops": {"f64": afm.afm_fma_peak(afm.F64, 0.25),
+                                       "f32": afm.afm_fma_peak(afm.F32, 0.25)}}
+
+    def trace_of(wl, truths=None):
+        cfg = afm.cfg_from(wl)
+        T = wl["n_traces"]
+        tl = [wl["truth"]] if truths is None else truths
+        rows = [afm.afm_trajectory(tl[s], cfg, wl["z0"], wl["v0"])[0][-wl["n_window"]:]
+                for s in range(T)]
+        return torch.as_tensor(np.stack(rows) + wlm.trace_noise(wl), device=dev)
+
+    # configs[1] in the other precision (kernel only, CUDA events)
+    wl = wlm.config(1)
+    P = wl["swarm"]["n_particles"]
+    other = afm.F64 if main_prec == afm.F32 else afm.F32
+    params = torch.as_tensor(wlm.draw_params(wl, P, seed=1), device=dev)
+    z0v0 = torch.as_tensor(wlm.draw_initial_states(wl, P, seed=2), device=dev)
+    tr = trace_of(wl)
+    out = torch.empty(P, dtype=torch.float64, device=dev)
+    cfg = afm.cfg_from(wl, precision=other)
+    ms = _event_ms(torch, lambda: afm.afm_forward_batch(params, tr, cfg, z0v0=z0v0,
+                                                        misfit=out), 3)
+    name = "f64" if other == afm.F64 else "f32"
+    ex["cfg1_%s_forward_ms" % name] = ms
+    ex["cfg1_%s_particle_steps_per_s" % name] = P * wl["n_steps"] / (ms * 1e-3)
+
+    # one full-size forward batch of configs[3] (both precisions) and configs[4]
+    for ci, precs in ((3, (afm.F64, afm.F32)), (4, (afm.F64,))):
+        wl = wlm.config(ci)
+        T, per = wl["n_traces"], wl["swarm"]["n_particles"]
+        truths = None if wl["truth"] is not None else wlm.pixel_truths(wl)
+        tr = trace_of(wl, truths)
+        params = torch.as_tensor(wlm.draw_params(wl, T * per, seed=1), device=dev)
+        out = torch.empty(T * per, dtype=torch.float64, device=dev)
+        for prec in precs:
+            cfg = afm.cfg_from(wl, precision=prec)
+            ms = _event_ms(torch, lambda: afm.afm_forward_batch(params, tr, cfg,
+                                                                misfit=out), 2)
+            name = "f64" if prec == afm.F64 else "f32"
+            ex["cfg%d_%s_batch_ms" % (ci, name)] = ms
+            ex["cfg%d_%s_particle_steps_per_s" % (ci, name)] = \
+                T * per * wl["n_steps"] / (ms * 1e-3)
+            ex["cfg%d_%s_full_inversion_s_extrapolated" % (ci, name)] = \
+                ms * 1e-3 * wl["swarm"]["n_iters"]
+
     for ci in (0, 2):
         wl = wlm.config(ci)
         cfg = afm.cfg_from(wl)
-        zs, _ = afm.afm_trajectory(wl["truth"], cfg, wl["z0"], wl["v0"])
-        trace = torch.as_tensor(zs[-wl["n_window"]:][None, :] + wlm.trace_noise(wl),
-                                device=dev)
+        trace = trace_of(wl)
         b, s = afm.bounds_from(wl), afm.swarm_from(wl)
         afm.afm_pso_invert(b, s, wl["pso_seed"], trace, cfg)       # warm-up
         t0 = time.perf_counter()
@@ -354,7 +415,7 @@ def extras(afm, torch, dev):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])

@@ -258,7 +258,9 @@ void afm_reset_launch_count(void);
 
 /* Tuning knobs (optional).  name: "block" (threads per CTA of the integrate
  * kernel: 32, 64 or 128; 0 = auto), "tile" (steps per time tile; 0 = auto),
- * "ppt" (particles per thread: 1 or 2; 0 = auto).
+ * "ppt" (particles per thread: 1 or 2; 0 = auto), "form" (FP64 kernel form:
+ * 1 = throughput, fewest FP64 instructions; 2 = latency, shortest dependent
+ * chains; 0 = auto by warps per SM sub-partition).
  * Returns AFM_EINVAL for an unknown name or value. */
 int afm_set_option(const char* name, int64_t value);
 

@@ -53,6 +53,8 @@ int fail(int code, const char* fmt, ...) {
 int g_opt_block = 0;  // 0 = auto
 int g_opt_tile = 0;   // 0 = auto
 int g_opt_ppt = 0;    // 0 = auto
+int g_opt_form = 0;   // 0 = auto, 1 = throughput form, 2 = latency form
+int g_n_sm = 148;
 
 // ---- grow-only device workspace ------------------------------------------------
 struct Buffer {
@@ -106,6 +108,7 @@ int check_device() {
     return fail(AFM_EUNSUPPORTED,
                 "device %s is sm_%d%d; this library is built for sm_100a only",
                 prop.name, prop.major, prop.minor);
+  g_n_sm = prop.multiProcessorCount;
   g_ws.checked_device = true;
   return AFM_OK;
 }
@@ -276,6 +279,17 @@ int pick_ppt(int64_t per, int n_traces) {
   return 1;
 }
 
+// Kernel form of the FP64 integrate kernel (afm_device.cuh, vdw_plus): the
+// latency form below two warps per SM sub-partition, where nothing hides the
+// dependent chains; the throughput form (fewest FP64 instructions) above.
+int pick_variant(int64_t per, int n_traces, int ppt) {
+  if (ppt == 2) return 2;
+  if (g_opt_form == 1) return 0;
+  if (g_opt_form == 2) return 1;
+  const int64_t warps = ((per + 31) / 32) * n_traces;
+  return warps < (int64_t)2 * 4 * g_n_sm ? 1 : 0;
+}
+
 BoxDev make_box(const afm_bounds* b, int D) {
   BoxDev bd;
   memset(&bd, 0, sizeof(bd));
@@ -342,7 +356,7 @@ int forward_locked(const double* params, int64_t P, const double* trace,
     LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
     return release_ws(st);
   }
-  LAUNCHED(launch_integrate_f64(mc, io, block, ppt, st));
+  LAUNCHED(launch_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st));
   return release_ws(st);
 }
 
@@ -543,7 +557,7 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
     if (f32)
       LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
     else
-      LAUNCHED(launch_integrate_f64(mc, io, block, ppt, st));
+      LAUNCHED(launch_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st));
     LAUNCHED(launch_pso_gbest(
         box, D, T, bpt, (Cand*)g_ws.cand.p, pbest, gbest, gbestJ,
         gbest_hist ? gbest_hist + (size_t)it * T * (D + 1) : nullptr, th_dev,
@@ -673,7 +687,7 @@ int afm_pso_shard_eval(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   if (f32)
     LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
   else
-    LAUNCHED(launch_integrate_f64(mc, io, block, ppt, st));
+    LAUNCHED(launch_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st));
   LAUNCHED(launch_pso_shard_cand(D, T, bpt, first_particle, (Cand*)g_ws.cand.p,
                                  pbest, cand_out, st));
   return release_ws(st);
@@ -798,6 +812,11 @@ int afm_set_option(const char* name, int64_t value) {
   if (!strcmp(name, "ppt")) {
     if (value < 0 || value > 2) return fail(AFM_EINVAL, "ppt must be 0, 1 or 2");
     g_opt_ppt = (int)value;
+    return AFM_OK;
+  }
+  if (!strcmp(name, "form")) {
+    if (value < 0 || value > 2) return fail(AFM_EINVAL, "form must be 0, 1 or 2");
+    g_opt_form = (int)value;
     return AFM_OK;
   }
   if (!strcmp(name, "tile")) {

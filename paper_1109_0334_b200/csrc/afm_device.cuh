@@ -39,6 +39,18 @@ __device__ __forceinline__ double rcp_fast(double q) {
   double p = fma(e, e, e);  // e + e^2
   return fma(r0, p, r0);
 }
+// c/q + b with the correction folded into the sum: c r0 (1 + p) + b =
+// (c r0) p + (c r0 + b).  The two products with r0 run beside the e -> p chain,
+// so the result is one dependent FMA after p instead of two (the stage-to-stage
+// recurrence of the RK4 step is latency-bound at low occupancy).
+__device__ __forceinline__ double vdw_plus(double c, double q, double b) {
+  const double r0 = rcp_seed(q);
+  const double e = fma(-q, r0, 1.0);
+  const double cr0 = c * r0;
+  const double cb = fma(c, r0, b);
+  const double p = fma(e, e, e);
+  return fma(cr0, p, cb);
+}
 // sqrt(x), x > 0 normal: g0 = x y0, e = 1 - x y0^2,
 // sqrt(x) = g0 (1 - e)^(-1/2) = g0 (1 + e/2 + 3 e^2/8 + 5 e^3/16 + ...);
 // truncated after e^2: relative error (5/16) e^3 <= 2^-58.
@@ -75,23 +87,31 @@ __device__ __forceinline__ bool ge_pos(double d, long long a0_bits) {
 
 // Free-flight (d >= a0) side of the DMT laws, and the whole of law NONE when
 // c0 = 0 is skipped by the caller.
+template <bool LAT>
 __device__ __forceinline__ double accel_free(const Particle64& P, double s,
                                              double d, double w) {
-  const double part = fma(P.c0, rcp_fast(d * d), fma(P.nbeta, d, s));
-  return fma(P.nalpha, w, part);
+  const double b0 = fma(P.nbeta, d, s);
+  if (LAT) return fma(P.nalpha, w, vdw_plus(P.c0, d * d, b0));
+  return fma(P.nalpha, w, fma(P.c0, rcp_fast(d * d), b0));
 }
 
 // DMT laws, both sides evaluated and selected per lane (straight-line code: the
-// reciprocal and the square-root chains overlap).  A lane on the other side
-// feeds its unused chain a harmless argument (rsqrt of a negative number is NaN
-// and is never selected).  The free-flight value is computed exactly as in
-// accel_free, so a lane's result does not depend on which form ran.
-template <int LAW>
+// reciprocal and the square-root chains are independent and overlap).  A lane
+// on the other side feeds its unused chain a harmless argument (rsqrt of a
+// negative number is NaN and is never selected).  The free-flight value is
+// computed exactly as in accel_free<LAT>, so within one form a lane's result
+// does not depend on which path ran.
+// (Measured and rejected: one shared rsqrt chain on a per-lane selected argument
+// with selected tail coefficients -- 14 instead of 19 FP64 instructions per
+// stage, but ten more 32-bit selects; 19.8 ms against 19.1 ms on configs[1].)
+template <int LAW, bool LAT>
 __device__ __forceinline__ double accel_both(const Particle64& P, double s,
                                              double d, double w,
                                              long long a0_bits) {
   const double b0 = fma(P.nbeta, d, s);
-  const double g_free = fma(P.nalpha, w, fma(P.c0, rcp_fast(d * d), b0));
+  const double g_free =
+      LAT ? fma(P.nalpha, w, vdw_plus(P.c0, d * d, b0))
+          : fma(P.nalpha, w, fma(P.c0, rcp_fast(d * d), b0));
   const double del = P.a0 - d;
   const double sq = sqrt_fast(del);
   const double part = fma(P.c1 * del, sq, P.c2 + b0);
@@ -167,7 +187,7 @@ __device__ __forceinline__ bool diverged_step(double d, const DivergeTest& T) {
   return false;
 }
 
-template <int LAW, int PPT>
+template <int LAW, int PPT, bool LAT>
 __device__ __forceinline__ void rk4_step(const Particle64 (&P)[PPT], double s0,
                                          double sh, double s1,
                                          long long a0_bits, double (&d)[PPT],
@@ -204,14 +224,14 @@ __device__ __forceinline__ void rk4_step(const Particle64 (&P)[PPT], double s0,
     unsigned hmax = 0u;
 #pragma unroll
     for (int q = 0; q < PPT; ++q) {
-      const double k1 = accel_free(P[q], s0, d[q], w[q]);
+      const double k1 = accel_free<LAT>(P[q], s0, d[q], w[q]);
       const double w2 = fma(0.5, k1, w[q]);
-      const double k2 = accel_free(P[q], sh, d2[q], w2);
+      const double k2 = accel_free<LAT>(P[q], sh, d2[q], w2);
       const double w3 = fma(0.5, k2, w[q]);
       const double d3 = fma(0.5, w2, d[q]);
-      const double k3 = accel_free(P[q], sh, d3, w3);
+      const double k3 = accel_free<LAT>(P[q], sh, d3, w3);
       const double d4 = d[q] + w3;
-      const double k4 = accel_free(P[q], s1, d4, w[q] + k3);
+      const double k4 = accel_free<LAT>(P[q], s1, d4, w[q] + k3);
       m = min(m, min(min(__double2hiint(d[q]), __double2hiint(d2[q])),
                      min(__double2hiint(d3), __double2hiint(d4))));
       const double t23 = k2 + k3;
@@ -240,14 +260,14 @@ __device__ __forceinline__ void rk4_step(const Particle64 (&P)[PPT], double s0,
   int m = 0x7fffffff;
 #pragma unroll
   for (int q = 0; q < PPT; ++q) {
-    const double k1 = accel_both<LAW>(P[q], s0, d[q], w[q], a0_bits);
+    const double k1 = accel_both<LAW, LAT>(P[q], s0, d[q], w[q], a0_bits);
     const double w2 = fma(0.5, k1, w[q]);
-    const double k2 = accel_both<LAW>(P[q], sh, d2[q], w2, a0_bits);
+    const double k2 = accel_both<LAW, LAT>(P[q], sh, d2[q], w2, a0_bits);
     const double w3 = fma(0.5, k2, w[q]);
     const double d3 = fma(0.5, w2, d[q]);
-    const double k3 = accel_both<LAW>(P[q], sh, d3, w3, a0_bits);
+    const double k3 = accel_both<LAW, LAT>(P[q], sh, d3, w3, a0_bits);
     const double d4 = d[q] + w3;
-    const double k4 = accel_both<LAW>(P[q], s1, d4, w[q] + k3, a0_bits);
+    const double k4 = accel_both<LAW, LAT>(P[q], s1, d4, w[q] + k3, a0_bits);
     m = min(m, min(min(__double2hiint(d[q]), __double2hiint(d2[q])),
                    min(__double2hiint(d3), __double2hiint(d4))));
     const double t23 = k2 + k3;

@@ -105,7 +105,7 @@ int launch_build_stream(const ModelConsts& mc, const double* trace, int n_traces
 int launch_build_stream_f32(const ModelConstsF32& mf, const double* trace,
                             int n_traces, float* stream, cudaStream_t st);
 int launch_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block,
-                         int ppt, cudaStream_t st);
+                         int variant, cudaStream_t st);
 int launch_integrate_f32(const ModelConstsF32& mf, const IntegrateIO& io,
                          int block, int ppt, cudaStream_t st);
 int launch_trajectory(const ModelConsts& mc, const double* theta_dev,

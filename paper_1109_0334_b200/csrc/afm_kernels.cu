@@ -113,7 +113,7 @@ __global__ void build_stream_kernel(ModelConsts mc,
 // integrate-and-misfit, FP64
 // ============================================================================
 // T steps of one time tile, [i0, i1), with (WIN) or without the misfit sum.
-template <int LAW, int PPT, bool WIN>
+template <int LAW, int PPT, bool LAT, bool WIN>
 __device__ __forceinline__ void run_steps(const double4* sp, int i0, int i1,
                                           const Particle64 (&P)[PPT],
                                           long long a0_bits,
@@ -128,7 +128,7 @@ __device__ __forceinline__ void run_steps(const double4* sp, int i0, int i1,
     // next row fetched one step ahead; the fetch past the last row of a tile
     // lands in the other stage or the padding and is discarded
     const double4 rn = sp[i + 1];
-    rk4_step<LAW, PPT>(P, r.x, r.y, r.z, a0_bits, d, w, mode, bad, T);
+    rk4_step<LAW, PPT, LAT>(P, r.x, r.y, r.z, a0_bits, d, w, mode, bad, T);
     if (WIN) {
 #pragma unroll
       for (int q = 0; q < PPT; ++q) {
@@ -143,7 +143,7 @@ __device__ __forceinline__ void run_steps(const double4* sp, int i0, int i1,
 // PPT particles per thread: particle q of a thread is local index
 // base + q * blockDim.x + tid (coalesced).  PPT = 2 interleaves two independent
 // dependency chains per thread for the throughput-bound batches.
-template <int LAW, int MODE, int PPT>
+template <int LAW, int MODE, int PPT, bool LAT>
 __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
                                      int blocks_per_tr) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -233,8 +233,8 @@ __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
     const int n_steps = min(mc.T, mc.N - n_begin);
     // steps [0, k0) of this tile precede the misfit window
     const int k0 = max(0, min(n_steps, mc.n0 - n_begin));
-    run_steps<LAW, PPT, false>(sp, 0, k0, P, a0_bits, T, d, w, J, bad, mode);
-    run_steps<LAW, PPT, true>(sp, k0, n_steps, P, a0_bits, T, d, w, J, bad, mode);
+    run_steps<LAW, PPT, LAT, false>(sp, 0, k0, P, a0_bits, T, d, w, J, bad, mode);
+    run_steps<LAW, PPT, LAT, true>(sp, k0, n_steps, P, a0_bits, T, d, w, J, bad, mode);
     __syncthreads();  // every thread is done reading stage st
     if (tid == 0 && tile + 2 < mc.n_tiles) {
       const int nb = (tile + 2) * mc.T;
@@ -308,7 +308,7 @@ __global__ void trajectory_kernel(ModelConsts mc, const double* __restrict__ th,
   const double4* rows = reinterpret_cast<const double4*>(stream);
   for (int n = 0; n < mc.N; ++n) {
     const double4 r = rows[n];
-    rk4_step<LAW, 1>(P, r.x, r.y, r.z, a0_bits, d, w, mode, bad, T);
+    rk4_step<LAW, 1, true>(P, r.x, r.y, r.z, a0_bits, d, w, mode, bad, T);
     if (zs && writer) zs[n + 1] = d[0] - mc.zc;
     if (vs && writer) vs[n + 1] = w[0] * inv_h;
   }
@@ -568,13 +568,13 @@ int launch_build_stream(const ModelConsts& mc, const double* trace, int n_traces
   return 1;
 }
 
-template <int LAW, int MODE, int PPT>
+template <int LAW, int MODE, int PPT, bool LAT>
 static int launch_integrate_t(const ModelConsts& mc, const IntegrateIO& io,
                               int block, cudaStream_t st) {
   const int bpt = blocks_per_trace(io.per, block * PPT);
   const unsigned grid = (unsigned)(bpt * io.n_traces);
   const size_t smem = (size_t)mc.T * 32 * 2 + 64;  // + barriers + over-read pad
-  auto kern = integrate_misfit_f64<LAW, MODE, PPT>;
+  auto kern = integrate_misfit_f64<LAW, MODE, PPT, LAT>;
   if (smem > 48 * 1024)
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                          (int)smem);
@@ -582,15 +582,20 @@ static int launch_integrate_t(const ModelConsts& mc, const IntegrateIO& io,
   return 1;
 }
 
+// variant: 0 = throughput form, 1 = latency form (short dependent chains),
+// 2 = two particles per thread (throughput form)
 int launch_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block,
-                         int ppt, cudaStream_t st) {
+                         int variant, cudaStream_t st) {
 #define AFM_DISPATCH(LAWV)                                                      \
   case LAWV:                                                                    \
-    if (ppt == 2)                                                               \
-      return io.mode ? launch_integrate_t<LAWV, 1, 2>(mc, io, block, st)        \
-                     : launch_integrate_t<LAWV, 0, 2>(mc, io, block, st);       \
-    return io.mode ? launch_integrate_t<LAWV, 1, 1>(mc, io, block, st)          \
-                   : launch_integrate_t<LAWV, 0, 1>(mc, io, block, st);
+    if (variant == 2)                                                           \
+      return io.mode ? launch_integrate_t<LAWV, 1, 2, false>(mc, io, block, st) \
+                     : launch_integrate_t<LAWV, 0, 2, false>(mc, io, block, st);\
+    if (variant == 1)                                                           \
+      return io.mode ? launch_integrate_t<LAWV, 1, 1, true>(mc, io, block, st)  \
+                     : launch_integrate_t<LAWV, 0, 1, true>(mc, io, block, st); \
+    return io.mode ? launch_integrate_t<LAWV, 1, 1, false>(mc, io, block, st)   \
+                   : launch_integrate_t<LAWV, 0, 1, false>(mc, io, block, st);
   switch (mc.law) {
     AFM_DISPATCH(AFM_LAW_NONE)
     AFM_DISPATCH(AFM_LAW_DMT)

@@ -12,7 +12,10 @@ Two ways to shard, both with every arithmetic step inside the CUDA library:
   loop at all; the per-pixel results are gathered once at the end.
 
 Philox counters and the tie-break use GLOBAL particle indices, so a sharded
-run replays the single-process afm_pso_invert bit for bit (FP64).
+run replays the single-process afm_pso_invert: bit for bit while both run the
+same form of the FP64 kernel (include/afm.h, option "form"; the auto choice
+depends on the local particle count), otherwise with misfits equal to ~1e-15
+relative and the same swarm unless two misfits tie at that level.
 
 This module holds no arithmetic of the method: it partitions index ranges and
 moves candidate rows.  The compute calls go through a backend object with the

@@ -114,6 +114,29 @@ def test_forward_launch_shapes(afm, block, tile):
     assert rel_err(Jg, Jo).max() < TOL_F64
 
 
+@pytest.mark.parametrize("cfg_i", [1, 2])
+def test_forward_kernel_forms_agree(afm, cfg_i):
+    """The throughput form (fewest FP64 instructions) and the latency form
+    (vdW term folded so that one dependent FMA follows the correction) of the
+    FP64 kernel: each within 1e-9 of the oracle, within rounding of one another."""
+    wl = wlm.scaled(wlm.config(cfg_i), n_cycles=24, n_skip_cycles=12)
+    trace = oracle_trace(wl)
+    n = 517
+    params = wlm.draw_params(wl, n, seed=21)
+    z0v0 = wlm.draw_initial_states(wl, n, seed=22) if cfg_i == 1 else None
+    Jo = _oracle_forward(wl, params, trace, z0v0)
+    out = {}
+    for form in (1, 2):
+        afm.afm_set_option("form", form)
+        try:
+            out[form] = _gpu_forward(afm, wl, params, trace, z0v0)
+        finally:
+            afm.afm_set_option("form", 0)
+        assert rel_err(out[form], Jo).max() < TOL_F64, form
+    assert not np.array_equal(out[1], out[2])      # they really are two code paths
+    assert rel_err(out[1], out[2]).max() < 1e-10
+
+
 def test_forward_cfg1_shape_random_phases(afm):
     """configs[1] shape (S=256, random initial phases, log-uniform theta) at 40
     cycles on 2065 particles."""
