@@ -412,6 +412,47 @@ def extras(afm, torch, dev, main_prec):
     return ex
 
 
+def run_one_batch(args):
+    """--one-batch CFG: one full-size forward batch (or, with --invert, the full
+    inversion) of BASELINE.json configs[CFG], for ncu captures of the other
+    launch regimes.  Prints a small JSON line; NOT the bench line."""
+    import torch
+    from paper_1109_0334_b200 import afm
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    wl = wlm.config(args.one_batch)
+    prec = afm.F32 if args.precision == "f32" else afm.F64
+    cfg = afm.cfg_from(wl, precision=prec)
+    T, per = wl["n_traces"], wl["swarm"]["n_particles"]
+    truths = [wl["truth"]] if wl["truth"] is not None else wlm.pixel_truths(wl)
+    c64 = afm.cfg_from(wl)
+    rows = [afm.afm_trajectory(truths[s], c64, wl["z0"], wl["v0"])[0][-wl["n_window"]:]
+            for s in range(T)]
+    trace = torch.as_tensor(np.stack(rows) + wlm.trace_noise(wl), device=dev)
+    if args.invert:
+        b, sw = afm.bounds_from(wl), afm.swarm_from(wl)
+        afm.afm_pso_invert(b, sw, wl["pso_seed"], trace, cfg)
+        t0 = time.perf_counter()
+        r = afm.afm_pso_invert(b, sw, wl["pso_seed"], trace, cfg)
+        ms = (time.perf_counter() - t0) * 1e3
+        units = float(T) * per * wl["n_steps"] * sw.n_iters
+        print(json.dumps({"one_batch": args.one_batch, "mode": "inversion",
+                          "dtype": args.precision, "ms": ms,
+                          "particle_steps_per_s": units / (ms * 1e-3),
+                          "J_star_first": float(r["J_star"][0])}))
+        return 0
+    params = torch.as_tensor(wlm.draw_params(wl, T * per, seed=1), device=dev)
+    z0v0 = (torch.as_tensor(wlm.draw_initial_states(wl, T * per, seed=2), device=dev)
+            if args.one_batch == 1 else None)
+    out = torch.empty(T * per, dtype=torch.float64, device=dev)
+    ms = _event_ms(torch, lambda: afm.afm_forward_batch(params, trace, cfg, z0v0=z0v0,
+                                                        misfit=out), args.steps)
+    print(json.dumps({"one_batch": args.one_batch, "mode": "forward",
+                      "dtype": args.precision, "ms": ms,
+                      "particle_steps_per_s": float(T) * per * wl["n_steps"] / (ms * 1e-3)}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -424,7 +465,13 @@ def main():
                     help="oracle sample size of the cpu_baseline leg")
     ap.add_argument("--ref-particles", type=int, default=512,
                     help="oracle sample size per step of --impl reference")
+    ap.add_argument("--one-batch", type=int, default=None, choices=[0, 1, 2, 3, 4],
+                    help="profiling aid: one full-size forward batch of configs[N]")
+    ap.add_argument("--invert", action="store_true",
+                    help="with --one-batch: time the full PSO inversion instead")
     args = ap.parse_args()
+    if args.one_batch is not None:
+        return run_one_batch(args)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     return run_reference(args) if args.impl == "reference" else run_ours(args)

@@ -251,6 +251,15 @@ int afm_trajectory(const double* theta, const afm_cfg* cfg, double z0,
 int afm_fma_peak(int32_t precision, double seconds, double* tflops,
                  void* cuda_stream);
 
+/* Dispatch probe ("what bounds the FP64 kernel"): time per
+ * DFMA warp-instruction per SM sub-partition, in ns, for
+ *   mode 0: x = fma(x, a, b) with a, b reused;  1: three distinct 64-bit register
+ *   operands;  2, 3: mode 1 plus 2 / 4 independent integer instructions per
+ *   DFMA;  4: mode 1 with 16 of 32 lanes active,
+ * at 1..8 resident warps per sub-partition.  Synchronous.  Not on the hot path. */
+int afm_dispatch_probe(int32_t mode, int32_t warps_per_subpartition,
+                       double* ns_per_dfma, void* cuda_stream);
+
 /* Kernel launches enqueued by this library on the calling thread since the
  * last reset (bench.py's gpu_launches). */
 int64_t afm_launch_count(void);

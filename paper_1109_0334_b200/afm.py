@@ -25,7 +25,8 @@ SYMBOLS = (
     "afm_forward_batch", "afm_forward_batch_host", "afm_pso_invert",
     "afm_pso_invert_host", "afm_pso_step", "afm_pso_init",
     "afm_pso_shard_init", "afm_pso_shard_eval", "afm_pso_shard_move",
-    "afm_philox4x32_10", "afm_trajectory", "afm_fma_peak", "afm_launch_count",
+    "afm_philox4x32_10", "afm_trajectory", "afm_fma_peak", "afm_dispatch_probe",
+    "afm_launch_count",
     "afm_reset_launch_count", "afm_set_option", "afm_last_error",
     "afm_version", "afm_shutdown",
 )
@@ -103,6 +104,8 @@ def lib():
         L.afm_trajectory.argtypes = [dp, C.POINTER(Cfg), C.c_double, C.c_double,
                                      dp, dp, vp]
         L.afm_fma_peak.argtypes = [i32, C.c_double, C.POINTER(C.c_double), vp]
+        L.afm_dispatch_probe.argtypes = [i32, i32, C.POINTER(C.c_double), vp]
+        L.afm_dispatch_probe.restype = C.c_int
         for name in ("afm_forward_batch", "afm_forward_batch_host", "afm_pso_invert",
                      "afm_pso_invert_host", "afm_pso_step", "afm_pso_init",
                      "afm_philox4x32_10", "afm_trajectory", "afm_fma_peak",
@@ -389,6 +392,14 @@ def afm_fma_peak(precision, seconds=0.2, stream=None):
     out = C.c_double(0.0)
     _check(lib().afm_fma_peak(int(precision), float(seconds), C.byref(out),
                               _stream_ptr(stream)))
+    return out.value
+
+
+def afm_dispatch_probe(mode, warps_per_subpartition, stream=None):
+    """ns per DFMA warp-instruction per SM sub-partition (include/afm.h)."""
+    out = C.c_double(0.0)
+    _check(lib().afm_dispatch_probe(int(mode), int(warps_per_subpartition),
+                                    C.byref(out), _stream_ptr(stream)))
     return out.value
 
 

@@ -798,6 +798,31 @@ int afm_fma_peak(int32_t precision, double seconds, double* tflops,
   return release_ws(st);
 }
 
+int afm_dispatch_probe(int32_t mode, int32_t warps_per_subpartition,
+                       double* ns_per_dfma, void* cuda_stream) {
+  if (!ns_per_dfma) return fail(AFM_EINVAL, "ns_per_dfma is NULL");
+  if (mode < 0 || mode > 4) return fail(AFM_EINVAL, "mode must be 0..4");
+  if (warps_per_subpartition < 1 || warps_per_subpartition > 8)
+    return fail(AFM_EINVAL, "warps_per_subpartition must be 1..8");
+  int rc = check_device();
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  if ((rc = acquire_ws(st))) return rc;
+  if (g_ws.scratch.ensure(1024)) return fail(AFM_ECUDA, "cudaMalloc failed");
+  double h[64];
+  for (int i = 0; i < 64; ++i) h[i] = 0.999 + 1e-6 * i;
+  CUDA_TRY(cudaMemcpyAsync(g_ws.scratch.p, h, sizeof(h), cudaMemcpyHostToDevice, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  double* base = (double*)g_ws.scratch.p;
+  const int n = launch_dispatch_probe(mode, warps_per_subpartition, g_n_sm, base,
+                                      base + 64, ns_per_dfma, st);
+  if (n < 0) return fail(AFM_ECUDA, "cudaEventCreate failed");
+  g_launches += n;
+  CUDA_TRY(cudaGetLastError());
+  return release_ws(st);
+}
+
 int64_t afm_launch_count(void) { return g_launches; }
 void afm_reset_launch_count(void) { g_launches = 0; }
 

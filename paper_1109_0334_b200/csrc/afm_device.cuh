@@ -9,6 +9,7 @@
 #pragma once
 
 #include <cuda_runtime.h>
+#include <math_constants.h>
 #include <stdint.h>
 
 #include "afm.h"
@@ -60,6 +61,42 @@ __device__ __forceinline__ double sqrt_fast(double x) {
   double e = fma(-g0, y0, 1.0);
   double p = fma(0.375, e, 0.5) * e;
   return fma(g0, p, g0);
+}
+
+// exp(x) with a short dependent chain (the LJ+exp law is latency-bound: a swarm
+// of 8 192 particles is 256 warps on 592 sub-partitions).  x = n ln2 + f with
+// n = rint(x log2 e), |f| <= 0.3466; exp(f) by its Taylor polynomial of degree
+// 13 (remainder f^14/14! <= 4.2e-18 relative) evaluated by Estrin's scheme: four
+// FMA levels instead of thirteen; 2^n goes into the exponent field.  Below
+// x log2 e = -1000 the result is 0 (exp < 1e-301: the adhesion term vanishes
+// against any tolerance), above 1023 it is +Inf (a diverging trajectory, R12).
+__device__ __forceinline__ double exp_fast(double x) {
+  const double t = x * 1.4426950408889634;
+  const double magic = 6755399441055744.0;  // 1.5 * 2^52: rint by add/sub
+  const double nm = t + magic;
+  const double n = nm - magic;
+  double f = fma(n, -6.93147180369123816490e-01, x);  // ln2 high part
+  f = fma(n, -1.90821492927058770002e-10, f);         // ln2 low part
+  const double f2 = f * f;
+  const double a0 = fma(f, 1.0, 1.0);
+  const double a1 = fma(f, 1.0 / 6.0, 0.5);
+  const double a2 = fma(f, 1.0 / 120.0, 1.0 / 24.0);
+  const double a3 = fma(f, 1.0 / 5040.0, 1.0 / 720.0);
+  const double a4 = fma(f, 1.0 / 362880.0, 1.0 / 40320.0);
+  const double a5 = fma(f, 1.0 / 39916800.0, 1.0 / 3628800.0);
+  const double a6 = fma(f, 1.0 / 6227020800.0, 1.0 / 479001600.0);
+  const double f4 = f2 * f2;
+  const double b0 = fma(a1, f2, a0);
+  const double b1 = fma(a3, f2, a2);
+  const double b2 = fma(a5, f2, a4);
+  const double f8 = f4 * f4;
+  const double g0 = fma(b1, f4, b0);
+  const double g1 = fma(a6, f4, b2);
+  const double pv = fma(g1, f8, g0);
+  // 2^n into the exponent: n is the low word of nm (two's complement)
+  const int ni = __double2loint(nm);
+  const double r = __hiloint2double(__double2hiint(pv) + (ni << 20), __double2loint(pv));
+  return (t > 1023.0) ? CUDART_INF : ((t < -1000.0) ? 0.0 : r);
 }
 
 // ---- per-particle constants in registers ------------------------------------
@@ -131,7 +168,7 @@ __device__ __forceinline__ double accel_smooth(const Particle64& P, double s,
     const double r2 = r * r;
     const double r4 = r2 * r2;
     double f = fma(P.c0, r4, fma(P.c1, r, b0));
-    f = fma(P.c2, exp(d * P.c3), f);
+    f = fma(P.c2, exp_fast(d * P.c3), f);
     return fma(P.nalpha, w, f);
   }
   return fma(P.nalpha, w, b0);  // AFM_LAW_NONE

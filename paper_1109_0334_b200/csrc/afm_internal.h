@@ -137,6 +137,9 @@ int launch_pso_shard_gbest(const BoxDev& box, int D, int n_traces, int n_ranks,
                            cudaStream_t st);
 int launch_fma_peak(int precision, int iters, int blocks, int threads,
                     void* sink, float* ms, cudaStream_t st);
+int launch_dispatch_probe(int mode, int warps_per_subpartition, int n_sm,
+                          const double* in, double* sink, double* ns_per_dfma,
+                          cudaStream_t st);
 int launch_philox(const uint32_t* ctr, int64_t n, uint32_t k0, uint32_t k1,
                   uint32_t* out, cudaStream_t st);
 
