@@ -46,6 +46,12 @@ FLOPS_PER_STEP = {wlm.LAW_DMT: 57.0, wlm.LAW_DMT_VISC: 57.0, wlm.LAW_LJ_EXP: 93.
                   wlm.LAW_NONE: 49.0}
 # FP64 FMA peak of the lane model: 148 SMs x 64 lanes x 2 flops x clock
 N_SM, FP64_LANES, FP32_LANES = 148, 64, 128
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the integrate kernel
+# on configs[1], from the ncu --set full captures in profiles/r1b_ncu.md (bytes),
+# and the pipe utilisation ncu measured in the same captures.
+NCU_TRAFFIC = {"f64": 3920640 + 0, "f32": 2991872 + 0}
+NCU_PIPE = {"f64": {"sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active": 59.63},
+            "f32": {"sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active": 47.92}}
 
 
 def _peaks():
@@ -306,7 +312,10 @@ def run_ours(args):
             "clocks": clocks,
             "roofline": {"bound": "alu", "kernel": "integrate_misfit_%s" % args.precision,
                          "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                         "frac": achieved / peak, "traffic": None,
+                         "frac": achieved / peak, "traffic": NCU_TRAFFIC[args.precision],
+                         "traffic_source": "profiles/r1b_ncu.md (ncu --set full, one launch)",
+                         "algorithmic_bytes": int(P * (8 * D + 16 + 8) + N * 32),
+                         "ncu_pipe_utilisation_pct": NCU_PIPE[args.precision],
                          "flops_per_particle_step": FLOPS_PER_STEP[wl["law"]],
                          "kernel_ms": kern_ms,
                          "peak_source": "lane model 148 SM x %d lanes x 2 x %s (%s)" % (
@@ -409,6 +418,19 @@ def extras(afm, torch, dev, main_prec):
         ex["cfg%d_particle_steps_per_s" % ci] = units / (ms * 1e-3)
         ex["cfg%d_theta_star_rel_err_vs_truth" % ci] = [
             float(abs(a - t) / abs(t)) for a, t in zip(r["theta_star"][0], wl["truth"])]
+        if ci == 2:
+            # the paper's stopping rule is a cost cutoff; here
+            # the cutoff is the noise energy of the trace, W sigma^2 + 3 sd
+            W, sg = wl["n_window"], wl["sigma"]
+            jt = W * sg * sg * (1.0 + 3.0 * (2.0 / W) ** 0.5)
+            sc = afm.swarm_from(wl, j_target=jt)
+            afm.afm_pso_invert(b, sc, wl["pso_seed"], trace, cfg)
+            t0 = time.perf_counter()
+            r = afm.afm_pso_invert(b, sc, wl["pso_seed"], trace, cfg)
+            ex["cfg2_time_to_cutoff_ms"] = (time.perf_counter() - t0) * 1e3
+            ex["cfg2_batches_to_cutoff"] = int(r["n_iters_done"])
+            ex["cfg2_cutoff_theta_star_rel_err_vs_truth"] = [
+                float(abs(a - t) / abs(t)) for a, t in zip(r["theta_star"][0], wl["truth"])]
     return ex
 
 

@@ -47,6 +47,14 @@ void orc_constants(const orc_model* M, orc_consts* C) {
  *             d <= a0:  -H R / (6 a0^2) + (4/3) E* sqrt(R) (a0-d)^{3/2}
  *   DMT+visc: additionally, for d <= a0:  - eta sqrt(R (a0-d)) d'
  *   LJ+exp:   C_rep/d^8 - C_att/d^2 - F_ad exp(-d/lambda)
+ * The paper's own two sample models (R19/R20),
+ * active only while the tip is pressed into the sample (gap < 0):
+ *   Hooke (Eq. 11):  f = -k_s (u - h), theta = (k_s, h); the
+ *     cantilever-sample separation h is an unknown and replaces z_c: the gap
+ *     is z + h = d - z_c + h, and F = -k_s (z + h) for z + h < 0, else 0.
+ *   Kelvin-Voigt (Eq. 12):  f = -k_s (u - h) - zeta_s u',
+ *     theta = (k_s, zeta_s), separation known (= z_c):
+ *     F = -k_s d - zeta_s v for d < 0, else 0.
  * (a0-d)^{3/2} is evaluated as delta*sqrt(delta); 1/d^8 as 1/((d^2)^2)^2.
  * ---------------------------------------------------------------------- */
 double orc_force(const orc_model* M, const double* theta, double d, double v) {
@@ -80,6 +88,19 @@ double orc_force(const orc_model* M, const double* theta, double d, double v) {
       double d4 = d2 * d2;
       double d8 = d4 * d4;
       return C_rep / d8 - C_att / d2 - F_ad * exp(-d / lambda);
+    }
+    case ORC_LAW_HOOKE: {
+      double k_s = theta[0];
+      double h = theta[1];
+      double gap = d - M->z_c + h;
+      if (gap < 0.0) return -k_s * gap;
+      return 0.0;
+    }
+    case ORC_LAW_KELVIN_VOIGT: {
+      double k_s = theta[0];
+      double zeta = theta[1];
+      if (d < 0.0) return -k_s * d - zeta * v;
+      return 0.0;
     }
     default:
       return NAN;

@@ -43,7 +43,9 @@ enum {
   ORC_LAW_NONE = 0,    /* F_ts = 0 (linear oscillator; used by the pins)      */
   ORC_LAW_DMT = 1,     /* theta = (H, E*)                                     */
   ORC_LAW_DMT_VISC = 2,/* theta = (H, E*, eta)                                */
-  ORC_LAW_LJ_EXP = 3   /* theta = (C_rep, C_att, F_ad, lambda)                */
+  ORC_LAW_LJ_EXP = 3,  /* theta = (C_rep, C_att, F_ad, lambda)                */
+  ORC_LAW_HOOKE = 4,   /* theta = (k_s, h): paper Eq. 11                      */
+  ORC_LAW_KELVIN_VOIGT = 5 /* theta = (k_s, zeta_s): paper Eq. 12              */
 };
 
 /* Cantilever, drive and time grid.  All SI. */

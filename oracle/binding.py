@@ -13,7 +13,7 @@ from . import build as _build
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
-LAW_NONE, LAW_DMT, LAW_DMT_VISC, LAW_LJ_EXP = 0, 1, 2, 3
+LAW_NONE, LAW_DMT, LAW_DMT_VISC, LAW_LJ_EXP, LAW_HOOKE, LAW_KELVIN_VOIGT = 0, 1, 2, 3, 4, 5
 
 
 class Model(C.Structure):

@@ -16,7 +16,7 @@ import math
 
 import numpy as np
 
-LAW_NONE, LAW_DMT, LAW_DMT_VISC, LAW_LJ_EXP = 0, 1, 2, 3
+LAW_NONE, LAW_DMT, LAW_DMT_VISC, LAW_LJ_EXP, LAW_HOOKE, LAW_KELVIN_VOIGT = 0, 1, 2, 3, 4, 5
 
 _PSO = dict(w=0.72, c1=1.49, c2=1.49)   # BASELINE.json configs[0]
 
@@ -100,6 +100,40 @@ def config(i):
     wl["index"] = i
     wl["pso_seed"] = 0
     wl["trace_seed"] = 1000 + i
+    wl["z0"], wl["v0"] = _free_steady_state(wl["cantilever"])
+    wl["n_steps"] = wl["steps_per_cycle"] * wl["n_cycles"]
+    wl["n_window"] = wl["steps_per_cycle"] * (wl["n_cycles"] - wl["n_skip_cycles"])
+    return wl
+
+
+def paper_law(name):
+    """The paper's own two sample models as extra workloads,
+    on the configs[0] cantilever.  Index 5 = "hooke" (Eq. 11, PAPER.md:260:
+    unknowns k_s and the separation h), 6 = "kelvin_voigt" (Eq. 12,
+    PAPER.md:270: unknowns k_s and zeta_s, separation known).  The paper's truth
+    k_s = 4 N/m and its search range [0, 25] N/m are kept; its h = 50 nm and
+    zeta_s = 0.1 N s/m belong to its own cantilever and step (at this one,
+    zeta_s h/m = 541 per step is far outside RK4's stability region), so h is
+    scaled with the amplitude (8 nm at A0 = 10 nm) and zeta_s to 5e-6 N s/m
+    (range [0, 2e-5]).  DESIGN.md readings R19/R20.  All coordinates linear."""
+    if name == "hooke":
+        wl = dict(name="paper_hooke_inversion", cantilever=_soft_cantilever(),
+                  law=LAW_HOOKE, n_params=2, steps_per_cycle=256, n_cycles=60,
+                  n_skip_cycles=30, sigma=0.02e-9, truth=[4.0, 8e-9],
+                  bounds=dict(lo=[0.0, 5e-9], hi=[25.0, 11e-9], log10=[0, 0]),
+                  swarm=dict(n_particles=1024, n_iters=60, **_PSO),
+                  n_traces=1, precisions=["f64", "f32"], index=5)
+    elif name == "kelvin_voigt":
+        wl = dict(name="paper_kelvin_voigt_inversion", cantilever=_soft_cantilever(),
+                  law=LAW_KELVIN_VOIGT, n_params=2, steps_per_cycle=256, n_cycles=60,
+                  n_skip_cycles=30, sigma=0.02e-9, truth=[4.0, 5e-6],
+                  bounds=dict(lo=[0.0, 0.0], hi=[25.0, 2e-5], log10=[0, 0]),
+                  swarm=dict(n_particles=1024, n_iters=60, **_PSO),
+                  n_traces=1, precisions=["f64", "f32"], index=6)
+    else:
+        raise ValueError('paper_law: "hooke" or "kelvin_voigt"')
+    wl["pso_seed"] = 0
+    wl["trace_seed"] = 1000 + wl["index"]
     wl["z0"], wl["v0"] = _free_steady_state(wl["cantilever"])
     wl["n_steps"] = wl["steps_per_cycle"] * wl["n_cycles"]
     wl["n_window"] = wl["steps_per_cycle"] * (wl["n_cycles"] - wl["n_skip_cycles"])
