@@ -59,12 +59,20 @@ typedef enum {
  *       DMT, plus  -eta sqrt(R (a0 - d)) d'  for d <= a0
  *   AFM_LAW_LJ_EXP    theta = (C_rep, C_att, F_ad, lambda)       D = 4
  *       C_rep / d^8 - C_att / d^2 - F_ad exp(-d / lambda)
+ * The paper's own sample models, active while the tip is pressed in:
+ *   AFM_LAW_HOOKE     theta = (k_s, h)   Eq. 11, PAPER.md:260    D = 2
+ *       gap = z + h (h, the cantilever-sample separation, is an unknown and
+ *       takes the place of z_c):  -k_s gap  for gap < 0, else 0
+ *   AFM_LAW_KELVIN_VOIGT  theta = (k_s, zeta_s)  Eq. 12, PAPER.md:270   D = 2
+ *       separation known (z_c):  -k_s d - zeta_s d'  for d < 0, else 0
  */
 typedef enum {
   AFM_LAW_NONE = 0,
   AFM_LAW_DMT = 1,
   AFM_LAW_DMT_VISC = 2,
-  AFM_LAW_LJ_EXP = 3
+  AFM_LAW_LJ_EXP = 3,
+  AFM_LAW_HOOKE = 4,
+  AFM_LAW_KELVIN_VOIGT = 5
 } afm_law;
 
 typedef enum { AFM_F64 = 0, AFM_F32 = 1 } afm_precision;

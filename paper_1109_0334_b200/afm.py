@@ -16,7 +16,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libafm_b200.so")
 
-LAW_NONE, LAW_DMT, LAW_DMT_VISC, LAW_LJ_EXP = 0, 1, 2, 3
+LAW_NONE, LAW_DMT, LAW_DMT_VISC, LAW_LJ_EXP, LAW_HOOKE, LAW_KELVIN_VOIGT = 0, 1, 2, 3, 4, 5
 F64, F32 = 0, 1
 OK, EINVAL, ECUDA, EUNSUPPORTED = 0, -1, -2, -3
 

@@ -143,13 +143,15 @@ int law_dims(int law) {
     case AFM_LAW_DMT: return 2;
     case AFM_LAW_DMT_VISC: return 3;
     case AFM_LAW_LJ_EXP: return 4;
+    case AFM_LAW_HOOKE: return 2;
+    case AFM_LAW_KELVIN_VOIGT: return 2;
     default: return -1;
   }
 }
 
 int validate_cfg(const afm_cfg* c) {
   if (!c) return fail(AFM_EINVAL, "cfg is NULL");
-  if (c->law < AFM_LAW_NONE || c->law > AFM_LAW_LJ_EXP)
+  if (c->law < AFM_LAW_NONE || c->law > AFM_LAW_KELVIN_VOIGT)
     return fail(AFM_EINVAL, "unknown law %d", c->law);
   if (c->law == AFM_LAW_NONE) {
     if (c->n_params < 0 || c->n_params > 4)
@@ -201,6 +203,7 @@ void make_consts(const afm_cfg* c, int block, ModelConsts* mc) {
   mc->c_hertz = h * h * (4.0 / 3.0) * sqrt(c->R > 0 ? c->R : 0.0) / m;
   mc->c_visc = h * sqrt(c->R > 0 ? c->R : 0.0) / m;
   mc->c_force = h * h / m;
+  mc->c_damp = h / m;
   mc->d_max = c->z_c + 100.0 * c->A0;
   mc->d_min = c->z_c - 100.0 * c->A0;
   mc->d_safe = fmax(0.0, 100.0 * c->A0 - fabs(c->z_c));
@@ -244,6 +247,8 @@ void make_consts_f32(const afm_cfg* c, ModelConstsF32* mf) {
   mf->c_att = mf->b6 / (c->k * len * len * len);
   mf->c_fad = mf->b6 / (c->k * len);
   mf->c_lam = 1.4426950408889634 * len;
+  mf->c_ks = mf->b6 / c->k;
+  mf->c_zeta = mf->b6 / (h * c->k);
   mf->d_max = (c->z_c + 100.0 * c->A0) / len;
   mf->d_min = (c->z_c - 100.0 * c->A0) / len;
   mf->d_safe = fmax(0.0, 100.0 * c->A0 - fabs(c->z_c)) / len;

@@ -171,6 +171,15 @@ __device__ __forceinline__ double accel_smooth(const Particle64& P, double s,
     f = fma(P.c2, exp_fast(d * P.c3), f);
     return fma(P.nalpha, w, f);
   }
+  if (LAW == AFM_LAW_HOOKE || LAW == AFM_LAW_KELVIN_VOIGT) {
+    // the paper's sample models (Eq. 11, 12): a spring (and a damper) that act
+    // while the tip is pressed in, d < P.a0 (= z_c - h for Hooke, 0 for
+    // Kelvin-Voigt).  Coefficients selected per lane, then two FMAs.
+    const bool in = d < P.a0;
+    const double ks = in ? P.c1 : 0.0;
+    const double cw = (LAW == AFM_LAW_KELVIN_VOIGT && in) ? P.c3 : P.nalpha;
+    return fma(cw, w, fma(ks, P.a0 - d, b0));
+  }
   return fma(P.nalpha, w, b0);  // AFM_LAW_NONE
 }
 
@@ -323,7 +332,8 @@ __device__ __forceinline__ void load_particle(Particle64& P, int law,
                                               double beta, double a0,
                                               double inv_a0sq, double c_vdw,
                                               double c_hertz, double c_visc,
-                                              double c_force) {
+                                              double c_force, double zc,
+                                              double c_damp) {
   P.nalpha = -alpha;
   P.nbeta = -beta;
   P.a0 = a0;
@@ -339,6 +349,13 @@ __device__ __forceinline__ void load_particle(Particle64& P, int law,
     P.c1 = -(th[1] * c_force);
     P.c2 = -(th[2] * c_force);
     P.c3 = -1.0 / th[3];
+  } else if (law == AFM_LAW_HOOKE) {
+    P.c1 = th[0] * c_force;          // (h^2/m) k_s
+    P.a0 = zc - th[1];               // pressed in while z + h < 0, i.e. d < z_c - h
+  } else if (law == AFM_LAW_KELVIN_VOIGT) {
+    P.c1 = th[0] * c_force;
+    P.a0 = 0.0;
+    P.c3 = -alpha - th[1] * c_damp;  // -(alpha + (h/m) zeta_s)
   }
 }
 

@@ -69,8 +69,11 @@ struct Model32 {
 // Per-particle law coefficients (scaled by beta/6 and the unit factors):
 //   DMT:    c0 = -kappa, c1 = eps, c2 = -kappa/a0^2, c3 = -nu
 //   LJ_EXP: c0 = crep,   c1 = -catt, c2 = -fad,      c3 = -log2(e)/lambda
+//   HOOKE / KELVIN_VOIGT: c1 = spring, c3 = -(alpha/6 + damper), thr = contact
+//           threshold on d (z_c - h, or 0)
 struct Particle32 {
   float c0, c1, c2, c3;
+  float thr;
 };
 
 __device__ __forceinline__ float accel_free32(const Model32& M,
@@ -106,6 +109,12 @@ __device__ __forceinline__ float accel_smooth32(const Model32& M,
     float f = fmaf(P.c0, r4, fmaf(P.c1, r, b0));
     f = fmaf(P.c2, ex2_32(d * P.c3), f);
     return fmaf(M.nalpha, w, f);
+  }
+  if (LAW == AFM_LAW_HOOKE || LAW == AFM_LAW_KELVIN_VOIGT) {
+    const bool in = d < P.thr;
+    const float ks = in ? P.c1 : 0.0f;
+    const float cw = (LAW == AFM_LAW_KELVIN_VOIGT && in) ? P.c3 : M.nalpha;
+    return fmaf(cw, w, fmaf(ks, P.thr - d, b0));
   }
   return fmaf(M.nalpha, w, b0);  // AFM_LAW_NONE
 }

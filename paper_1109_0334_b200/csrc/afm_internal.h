@@ -29,6 +29,7 @@ struct ModelConsts {
   double c_hertz;    // h^2 (4/3) sqrt(R)/m:  eps   = E* c_hertz
   double c_visc;     // h sqrt(R) / m:        nu    = eta c_visc
   double c_force;    // h^2 / m
+  double c_damp;     // h / m:  (h/m) zeta_s adds to alpha (Kelvin-Voigt)
   double d_max;      // z_c + 100 A0   (divergence rule R12 on d)
   double d_min;      // z_c - 100 A0   (negative)
   double d_safe;     // max(0, 100 A0 - |z_c|): |d| < d_safe => not diverged
@@ -58,6 +59,8 @@ struct ModelConstsF32 {
   double c_visc;     // c3 = -theta2 c_visc
   double c_rep, c_att, c_fad;  // LJ+exp: c0 = theta0 c_rep, c1 = -theta1 c_att, c2 = -theta2 c_fad
   double c_lam;      // c3 = -c_lam / theta3  (log2(e) len)
+  double c_ks;       // Hooke / Kelvin-Voigt: c1 = theta0 c_ks   (b6 / k)
+  double c_zeta;     // Kelvin-Voigt: c3 = -(a6 + theta1 c_zeta)  (b6 / (h k))
   double d_max, d_min, d_safe;  // nm
   double z0, v0;     // default initial state, SI
   int32_t law, D, N, n0, W, T, n_tiles, pad_;

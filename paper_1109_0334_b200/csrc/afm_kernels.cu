@@ -206,7 +206,7 @@ __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
       }
     }
     load_particle(P[q], LAW, th, mc.alpha, mc.beta, mc.a0, mc.inv_a0sq,
-                  mc.c_vdw, mc.c_hertz, mc.c_visc, mc.c_force);
+                  mc.c_vdw, mc.c_hertz, mc.c_visc, mc.c_force, mc.zc, mc.c_damp);
     double z0 = mc.z0, v0 = mc.v0;
     if (io.z0v0 != nullptr) {
       z0 = io.z0v0[2 * gp[q]];
@@ -293,7 +293,7 @@ __global__ void trajectory_kernel(ModelConsts mc, const double* __restrict__ th,
   for (int j = 0; j < mc.D && j < 4; ++j) t4[j] = th[j];
   Particle64 P[1];
   load_particle(P[0], LAW, t4, mc.alpha, mc.beta, mc.a0, mc.inv_a0sq, mc.c_vdw,
-                mc.c_hertz, mc.c_visc, mc.c_force);
+                mc.c_hertz, mc.c_visc, mc.c_force, mc.zc, mc.c_damp);
   double d[1] = {z0 + mc.zc}, w[1] = {v0 * mc.h};
   const long long a0_bits = __double_as_longlong(mc.a0);
   const double inv_h = 1.0 / mc.h;
@@ -601,6 +601,8 @@ int launch_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block
     AFM_DISPATCH(AFM_LAW_DMT)
     AFM_DISPATCH(AFM_LAW_DMT_VISC)
     AFM_DISPATCH(AFM_LAW_LJ_EXP)
+    AFM_DISPATCH(AFM_LAW_HOOKE)
+    AFM_DISPATCH(AFM_LAW_KELVIN_VOIGT)
     default:
       return -1;
   }
@@ -625,6 +627,14 @@ int launch_trajectory(const ModelConsts& mc, const double* theta_dev,
       break;
     case AFM_LAW_LJ_EXP:
       trajectory_kernel<AFM_LAW_LJ_EXP>
+          <<<1, 32, 0, st>>>(mc, theta_dev, stream, z0, v0, zs, vs);
+      break;
+    case AFM_LAW_HOOKE:
+      trajectory_kernel<AFM_LAW_HOOKE>
+          <<<1, 32, 0, st>>>(mc, theta_dev, stream, z0, v0, zs, vs);
+      break;
+    case AFM_LAW_KELVIN_VOIGT:
+      trajectory_kernel<AFM_LAW_KELVIN_VOIGT>
           <<<1, 32, 0, st>>>(mc, theta_dev, stream, z0, v0, zs, vs);
       break;
     default:

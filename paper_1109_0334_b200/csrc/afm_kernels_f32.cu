@@ -150,7 +150,7 @@ __global__ void integrate_misfit_f32(ModelConstsF32 mf, IntegrateIO io,
         th[j] = (MODE == 1 && io.box.lg[j]) ? pow(10.0, xv) : xv;
       }
     }
-    P[q].c0 = P[q].c1 = P[q].c2 = P[q].c3 = 0.0f;
+    P[q].c0 = P[q].c1 = P[q].c2 = P[q].c3 = P[q].thr = 0.0f;
     if (LAW == AFM_LAW_DMT || LAW == AFM_LAW_DMT_VISC) {
       const double kappa = th[0] * mf.c_vdw;
       P[q].c0 = (float)(-kappa);
@@ -162,6 +162,12 @@ __global__ void integrate_misfit_f32(ModelConstsF32 mf, IntegrateIO io,
       P[q].c1 = (float)(-(th[1] * mf.c_att));
       P[q].c2 = (float)(-(th[2] * mf.c_fad));
       P[q].c3 = (float)(-mf.c_lam / th[3]);
+    } else if (LAW == AFM_LAW_HOOKE) {
+      P[q].c1 = (float)(th[0] * mf.c_ks);
+      P[q].thr = (float)(mf.zc - th[1] / mf.len);
+    } else if (LAW == AFM_LAW_KELVIN_VOIGT) {
+      P[q].c1 = (float)(th[0] * mf.c_ks);
+      P[q].c3 = (float)(-mf.a6 - th[1] * mf.c_zeta);
     }
     double z0 = mf.z0, v0 = mf.v0;
     if (io.z0v0 != nullptr) {
@@ -280,6 +286,8 @@ int launch_integrate_f32(const ModelConstsF32& mf, const IntegrateIO& io,
     AFM_DISPATCH32(AFM_LAW_DMT)
     AFM_DISPATCH32(AFM_LAW_DMT_VISC)
     AFM_DISPATCH32(AFM_LAW_LJ_EXP)
+    AFM_DISPATCH32(AFM_LAW_HOOKE)
+    AFM_DISPATCH32(AFM_LAW_KELVIN_VOIGT)
     default:
       return -1;
   }
