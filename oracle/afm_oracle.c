@@ -321,12 +321,10 @@ void orc_theta_of_x(const orc_box* B, int32_t D, const double* x,
  *   n_iters forward batches; the result is the global best after the last.
  * Each trace (pixel) owns an independent swarm of n_particles.
  * ---------------------------------------------------------------------- */
-void orc_pso_invert(const orc_model* M, const orc_box* B, const orc_swarm* Sw,
-                    uint64_t seed, const double* trace, int32_t n_traces,
-                    double z0, double v0, double* theta_star, double* J_star,
-                    double* dump, double* gbest_hist) {
-  orc_consts C;
-  const int32_t D = M->n_theta;
+void orc_pso_core(orc_eval_fn eval, const void* ctx, int64_t W, int32_t D,
+                  const orc_box* B, const orc_swarm* Sw, uint64_t seed,
+                  const double* trace, int32_t n_traces, double* theta_star,
+                  double* J_star, double* dump, double* gbest_hist) {
   const int64_t P = Sw->n_particles;
   const int64_t PT = P * (int64_t)n_traces;
   const int64_t rec = 3 * D + 2;
@@ -339,7 +337,6 @@ void orc_pso_invert(const orc_model* M, const orc_box* B, const orc_swarm* Sw,
   double* gbestJ = (double*)malloc((size_t)n_traces * sizeof(double));
   int64_t gp;
   int32_t it, j, s;
-  orc_constants(M, &C);
 
   /* initialisation: uniform positions and velocities in the search space */
   for (gp = 0; gp < PT; ++gp) {
@@ -367,7 +364,7 @@ void orc_pso_invert(const orc_model* M, const orc_box* B, const orc_swarm* Sw,
     for (gp = 0; gp < PT; ++gp) {
       double theta[4];
       orc_theta_of_x(B, D, x + gp * D, theta);
-      J[gp] = orc_misfit(M, theta, z0, v0, trace + (gp / P) * C.W);
+      J[gp] = eval(ctx, theta, trace + (gp / P) * W);
     }
     /* personal best (strict <; NaN and +Inf never win) */
     for (gp = 0; gp < PT; ++gp) {
@@ -443,4 +440,29 @@ void orc_pso_invert(const orc_model* M, const orc_box* B, const orc_swarm* Sw,
   free(J);
   free(gbest);
   free(gbestJ);
+}
+
+/* The point-mass forward solve as the PSO's cost function. */
+typedef struct {
+  const orc_model* M;
+  double z0, v0;
+} pm_ctx;
+
+static double pm_eval(const void* ctx, const double* theta, const double* U) {
+  const pm_ctx* c = (const pm_ctx*)ctx;
+  return orc_misfit(c->M, theta, c->z0, c->v0, U);
+}
+
+void orc_pso_invert(const orc_model* M, const orc_box* B, const orc_swarm* Sw,
+                    uint64_t seed, const double* trace, int32_t n_traces,
+                    double z0, double v0, double* theta_star, double* J_star,
+                    double* dump, double* gbest_hist) {
+  orc_consts C;
+  pm_ctx ctx;
+  orc_constants(M, &C);
+  ctx.M = M;
+  ctx.z0 = z0;
+  ctx.v0 = v0;
+  orc_pso_core(pm_eval, &ctx, C.W, M->n_theta, B, Sw, seed, trace, n_traces,
+               theta_star, J_star, dump, gbest_hist);
 }

@@ -149,6 +149,15 @@ void   orc_pso_invert(const orc_model* M, const orc_box* B,
                       double* theta_star, double* J_star, double* dump,
                       double* gbest_hist);
 
+/* The PSO loop itself, around any cost function eval(ctx, theta, U_s) (the
+ * point-mass misfit above, or the beam misfit of afm_oracle_beam.h). */
+typedef double (*orc_eval_fn)(const void* ctx, const double* theta,
+                              const double* trace_s);
+void   orc_pso_core(orc_eval_fn eval, const void* ctx, int64_t W, int32_t D,
+                    const orc_box* B, const orc_swarm* Sw, uint64_t seed,
+                    const double* trace, int32_t n_traces, double* theta_star,
+                    double* J_star, double* dump, double* gbest_hist);
+
 #ifdef __cplusplus
 }
 #endif

@@ -41,6 +41,22 @@ class Swarm(C.Structure):
                 ("w", C.c_double), ("c1", C.c_double), ("c2", C.c_double)]
 
 
+class Beam(C.Structure):
+    _fields_ = [("L", C.c_double), ("E", C.c_double), ("I", C.c_double),
+                ("mu", C.c_double), ("Q", C.c_double), ("f_drive", C.c_double),
+                ("A_base", C.c_double), ("A_ref", C.c_double), ("z_c", C.c_double),
+                ("R", C.c_double), ("a0", C.c_double), ("law", C.c_int32),
+                ("n_theta", C.c_int32), ("n_modes", C.c_int32),
+                ("n_points", C.c_int32), ("S", C.c_int32), ("n_cycles", C.c_int32),
+                ("n_skip", C.c_int32), ("literal_eq7", C.c_int32)]
+
+
+class BeamModes(C.Structure):
+    _fields_ = [(n, C.c_double * 8) for n in ("bL", "omega", "phiL", "norm", "intphi",
+                                              "gain", "fgain")] + \
+               [("w", C.c_double), ("dt", C.c_double), ("N", C.c_int64), ("W", C.c_int64)]
+
+
 _dp = C.POINTER(C.c_double)
 _libs = {}
 
@@ -96,6 +112,24 @@ def lib(openmp=False):
                                      C.c_int32, C.c_double, C.c_double, _dp,
                                      _dp, _dp, _dp]
         L.orc_pso_invert.restype = None
+        L.orc_beam_setup.argtypes = [C.POINTER(Beam), C.POINTER(BeamModes)]
+        L.orc_beam_setup.restype = None
+        L.orc_beam_shape.argtypes = [C.POINTER(Beam), C.POINTER(BeamModes), C.c_int32,
+                                     C.c_double]
+        L.orc_beam_shape.restype = C.c_double
+        L.orc_beam_integrate.argtypes = [C.POINTER(Beam), _dp, _dp, _dp, _dp, _dp]
+        L.orc_beam_integrate.restype = C.c_int
+        L.orc_beam_window.argtypes = [C.POINTER(Beam), _dp, _dp]
+        L.orc_beam_window.restype = C.c_int
+        L.orc_beam_misfit.argtypes = [C.POINTER(Beam), _dp, _dp]
+        L.orc_beam_misfit.restype = C.c_double
+        L.orc_beam_forward_batch.argtypes = [C.POINTER(Beam), _dp, C.c_int64, _dp,
+                                             C.c_int32, _dp]
+        L.orc_beam_forward_batch.restype = None
+        L.orc_beam_pso_invert.argtypes = [C.POINTER(Beam), C.POINTER(Box),
+                                          C.POINTER(Swarm), C.c_uint64, _dp, C.c_int32,
+                                          _dp, _dp, _dp, _dp]
+        L.orc_beam_pso_invert.restype = None
         _libs[key] = L
     return _libs[key]
 
@@ -232,4 +266,69 @@ def pso_invert(M, B, Sw, seed, trace, z0, v0, n_traces=1, dump=False,
     lib(openmp).orc_pso_invert(C.byref(M), C.byref(B), C.byref(Sw), seed,
                                _ptr(tr), n_traces, z0, v0, _ptr(th), _ptr(Js),
                                _ptr(dmp), _ptr(gh))
+    return dict(theta_star=th, J_star=Js, dump=dmp, gbest_hist=gh)
+
+
+# ---- the multi-mode Euler-Bernoulli beam (afm_oracle_beam.h) ------------------
+
+def beam_from(wl, **over):
+    b = wl["beam"]
+    kw = dict(L=b["L"], E=b["E"], I=b["I"], mu=b["mu"], Q=b["Q"], f_drive=b["f_drive"],
+              A_base=b["A_base"], A_ref=b["A_ref"], z_c=b["z_c"], R=b["R"], a0=b["a0"],
+              law=wl["law"], n_theta=wl["n_params"], n_modes=b["n_modes"],
+              n_points=b["n_points"], S=wl["steps_per_cycle"], n_cycles=wl["n_cycles"],
+              n_skip=wl["n_skip_cycles"], literal_eq7=0)
+    kw.update(over)
+    return Beam(**kw)
+
+
+def beam_setup(B):
+    mo = BeamModes()
+    lib().orc_beam_setup(C.byref(B), C.byref(mo))
+    return mo
+
+
+def beam_shape(B, mo, i, x):
+    return lib().orc_beam_shape(C.byref(B), C.byref(mo), int(i), float(x))
+
+
+def beam_integrate(B, theta, eta0=None, want_eta=False):
+    """(diverged, tip_u[N+1], tip_v[N+1], eta[N+1][2m] or None)."""
+    th = _f64(theta)
+    mo = beam_setup(B)
+    u, v = np.empty(mo.N + 1), np.empty(mo.N + 1)
+    eta = np.empty((mo.N + 1, 2 * B.n_modes)) if want_eta else None
+    e0 = None if eta0 is None else _f64(eta0)
+    bad = lib().orc_beam_integrate(C.byref(B), _ptr(th), _ptr(e0), _ptr(u), _ptr(v),
+                                   _ptr(eta))
+    return bad, u, v, eta
+
+
+def beam_window(B, theta):
+    th = _f64(theta)
+    w = np.empty(beam_setup(B).W)
+    bad = lib().orc_beam_window(C.byref(B), _ptr(th), _ptr(w))
+    return bad, w
+
+
+def beam_forward_batch(B, params, trace, n_traces=1, openmp=False):
+    params = _f64(params)
+    tr = _f64(trace)
+    assert tr.size == n_traces * beam_setup(B).W
+    out = np.empty(params.shape[0])
+    lib(openmp).orc_beam_forward_batch(C.byref(B), _ptr(params), params.shape[0],
+                                       _ptr(tr), n_traces, _ptr(out))
+    return out
+
+
+def beam_pso_invert(B, Bx, Sw, seed, trace, n_traces=1, dump=False, openmp=False):
+    D = B.n_theta
+    PT = Sw.n_particles * n_traces
+    tr = _f64(trace)
+    th = np.empty((n_traces, D))
+    Js = np.empty(n_traces)
+    dmp = np.empty((Sw.n_iters, PT, 3 * D + 2)) if dump else None
+    gh = np.empty((Sw.n_iters, n_traces, D + 1))
+    lib(openmp).orc_beam_pso_invert(C.byref(B), C.byref(Bx), C.byref(Sw), seed, _ptr(tr),
+                                    n_traces, _ptr(th), _ptr(Js), _ptr(dmp), _ptr(gh))
     return dict(theta_star=th, J_star=Js, dump=dmp, gbest_hist=gh)

@@ -11,7 +11,7 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = os.path.join(HERE, "afm_oracle.c")
+SRCS = [os.path.join(HERE, "afm_oracle.c"), os.path.join(HERE, "afm_oracle_beam.c")]
 FLAGS = ["-O2", "-std=c99", "-ffp-contract=off", "-fno-fast-math", "-fPIC",
          "-shared", "-Wall", "-Wextra"]
 
@@ -21,7 +21,8 @@ def _stale(out):
         return True
     t = os.path.getmtime(out)
     return any(os.path.getmtime(os.path.join(HERE, f)) > t
-               for f in ("afm_oracle.c", "afm_oracle.h", "build.py"))
+               for f in ("afm_oracle.c", "afm_oracle.h", "afm_oracle_beam.c",
+                         "afm_oracle_beam.h", "build.py"))
 
 
 def build(force=False, verbose=False):
@@ -30,7 +31,7 @@ def build(force=False, verbose=False):
                         ("libafm_oracle_omp.so", ["-fopenmp", "-DORC_OPENMP"])):
         out = os.path.join(HERE, name)
         if force or _stale(out):
-            cmd = ["gcc"] + FLAGS + extra + [SRC, "-o", out, "-lm"]
+            cmd = ["gcc"] + FLAGS + extra + SRCS + ["-o", out, "-lm"]
             if verbose:
                 print(" ".join(cmd))
             subprocess.check_call(cmd)

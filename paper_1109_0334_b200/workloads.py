@@ -140,6 +140,31 @@ def paper_law(name):
     return wl
 
 
+def beam_workload():
+    """The paper's own forward model as an extra workload: the
+    Appendix A cantilever (L = 525 um, E = 1.76e11 Pa, 35 x 5 um
+    section, mu = 4.0775e-7 kg/m, 8 modes, 501 modal-function points; first
+    natural frequency 25 468.9 Hz), base-excited at that frequency, tapping on a
+    DMT sample.  The paper gives no damping and no tapping set-point: Q = 50 and
+    a base amplitude that makes the free tip amplitude ~10 nm (A_base = A_ref /
+    (1.566 Q), 1.566 = first-mode participation factor) with the sample 8 nm
+    below the tip (R21).  S = 512 steps per cycle keeps RK4 stable on
+    mode 8 (h w_8 = 1.94); starts from rest, 80 cycles, misfit over the last 40."""
+    width, height = 35e-6, 5e-6
+    beam = dict(L=525e-6, E=1.76e11, I=width * height ** 3 / 12.0, mu=4.0775e-7,
+                Q=50.0, f_drive=25468.9, A_ref=10e-9, A_base=10e-9 / (1.566 * 50.0),
+                z_c=8e-9, R=10e-9, a0=0.3e-9, n_modes=8, n_points=501)
+    wl = dict(name="paper_beam_dmt_inversion", beam=beam, law=LAW_DMT, n_params=2,
+              steps_per_cycle=512, n_cycles=80, n_skip_cycles=40, sigma=0.02e-9,
+              truth=[1e-19, 1e9],
+              bounds=dict(lo=[-20.0, 8.0], hi=[-18.0, 10.0], log10=[1, 1]),
+              swarm=dict(n_particles=1024, n_iters=40, **_PSO),
+              n_traces=1, precisions=["f64"], index=7, pso_seed=0, trace_seed=1007)
+    wl["n_steps"] = wl["steps_per_cycle"] * wl["n_cycles"]
+    wl["n_window"] = wl["steps_per_cycle"] * (wl["n_cycles"] - wl["n_skip_cycles"])
+    return wl
+
+
 def _rng(seed):
     return np.random.Generator(np.random.Philox(key=int(seed)))
 
