@@ -240,6 +240,60 @@ int afm_pso_shard_move(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
                        const double* pbest, double* gbest, double* gbestJ,
                        double* theta_star, double* J_star, void* cuda_stream);
 
+/* ---- Multi-mode Euler-Bernoulli cantilever (the paper's own forward model) ----
+ * PAPER.md:59-66 (Eq. 1-2), 128-139 (Eq. 6-7, Newton + Simpson initialisation,
+ * RK4), Appendix A/B; R21/R22.
+ *   u(x,t) = sum_i Phi_i(x) eta_i(t),  i < n_modes <= 8
+ *   eta_i'' + (w_i/Q) eta_i' + w_i^2 eta_i =
+ *       [ F_ts(u(L)+z_c, u'(L); theta) Phi_i(L) + mu A_base w^2 cos(w t) <1,Phi_i> ]
+ *       / (mu <Phi_i,Phi_i>)
+ * from rest, classical RK4 with steps_per_cycle steps per drive period; the
+ * misfit is sum over the window of (u(L,t_n) - U_n)^2; +Inf if a state is
+ * non-finite or |u(L)| > 100 A_ref.  FP64 only.  Host struct, plain POD. */
+typedef struct {
+  double L, E, I, mu;      /* length m, Young's modulus Pa, area moment m^4, kg/m */
+  double Q;                /* modal quality factor (2 zeta = 1/Q)                */
+  double f_drive;          /* Hz                                                 */
+  double A_base;           /* base displacement amplitude y_ex = A_base cos(wt)  */
+  double A_ref;            /* reference tip amplitude of the divergence rule, m  */
+  double z_c, R, a0;       /* as in afm_cfg                                      */
+  int32_t law, n_params;   /* afm_law and its D                                  */
+  int32_t n_modes;         /* 1, 2, 4 or 8                                       */
+  int32_t n_points;        /* Simpson points for the inner products (odd, >= 3)  */
+  int32_t steps_per_cycle, n_cycles, n_skip_cycles;
+  int32_t n_traces;
+} afm_beam_cfg;
+
+/* Modal data computed by the library's initialisation kernel (tests): all host,
+ * [n_modes] each, any may be NULL.  omega rad/s; phi_L = Phi_i(L);
+ * participation = Phi_i(L) <1,Phi_i>/<Phi_i,Phi_i>;
+ * compliance = Phi_i(L)^2 / (mu <Phi_i,Phi_i>)  [1/kg].  Synchronous. */
+int afm_beam_modes(const afm_beam_cfg* cfg, double* beta_L, double* omega,
+                   double* phi_L, double* participation, double* compliance,
+                   void* cuda_stream);
+
+/* Forward batch of the beam model.  params device [P][D]: physical theta, or
+ * PSO coordinates when bounds != NULL (theta_j = 10^x_j where
+ * bounds->log10_scale[j]); trace device [n_traces][W]; misfit device [P].
+ * Asynchronous apart from one 512-byte read-back of the modal constants. */
+int afm_beam_forward_batch(const double* params, int64_t n_particles,
+                           const double* trace, const afm_beam_cfg* cfg,
+                           const afm_bounds* bounds, double* misfit,
+                           void* cuda_stream);
+
+/* afm_pso_invert around the beam forward batch: same swarm rules, same Philox
+ * streams, same outputs. */
+int afm_beam_pso_invert(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                        uint64_t seed, const double* trace,
+                        const afm_beam_cfg* cfg, double* theta_star,
+                        double* J_star, double* swarm_dump, double* gbest_hist,
+                        int32_t* n_iters_done, void* cuda_stream);
+
+/* Tip deflection and velocity of ONE particle, device [N+1] each (or NULL),
+ * index 0 = rest.  theta host [D].  Asynchronous. */
+int afm_beam_trajectory(const double* theta, const afm_beam_cfg* cfg,
+                        double* tip_u, double* tip_v, void* cuda_stream);
+
 /* Philox4x32-10 on the device for n counters (tests: known answers).
  *   ctr device [n][4] uint32, key host [2], out device [n][4].  Async. */
 int afm_philox4x32_10(const uint32_t* ctr, int64_t n, const uint32_t* key,

@@ -25,11 +25,31 @@ SYMBOLS = (
     "afm_forward_batch", "afm_forward_batch_host", "afm_pso_invert",
     "afm_pso_invert_host", "afm_pso_step", "afm_pso_init",
     "afm_pso_shard_init", "afm_pso_shard_eval", "afm_pso_shard_move",
-    "afm_philox4x32_10", "afm_trajectory", "afm_fma_peak", "afm_dispatch_probe",
+    "afm_beam_modes", "afm_beam_forward_batch", "afm_beam_pso_invert",
+    "afm_beam_trajectory", "afm_philox4x32_10", "afm_trajectory", "afm_fma_peak", "afm_dispatch_probe",
     "afm_launch_count",
     "afm_reset_launch_count", "afm_set_option", "afm_last_error",
     "afm_version", "afm_shutdown",
 )
+
+
+class BeamCfg(C.Structure):
+    _fields_ = [("L", C.c_double), ("E", C.c_double), ("I", C.c_double),
+                ("mu", C.c_double), ("Q", C.c_double), ("f_drive", C.c_double),
+                ("A_base", C.c_double), ("A_ref", C.c_double), ("z_c", C.c_double),
+                ("R", C.c_double), ("a0", C.c_double), ("law", C.c_int32),
+                ("n_params", C.c_int32), ("n_modes", C.c_int32),
+                ("n_points", C.c_int32), ("steps_per_cycle", C.c_int32),
+                ("n_cycles", C.c_int32), ("n_skip_cycles", C.c_int32),
+                ("n_traces", C.c_int32)]
+
+    @property
+    def n_steps(self):
+        return self.steps_per_cycle * self.n_cycles
+
+    @property
+    def n_window(self):
+        return self.steps_per_cycle * (self.n_cycles - self.n_skip_cycles)
 
 
 class AfmError(RuntimeError):
@@ -100,6 +120,16 @@ def lib():
         L.afm_pso_shard_move.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), i32,
                                          i32, u64, i32, i32, i64, dp, i32, dp, dp, dp,
                                          dp, dp, dp, dp, vp]
+        L.afm_beam_modes.argtypes = [C.POINTER(BeamCfg), dp, dp, dp, dp, dp, vp]
+        L.afm_beam_forward_batch.argtypes = [dp, i64, dp, C.POINTER(BeamCfg),
+                                             C.POINTER(Bounds), dp, vp]
+        L.afm_beam_pso_invert.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), u64, dp,
+                                          C.POINTER(BeamCfg), dp, dp, dp, dp,
+                                          C.POINTER(i32), vp]
+        L.afm_beam_trajectory.argtypes = [dp, C.POINTER(BeamCfg), dp, dp, vp]
+        for name in ("afm_beam_modes", "afm_beam_forward_batch", "afm_beam_pso_invert",
+                     "afm_beam_trajectory"):
+            getattr(L, name).restype = C.c_int
         L.afm_philox4x32_10.argtypes = [dp, i64, C.POINTER(C.c_uint32), dp, vp]
         L.afm_trajectory.argtypes = [dp, C.POINTER(Cfg), C.c_double, C.c_double,
                                      dp, dp, vp]
@@ -360,6 +390,81 @@ def afm_pso_shard_move(bounds, swarm, n_dims, n_traces, seed, iteration, do_move
                                     _ptr(st["theta_star"]), _ptr(st["J_star"]),
                                     _stream_ptr(stream)))
     return st
+
+
+def beam_cfg_from(wl, **over):
+    """afm_beam_cfg of a workloads.beam_workload() dictionary."""
+    b = wl["beam"]
+    kw = dict(L=b["L"], E=b["E"], I=b["I"], mu=b["mu"], Q=b["Q"], f_drive=b["f_drive"],
+              A_base=b["A_base"], A_ref=b["A_ref"], z_c=b["z_c"], R=b["R"], a0=b["a0"],
+              law=wl["law"], n_params=wl["n_params"], n_modes=b["n_modes"],
+              n_points=b["n_points"], steps_per_cycle=wl["steps_per_cycle"],
+              n_cycles=wl["n_cycles"], n_skip_cycles=wl["n_skip_cycles"],
+              n_traces=wl["n_traces"])
+    kw.update(over)
+    return BeamCfg(**kw)
+
+
+def afm_beam_modes(cfg, stream=None):
+    """dict of host arrays [n_modes]: beta_L, omega, phi_L, participation, compliance."""
+    m = cfg.n_modes
+    out = {k: np.empty(m) for k in ("beta_L", "omega", "phi_L", "participation",
+                                    "compliance")}
+    _check(lib().afm_beam_modes(C.byref(cfg), _hptr(out["beta_L"]), _hptr(out["omega"]),
+                                _hptr(out["phi_L"]), _hptr(out["participation"]),
+                                _hptr(out["compliance"]), _stream_ptr(stream)))
+    return out
+
+
+def afm_beam_forward_batch(params, trace, cfg, bounds=None, misfit=None, stream=None):
+    torch = _torch()
+    params = _dev_f64(params, "params")
+    trace = _dev_f64(trace, "trace")
+    P = params.shape[0]
+    if trace.numel() != cfg.n_traces * cfg.n_window:
+        raise ValueError("trace must hold n_traces * W samples")
+    if misfit is None:
+        misfit = torch.empty(P, dtype=torch.float64, device=params.device)
+    _check(lib().afm_beam_forward_batch(_ptr(params), P, _ptr(trace), C.byref(cfg),
+                                        None if bounds is None else C.byref(bounds),
+                                        _ptr(misfit), _stream_ptr(stream)))
+    return misfit
+
+
+def afm_beam_pso_invert(bounds, swarm, seed, trace, cfg, dump=False, hist=False,
+                        stream=None):
+    torch = _torch()
+    trace = _dev_f64(trace, "trace")
+    if trace.numel() != cfg.n_traces * cfg.n_window:
+        raise ValueError("trace must hold n_traces * W samples")
+    D, T = cfg.n_params, cfg.n_traces
+    PT = swarm.n_particles * T
+    th = np.empty((T, D), dtype=np.float64)
+    Js = np.empty(T, dtype=np.float64)
+    dmp = (torch.empty((swarm.n_iters, PT, 3 * D + 2), dtype=torch.float64,
+                       device=trace.device) if dump else None)
+    gh = (torch.empty((swarm.n_iters, T, D + 1), dtype=torch.float64,
+                      device=trace.device) if hist else None)
+    done = C.c_int32(0)
+    _check(lib().afm_beam_pso_invert(C.byref(bounds), C.byref(swarm), int(seed),
+                                     _ptr(trace), C.byref(cfg), _hptr(th), _hptr(Js),
+                                     _ptr(dmp), _ptr(gh), C.byref(done),
+                                     _stream_ptr(stream)))
+    return dict(theta_star=th, J_star=Js, n_iters_done=done.value, dump=dmp,
+                gbest_hist=gh)
+
+
+def afm_beam_trajectory(theta, cfg, stream=None):
+    """(tip_u[N+1], tip_v[N+1]) of one particle, as numpy arrays."""
+    torch = _torch()
+    theta = _host_f64(theta)
+    N = cfg.n_steps
+    u = torch.empty(N + 1, dtype=torch.float64, device="cuda")
+    v = torch.empty(N + 1, dtype=torch.float64, device="cuda")
+    _check(lib().afm_beam_trajectory(_hptr(theta), C.byref(cfg), _ptr(u), _ptr(v),
+                                     _stream_ptr(stream)))
+    torch.cuda.synchronize()
+    return u.cpu().numpy(), v.cpu().numpy()
 
 
 def afm_philox4x32_10(ctr, key, stream=None):

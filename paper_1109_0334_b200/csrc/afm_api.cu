@@ -728,6 +728,267 @@ int afm_pso_shard_move(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   return AFM_OK;
 }
 
+// ---- multi-mode beam ------------------------------------------------------------
+static int validate_beam(const afm_beam_cfg* c) {
+  if (!c) return fail(AFM_EINVAL, "beam cfg is NULL");
+  if (c->law < AFM_LAW_NONE || c->law > AFM_LAW_KELVIN_VOIGT)
+    return fail(AFM_EINVAL, "unknown law %d", c->law);
+  if (c->law == AFM_LAW_NONE) {
+    if (c->n_params < 0 || c->n_params > 4)
+      return fail(AFM_EINVAL, "n_params %d out of range 0..4", c->n_params);
+  } else if (c->n_params != law_dims(c->law)) {
+    return fail(AFM_EINVAL, "law %d needs n_params = %d", c->law, law_dims(c->law));
+  }
+  if (!(c->L > 0) || !(c->E > 0) || !(c->I > 0) || !(c->mu > 0) || !(c->Q > 0) ||
+      !(c->f_drive > 0) || !(c->A_ref > 0) || !isfinite(c->A_base) ||
+      !isfinite(c->z_c))
+    return fail(AFM_EINVAL, "L, E, I, mu, Q, f_drive, A_ref must be positive");
+  if ((c->law == AFM_LAW_DMT || c->law == AFM_LAW_DMT_VISC) &&
+      (!(c->R > 0) || !(c->a0 > 0)))
+    return fail(AFM_EINVAL, "DMT laws need R > 0 and a0 > 0");
+  if (c->n_modes != 1 && c->n_modes != 2 && c->n_modes != 4 && c->n_modes != 8)
+    return fail(AFM_EINVAL, "n_modes must be 1, 2, 4 or 8");
+  if (c->n_points < 3 || !(c->n_points & 1) || c->n_points > 100001)
+    return fail(AFM_EINVAL, "n_points must be odd, 3..100001");
+  if (c->steps_per_cycle < 1 || c->n_cycles < 1)
+    return fail(AFM_EINVAL, "steps_per_cycle and n_cycles must be >= 1");
+  if (c->n_skip_cycles < 0 || c->n_skip_cycles >= c->n_cycles)
+    return fail(AFM_EINVAL, "need 0 <= n_skip_cycles < n_cycles");
+  if ((int64_t)c->steps_per_cycle * c->n_cycles > (int64_t)1 << 30)
+    return fail(AFM_EINVAL, "more than 2^30 steps");
+  if (c->n_traces < 1) return fail(AFM_EINVAL, "n_traces must be >= 1");
+  return AFM_OK;
+}
+
+// Initialisation kernel -> host copy of the modal constants, then the scaled
+// force-law factors with m = m_1.  Workspace lock held.
+static int beam_prepare(const afm_beam_cfg* c, BeamConsts* bc, BeamModeConsts* mo,
+                        cudaStream_t st) {
+  const double w = 2.0 * M_PI * c->f_drive;
+  const double h = 2.0 * M_PI / (w * (double)c->steps_per_cycle);
+  if (g_ws.scratch.ensure(sizeof(BeamModeConsts) + 64))
+    return fail(AFM_ECUDA, "cudaMalloc failed");
+  BeamModeConsts* dmo = (BeamModeConsts*)((char*)g_ws.scratch.p + 64);
+  CUDA_TRY(cudaMemsetAsync(dmo, 0, sizeof(BeamModeConsts), st));
+  LAUNCHED(launch_beam_setup(*c, h, dmo, st));
+  CUDA_TRY(cudaMemcpyAsync(mo, dmo, sizeof(BeamModeConsts), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  memset(bc, 0, sizeof(*bc));
+  const double m = mo->m1;
+  const double sqR = sqrt(c->R > 0 ? c->R : 0.0);
+  bc->h = h;
+  bc->w_drive = w;
+  bc->zc = c->z_c;
+  bc->a0 = c->a0;
+  bc->inv_a0sq = (c->a0 > 0) ? 1.0 / (c->a0 * c->a0) : 0.0;
+  bc->c_vdw = h * h * c->R / (6.0 * m);
+  bc->c_hertz = h * h * (4.0 / 3.0) * sqR / m;
+  bc->c_visc = h * sqR / m;
+  bc->c_force = h * h / m;
+  bc->c_damp = h / m;
+  bc->u_max = 100.0 * c->A_ref;
+  bc->law = c->law;
+  bc->D = c->n_params;
+  bc->M = c->n_modes;
+  bc->N = c->steps_per_cycle * c->n_cycles;
+  bc->W = c->steps_per_cycle * (c->n_cycles - c->n_skip_cycles);
+  bc->n0 = bc->N - bc->W;
+  int T = g_opt_tile > 0 ? g_opt_tile : 64;
+  if (T > bc->N) T = bc->N;
+  bc->T = T;
+  bc->n_tiles = (bc->N + T - 1) / T;
+  return AFM_OK;
+}
+
+// cos(w t) at the three abscissae of every step + the trace: the point-mass
+// stream builder with unit amplitude and no offsets.
+static int beam_stream(const BeamConsts& bc, const double* trace, int n_traces,
+                       cudaStream_t st) {
+  ModelConsts mc;
+  memset(&mc, 0, sizeof(mc));
+  mc.h = bc.h;
+  mc.w_drive = bc.w_drive;
+  mc.drive_amp = 1.0;
+  mc.N = bc.N;
+  mc.W = bc.W;
+  mc.n0 = bc.n0;
+  if (g_ws.stream.ensure((size_t)n_traces * bc.N * 32 + 64))
+    return fail(AFM_ECUDA, "cudaMalloc of the time-tile stream failed");
+  LAUNCHED(launch_build_stream(mc, trace, n_traces, (double*)g_ws.stream.p, st));
+  return AFM_OK;
+}
+
+int afm_beam_modes(const afm_beam_cfg* cfg, double* beta_L, double* omega,
+                   double* phi_L, double* participation, double* compliance,
+                   void* cuda_stream) {
+  int rc = validate_beam(cfg);
+  if (rc) return rc;
+  if ((rc = check_device())) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  if ((rc = acquire_ws(st))) return rc;
+  BeamConsts bc;
+  BeamModeConsts mo;
+  if ((rc = beam_prepare(cfg, &bc, &mo, st))) return rc;
+  for (int i = 0; i < cfg->n_modes; ++i) {
+    if (beta_L) beta_L[i] = mo.bL[i];
+    if (omega) omega[i] = mo.omega[i];
+    if (phi_L) phi_L[i] = mo.phiL[i];
+    if (participation) participation[i] = mo.part[i];
+    if (compliance) compliance[i] = mo.compl_[i];
+  }
+  return release_ws(st);
+}
+
+int afm_beam_forward_batch(const double* params, int64_t n_particles,
+                           const double* trace, const afm_beam_cfg* cfg,
+                           const afm_bounds* bounds, double* misfit,
+                           void* cuda_stream) {
+  int rc = validate_beam(cfg);
+  if (rc) return rc;
+  if (n_particles < 1 || n_particles % cfg->n_traces)
+    return fail(AFM_EINVAL, "n_particles must be a positive multiple of n_traces");
+  if (!trace || !misfit || (!params && cfg->n_params > 0))
+    return fail(AFM_EINVAL, "NULL array");
+  if (bounds && (rc = validate_bounds(bounds, cfg->n_params))) return rc;
+  if ((rc = check_device())) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  if ((rc = acquire_ws(st))) return rc;
+  BeamConsts bc;
+  BeamModeConsts mo;
+  if ((rc = beam_prepare(cfg, &bc, &mo, st))) return rc;
+  if ((rc = beam_stream(bc, trace, cfg->n_traces, st))) return rc;
+  IntegrateIO io;
+  memset(&io, 0, sizeof(io));
+  io.params = params;
+  io.stream = (const double*)g_ws.stream.p;
+  io.J = misfit;
+  io.per = n_particles / cfg->n_traces;
+  io.n_traces = cfg->n_traces;
+  io.mode = 0;
+  if (bounds) {  // coordinates in, personal bests untouched: map only
+    io.box = make_box(bounds, cfg->n_params);
+    io.mode = 2;
+  }
+  LAUNCHED(launch_beam_integrate(bc, mo, io, pick_block(io.per, io.n_traces), st));
+  return release_ws(st);
+}
+
+int afm_beam_pso_invert(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                        uint64_t seed, const double* trace,
+                        const afm_beam_cfg* cfg, double* theta_star,
+                        double* J_star, double* swarm_dump, double* gbest_hist,
+                        int32_t* n_iters_done, void* cuda_stream) {
+  int rc = validate_beam(cfg);
+  if (rc) return rc;
+  if (cfg->n_params < 1) return fail(AFM_EINVAL, "nothing to invert: n_params = 0");
+  if ((rc = validate_bounds(bounds, cfg->n_params))) return rc;
+  if ((rc = validate_swarm(swarm))) return rc;
+  if (!trace || !theta_star || !J_star)
+    return fail(AFM_EINVAL, "trace/theta_star/J_star is NULL");
+  if ((rc = check_device())) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  if ((rc = acquire_ws(st))) return rc;
+  BeamConsts bc;
+  BeamModeConsts mo;
+  if ((rc = beam_prepare(cfg, &bc, &mo, st))) return rc;
+  if ((rc = beam_stream(bc, trace, cfg->n_traces, st))) return rc;
+  const int D = cfg->n_params, T = cfg->n_traces;
+  const int64_t per = swarm->n_particles, PT = per * T;
+  const int block = pick_block(per, T);
+  const int bpt = blocks_per_trace(per, block);
+  const size_t n_dbl = (size_t)PT * (3 * D + 2) + (size_t)T * (2 * D + 2);
+  if (g_ws.swarm.ensure(n_dbl * 8) || g_ws.cand.ensure((size_t)bpt * T * sizeof(Cand)))
+    return fail(AFM_ECUDA, "cudaMalloc of the PSO workspace failed");
+  double* x = (double*)g_ws.swarm.p;
+  double* v = x + PT * D;
+  double* pbest = v + PT * D;
+  double* J = pbest + PT * D;
+  double* pbestJ = J + PT;
+  double* gbest = pbestJ + PT;
+  double* gbestJ = gbest + (size_t)T * D;
+  double* th_dev = gbestJ + T;
+  double* Js_dev = th_dev + (size_t)T * D;
+  if ((rc = ensure_pinned((size_t)T * 8))) return rc;
+  BoxDev box = make_box(bounds, D);
+  SwarmDev sw = {swarm->w, swarm->c1, swarm->c2};
+  LAUNCHED(launch_pso_init(box, D, per, T, seed, 0, x, v, pbest, pbestJ, gbest,
+                           gbestJ, st));
+  IntegrateIO io;
+  memset(&io, 0, sizeof(io));
+  io.params = x;
+  io.stream = (const double*)g_ws.stream.p;
+  io.J = J;
+  io.pbest = pbest;
+  io.pbestJ = pbestJ;
+  io.cand = (Cand*)g_ws.cand.p;
+  io.box = box;
+  io.per = per;
+  io.n_traces = T;
+  io.mode = 1;
+  int done = 0;
+  for (int it = 0; it < swarm->n_iters; ++it) {
+    const bool last = (it == swarm->n_iters - 1);
+    LAUNCHED(launch_beam_integrate(bc, mo, io, block, st));
+    LAUNCHED(launch_pso_gbest(
+        box, D, T, bpt, (Cand*)g_ws.cand.p, pbest, gbest, gbestJ,
+        gbest_hist ? gbest_hist + (size_t)it * T * (D + 1) : nullptr, th_dev,
+        Js_dev, st));
+    bool stop = last;
+    if (!stop && swarm->j_target > 0) {
+      double* hJ = (double*)g_ws.pinned;
+      CUDA_TRY(cudaMemcpyAsync(hJ, gbestJ, (size_t)T * 8, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(cudaStreamSynchronize(st));
+      stop = true;
+      for (int s = 0; s < T; ++s)
+        if (!(hJ[s] <= swarm->j_target)) stop = false;
+    }
+    double* dump_row =
+        swarm_dump ? swarm_dump + (size_t)it * PT * (3 * D + 2) : nullptr;
+    if (!stop || dump_row)
+      LAUNCHED(launch_pso_move(box, sw, D, per, T, seed, 0, (uint32_t)it,
+                               stop ? 0 : 1, J, x, v, pbest, pbestJ, gbest,
+                               dump_row, st));
+    done = it + 1;
+    if (stop) break;
+  }
+  CUDA_TRY(cudaMemcpyAsync(theta_star, th_dev, (size_t)T * D * 8,
+                           cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaMemcpyAsync(J_star, Js_dev, (size_t)T * 8, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  if (n_iters_done) *n_iters_done = done;
+  return release_ws(st);
+}
+
+int afm_beam_trajectory(const double* theta, const afm_beam_cfg* cfg,
+                        double* tip_u, double* tip_v, void* cuda_stream) {
+  int rc = validate_beam(cfg);
+  if (rc) return rc;
+  if (!theta && cfg->n_params > 0) return fail(AFM_EINVAL, "theta is NULL");
+  if ((rc = check_device())) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  if ((rc = acquire_ws(st))) return rc;
+  BeamConsts bc;
+  BeamModeConsts mo;
+  if ((rc = beam_prepare(cfg, &bc, &mo, st))) return rc;
+  // zero trace (unused by the trajectory kernel) placed after the stream
+  if (g_ws.stream.ensure((size_t)bc.N * 32 + (size_t)bc.W * 8 + 128))
+    return fail(AFM_ECUDA, "cudaMalloc failed");
+  double* zero_trace = (double*)((char*)g_ws.stream.p + (size_t)bc.N * 32 + 64);
+  CUDA_TRY(cudaMemsetAsync(zero_trace, 0, (size_t)bc.W * 8, st));
+  if ((rc = beam_stream(bc, zero_trace, 1, st))) return rc;
+  double* th_dev = (double*)g_ws.scratch.p;  // first 64 bytes of scratch
+  if (cfg->n_params > 0)
+    CUDA_TRY(cudaMemcpyAsync(th_dev, theta, (size_t)cfg->n_params * 8,
+                             cudaMemcpyHostToDevice, st));
+  LAUNCHED(launch_beam_trajectory(bc, mo, th_dev, (const double*)g_ws.stream.p,
+                                  tip_u, tip_v, st));
+  return release_ws(st);
+}
+
 int afm_philox4x32_10(const uint32_t* ctr, int64_t n, const uint32_t* key,
                       uint32_t* out, void* cuda_stream) {
   if (!ctr || !key || !out || n < 0)

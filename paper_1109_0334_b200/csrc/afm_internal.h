@@ -66,6 +66,25 @@ struct ModelConstsF32 {
   int32_t law, D, N, n0, W, T, n_tiles, pad_;
 };
 
+// Per-mode constants of the beam kernel in per-step, tip-weighted variables
+// (afm_beam.cu): a_i = Phi_i(L) eta_i, b_i = h Phi_i(L) eta_i',
+//   b_i' = Gamma_i cos(w t) - alpha_i b_i - beta_i a_i + kappa_i fhat,
+// fhat = (h^2/m_1) F_ts, m_1 = first-mode effective mass, kappa_0 = 1.
+struct BeamModeConsts {
+  double Gamma[8], alpha[8], beta[8], kappa[8];
+  // raw modal data for afm_beam_modes
+  double bL[8], omega[8], phiL[8], part[8], compl_[8];
+  double m1;  // mu <Phi_0,Phi_0> / Phi_0(L)^2
+};
+
+struct BeamConsts {
+  double h, w_drive;
+  double zc, a0, inv_a0sq;
+  double c_vdw, c_hertz, c_visc, c_force, c_damp;  // as ModelConsts, with m = m_1
+  double u_max;      // 100 A_ref
+  int32_t law, D, M, N, n0, W, T, n_tiles;
+};
+
 struct BoxDev {
   double lo[4], hi[4];
   int32_t lg[4];
@@ -143,6 +162,13 @@ int launch_fma_peak(int precision, int iters, int blocks, int threads,
 int launch_dispatch_probe(int mode, int warps_per_subpartition, int n_sm,
                           const double* in, double* sink, double* ns_per_dfma,
                           cudaStream_t st);
+int launch_beam_setup(const afm_beam_cfg& cfg, double h, BeamModeConsts* dev_out,
+                      cudaStream_t st);
+int launch_beam_integrate(const BeamConsts& bc, const BeamModeConsts& mo,
+                          const IntegrateIO& io, int block, cudaStream_t st);
+int launch_beam_trajectory(const BeamConsts& bc, const BeamModeConsts& mo,
+                           const double* theta_dev, const double* stream,
+                           double* tip_u, double* tip_v, cudaStream_t st);
 int launch_philox(const uint32_t* ctr, int64_t n, uint32_t k0, uint32_t k1,
                   uint32_t* out, cudaStream_t st);
 
