@@ -434,6 +434,39 @@ def extras(afm, torch, dev, main_prec):
     return ex
 
 
+def _one_batch_beam(args, afm, torch, dev):
+    """--one-batch 7: the paper's 8-mode Euler-Bernoulli forward model
+    (workloads.beam_workload): one forward batch of --beam-particles particles, or
+    with --invert the 1 024 x 40 inversion."""
+    wl = wlm.beam_workload()
+    cfg = afm.beam_cfg_from(wl)
+    u, _ = afm.afm_beam_trajectory(wl["truth"], cfg)
+    trace = torch.as_tensor(u[-wl["n_window"]:][None, :] + wlm.trace_noise(wl), device=dev)
+    if args.invert:
+        b, sw = afm.bounds_from(wl), afm.swarm_from(wl)
+        afm.afm_beam_pso_invert(b, sw, wl["pso_seed"], trace, cfg)
+        t0 = time.perf_counter()
+        r = afm.afm_beam_pso_invert(b, sw, wl["pso_seed"], trace, cfg)
+        ms = (time.perf_counter() - t0) * 1e3
+        units = float(sw.n_particles) * wl["n_steps"] * sw.n_iters
+        print(json.dumps({"one_batch": 7, "mode": "inversion", "dtype": "f64", "ms": ms,
+                          "n_modes": cfg.n_modes,
+                          "particle_steps_per_s": units / (ms * 1e-3),
+                          "theta_star": [float(x) for x in r["theta_star"][0]]}))
+        return 0
+    P = args.beam_particles
+    params = torch.as_tensor(wlm.draw_params(wl, P, seed=1), device=dev)
+    out = torch.empty(P, dtype=torch.float64, device=dev)
+    ms = _event_ms(torch, lambda: afm.afm_beam_forward_batch(params, trace, cfg, misfit=out),
+                   args.steps)
+    # FP64 instructions per particle-step of the 8-mode step (DESIGN.md section 6)
+    print(json.dumps({"one_batch": 7, "mode": "forward", "dtype": "f64", "ms": ms,
+                      "n_modes": cfg.n_modes, "particles": P,
+                      "particle_steps_per_s": float(P) * wl["n_steps"] / (ms * 1e-3),
+                      "mode_steps_per_s": float(P) * wl["n_steps"] * cfg.n_modes / (ms * 1e-3)}))
+    return 0
+
+
 def run_one_batch(args):
     """--one-batch CFG: one full-size forward batch (or, with --invert, the full
     inversion) of BASELINE.json configs[CFG], for ncu captures of the other
@@ -442,6 +475,8 @@ def run_one_batch(args):
     from paper_1109_0334_b200 import afm
     torch.cuda.set_device(0)
     dev = torch.device("cuda", 0)
+    if args.one_batch == 7:
+        return _one_batch_beam(args, afm, torch, dev)
     wl = wlm.config(args.one_batch)
     prec = afm.F32 if args.precision == "f32" else afm.F64
     cfg = afm.cfg_from(wl, precision=prec)
@@ -487,8 +522,10 @@ def main():
                     help="oracle sample size of the cpu_baseline leg")
     ap.add_argument("--ref-particles", type=int, default=512,
                     help="oracle sample size per step of --impl reference")
-    ap.add_argument("--one-batch", type=int, default=None, choices=[0, 1, 2, 3, 4],
-                    help="profiling aid: one full-size forward batch of configs[N]")
+    ap.add_argument("--one-batch", type=int, default=None, choices=[0, 1, 2, 3, 4, 7],
+                    help="profiling aid: one full-size forward batch of configs[N]; "
+                         "7 = the paper's 8-mode beam workload")
+    ap.add_argument("--beam-particles", type=int, default=65536)
     ap.add_argument("--invert", action="store_true",
                     help="with --one-batch: time the full PSO inversion instead")
     args = ap.parse_args()
