@@ -331,7 +331,10 @@ void afm_reset_launch_count(void);
  * kernel: 32, 64 or 128; 0 = auto), "tile" (steps per time tile; 0 = auto),
  * "ppt" (particles per thread: 1 or 2; 0 = auto), "form" (FP64 kernel form:
  * 1 = throughput, fewest FP64 instructions; 2 = latency, shortest dependent
- * chains; 0 = auto by warps per SM sub-partition).
+ * chains; 0 = auto by warps per SM sub-partition), "pack" (order the particles
+ * of a DMT-law batch by trace, initial phase and stiffness so that the lanes of a
+ * warp touch the sample together: 1 = never, 2 = always, 0 = auto in the
+ * throughput regime; results do not depend on it).
  * Returns AFM_EINVAL for an unknown name or value. */
 int afm_set_option(const char* name, int64_t value);
 

@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["afm_kernels.cu", "afm_kernels_f32.cu", "afm_microbench.cu", "afm_beam.cu", "afm_api.cu"]
+SOURCES = ["afm_kernels.cu", "afm_kernels_f32.cu", "afm_microbench.cu", "afm_beam.cu", "afm_sort.cu", "afm_api.cu"]
 HEADERS = ["afm_internal.h", "afm_device_common.cuh", "afm_device.cuh", "afm_device_f32.cuh"]
 OUT = os.path.join(HERE, "libafm_b200.so")
 

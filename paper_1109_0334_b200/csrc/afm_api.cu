@@ -54,6 +54,7 @@ int g_opt_block = 0;  // 0 = auto
 int g_opt_tile = 0;   // 0 = auto
 int g_opt_ppt = 0;    // 0 = auto
 int g_opt_form = 0;   // 0 = auto, 1 = throughput form, 2 = latency form
+int g_opt_pack = 0;   // 0 = auto, 1 = never, 2 = always (DMT laws only)
 int g_n_sm = 148;
 
 // ---- grow-only device workspace ------------------------------------------------
@@ -89,6 +90,7 @@ struct Workspace {
   Buffer cand;                         // block candidates
   Buffer h_params, h_trace, h_z0v0, h_misfit;  // staging for the *_host calls
   Buffer scratch;                      // theta for afm_trajectory
+  Buffer sort;                         // warp-packing keys, order, radix-sort temp
   cudaEvent_t last_use = nullptr;      // orders reuse across streams
   cudaStream_t last_stream = nullptr;
   bool checked_device = false;
@@ -295,6 +297,49 @@ int pick_variant(int64_t per, int n_traces, int ppt) {
   return warps < (int64_t)2 * 4 * g_n_sm ? 1 : 0;
 }
 
+// Warp packing (afm_sort.cu) for the DMT laws in the throughput regime of a
+// forward batch: on success *order is the device order array and the packed
+// copies of params / z0v0 and a packed misfit buffer are ready; *order stays
+// nullptr when packing does not apply.  Lock held.
+struct Packed {
+  const uint32_t* order = nullptr;
+  double* params = nullptr;
+  double* z0v0 = nullptr;
+  double* J = nullptr;
+};
+
+int pack_inputs(const afm_cfg* cfg, const double* params, const double* z0v0,
+                int64_t per, int n_traces, Packed* pk, cudaStream_t st) {
+  const bool dmt = (cfg->law == AFM_LAW_DMT || cfg->law == AFM_LAW_DMT_VISC);
+  const int D = cfg->n_params;
+  const int64_t PT = per * n_traces;
+  const int64_t warps = ((per + 31) / 32) * n_traces;
+  if (!dmt || g_opt_pack == 1 || PT >= ((int64_t)1 << 31) || n_traces >= (1 << 24))
+    return AFM_OK;
+  if (g_opt_pack == 0 && warps < (int64_t)2 * 4 * g_n_sm) return AFM_OK;
+  const size_t ws = sort_workspace_bytes(PT);
+  const size_t a256 = 255;
+  const size_t o_bytes = ((size_t)PT * 4 + a256) & ~a256;
+  const size_t p_bytes = ((size_t)PT * D * 8 + a256) & ~a256;
+  const size_t z_bytes = ((size_t)PT * 16 + a256) & ~a256;
+  const size_t j_bytes = ((size_t)PT * 8 + a256) & ~a256;
+  if (g_ws.sort.ensure(o_bytes + p_bytes + z_bytes + j_bytes + ws + 256))
+    return fail(AFM_ECUDA, "cudaMalloc of the packing workspace failed");
+  char* base = (char*)g_ws.sort.p;
+  uint32_t* order = (uint32_t*)base;
+  pk->params = (double*)(base + o_bytes);
+  pk->z0v0 = z0v0 ? (double*)(base + o_bytes + p_bytes) : nullptr;
+  pk->J = (double*)(base + o_bytes + p_bytes + z_bytes);
+  void* scratch = base + o_bytes + p_bytes + z_bytes + j_bytes;
+  const int n = launch_pack_order(params, z0v0, D, per, PT, 2.0 * M_PI * cfg->f_drive,
+                                  cfg->z0, cfg->v0, scratch, ws, order, st);
+  if (n < 0) return fail(AFM_ECUDA, "radix sort of the packing keys failed");
+  g_launches += n;
+  LAUNCHED(launch_pack_gather(order, params, z0v0, D, PT, pk->params, pk->z0v0, st));
+  pk->order = order;
+  return AFM_OK;
+}
+
 BoxDev make_box(const afm_bounds* b, int D) {
   BoxDev bd;
   memset(&bd, 0, sizeof(bd));
@@ -357,11 +402,18 @@ int forward_locked(const double* params, int64_t P, const double* trace,
   io.per = per;
   io.n_traces = cfg->n_traces;
   io.mode = 0;
-  if (f32) {
-    LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
-    return release_ws(st);
+  Packed pk;
+  if ((rc = pack_inputs(cfg, params, z0v0, per, cfg->n_traces, &pk, st))) return rc;
+  if (pk.order) {
+    io.params = pk.params;
+    io.z0v0 = pk.z0v0;
+    io.J = pk.J;
   }
-  LAUNCHED(launch_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st));
+  if (f32)
+    LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
+  else
+    LAUNCHED(launch_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st));
+  if (pk.order) LAUNCHED(launch_pack_scatter(pk.order, pk.J, P, misfit, st));
   return release_ws(st);
 }
 
@@ -1110,6 +1162,11 @@ int afm_set_option(const char* name, int64_t value) {
     g_opt_form = (int)value;
     return AFM_OK;
   }
+  if (!strcmp(name, "pack")) {
+    if (value < 0 || value > 2) return fail(AFM_EINVAL, "pack must be 0, 1 or 2");
+    g_opt_pack = (int)value;
+    return AFM_OK;
+  }
   if (!strcmp(name, "tile")) {
     if (value < 0 || value > 2048)
       return fail(AFM_EINVAL, "tile must be in 0..2048");
@@ -1132,6 +1189,7 @@ void afm_shutdown(void) {
   g_ws.h_z0v0.release();
   g_ws.h_misfit.release();
   g_ws.scratch.release();
+  g_ws.sort.release();
   if (g_ws.pinned) cudaFreeHost(g_ws.pinned);
   g_ws.pinned = nullptr;
   g_ws.pinned_cap = 0;

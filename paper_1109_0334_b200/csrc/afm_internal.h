@@ -169,6 +169,21 @@ int launch_beam_integrate(const BeamConsts& bc, const BeamModeConsts& mo,
 int launch_beam_trajectory(const BeamConsts& bc, const BeamModeConsts& mo,
                            const double* theta_dev, const double* stream,
                            double* tip_u, double* tip_v, cudaStream_t st);
+// Warp packing (afm_sort.cu): order[] = particle indices sorted by (trace, initial
+// phase bin, stiffness-like parameter), so that the lanes of a warp touch the
+// sample at about the same time.  ws/ws_bytes: scratch for the radix sort.  The
+// integrate kernels are left untouched: inputs are gathered into packed copies
+// and the misfits scattered back.
+size_t sort_workspace_bytes(int64_t PT);
+int launch_pack_order(const double* params, const double* z0v0, int D, int64_t per,
+                      int64_t PT, double w_drive, double z0_default,
+                      double v0_default, void* ws, size_t ws_bytes,
+                      uint32_t* order, cudaStream_t st);
+int launch_pack_gather(const uint32_t* order, const double* params,
+                       const double* z0v0, int D, int64_t PT, double* params_s,
+                       double* z0v0_s, cudaStream_t st);
+int launch_pack_scatter(const uint32_t* order, const double* J_s, int64_t PT,
+                        double* J, cudaStream_t st);
 int launch_philox(const uint32_t* ctr, int64_t n, uint32_t k0, uint32_t k1,
                   uint32_t* out, cudaStream_t st);
 

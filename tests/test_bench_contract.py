@@ -37,7 +37,8 @@ def test_gpu_arm_json_line(prec):
     d = _run("--steps", "3", "--warmup", "3", "--no-extras", "--precision", prec)
     assert BASE_KEYS | {"roofline", "clocks"} <= set(d)
     assert d["dtype"] == prec and d["n_gpus"] == 1 and d["steps"] == 3
-    assert d["gpu_launches"] == 3 * 5      # build_stream + integrate + best + gbest + move
+    # build_stream, pack_key, pack_gather, integrate, pack_scatter, best, gbest, move
+    assert d["gpu_launches"] == 3 * 8
     r = d["roofline"]
     assert r["bound"] == "alu" and 0.05 < r["frac"] < 1.0 and r["traffic"] > 0
     assert r["achieved"] == pytest.approx(r["frac"] * r["peak"])

@@ -253,3 +253,40 @@ def test_bad_arguments_are_rejected(afm):
     J = afm.afm_forward_batch(p + 1e-19, t, cfg)   # a valid call still works afterwards
     torch.cuda.synchronize()
     assert J.shape == (4,)
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_warp_packing_changes_no_result(afm, precision):
+    """afm_set_option("pack"): the particles of a DMT batch are integrated in the
+    order (trace, initial phase bin, stiffness) instead of the caller's order.
+    Every misfit must be bit-identical, for one trace with random phases and for
+    several traces, forward and inside an inversion."""
+    import torch
+    wl = wlm.scaled(wlm.config(1), n_cycles=12, n_skip_cycles=6)
+    trace = oracle_trace(wl)
+    n = 3000 + 7
+    params = wlm.draw_params(wl, n, seed=51)
+    z0v0 = wlm.draw_initial_states(wl, n, seed=52)
+    out = {}
+    for pack in (1, 2):
+        afm.afm_set_option("pack", pack)
+        try:
+            out[pack] = _gpu_forward(afm, wl, params, trace, z0v0, precision=precision)
+            w4 = wlm.scaled(wlm.config(4), n_cycles=8, n_skip_cycles=4, n_traces=3)
+            tr4 = oracle_trace(w4, truths=wlm.pixel_truths(w4))
+            p4 = wlm.draw_params(w4, 3 * 211, seed=53)
+            out[pack, 4] = _gpu_forward(afm, w4, p4, tr4, precision=precision)
+            w2 = wlm.scaled(wlm.config(2), n_cycles=8, n_skip_cycles=4, n_particles=300,
+                            n_iters=4)
+            g = afm.afm_pso_invert(afm.bounds_from(w2), afm.swarm_from(w2), 0,
+                                   torch.as_tensor(oracle_trace(w2), device="cuda"),
+                                   afm.cfg_from(w2, precision=precision), dump=True)
+            out[pack, 2] = g["dump"].cpu().numpy()
+        finally:
+            afm.afm_set_option("pack", 0)
+    assert np.array_equal(out[1], out[2])
+    assert np.array_equal(out[1, 4], out[2, 4])
+    assert np.array_equal(out[1, 2], out[2, 2])
+    if precision == 0:
+        Jo = _oracle_forward(wl, params, trace, z0v0)
+        assert rel_err(out[2], Jo).max() < TOL_F64
