@@ -309,7 +309,8 @@ struct Packed {
 };
 
 int pack_inputs(const afm_cfg* cfg, const double* params, const double* z0v0,
-                int64_t per, int n_traces, Packed* pk, cudaStream_t st) {
+                int64_t per, int n_traces, const BoxDev* map, Packed* pk,
+                cudaStream_t st) {
   const bool dmt = (cfg->law == AFM_LAW_DMT || cfg->law == AFM_LAW_DMT_VISC);
   const int D = cfg->n_params;
   const int64_t PT = per * n_traces;
@@ -335,7 +336,7 @@ int pack_inputs(const afm_cfg* cfg, const double* params, const double* z0v0,
                                   cfg->z0, cfg->v0, scratch, ws, order, st);
   if (n < 0) return fail(AFM_ECUDA, "radix sort of the packing keys failed");
   g_launches += n;
-  LAUNCHED(launch_pack_gather(order, params, z0v0, D, PT, pk->params, pk->z0v0, st));
+  LAUNCHED(launch_pack_gather(order, params, z0v0, D, PT, pk->params, pk->z0v0, map, st));
   pk->order = order;
   return AFM_OK;
 }
@@ -403,7 +404,8 @@ int forward_locked(const double* params, int64_t P, const double* trace,
   io.n_traces = cfg->n_traces;
   io.mode = 0;
   Packed pk;
-  if ((rc = pack_inputs(cfg, params, z0v0, per, cfg->n_traces, &pk, st))) return rc;
+  if ((rc = pack_inputs(cfg, params, z0v0, per, cfg->n_traces, nullptr, &pk, st)))
+    return rc;
   if (pk.order) {
     io.params = pk.params;
     io.z0v0 = pk.z0v0;
@@ -571,7 +573,7 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
   // gbest [T][D]; gbestJ [T]; theta* [T][D]; J* [T]
   const size_t n_dbl = (size_t)PT * (3 * D + 2) + (size_t)T * (2 * D + 2);
   if (g_ws.swarm.ensure(n_dbl * 8) ||
-      g_ws.cand.ensure((size_t)bpt * T * sizeof(Cand)) ||
+      g_ws.cand.ensure((size_t)(bpt + blocks_per_trace(per, 128)) * T * sizeof(Cand)) ||
       g_ws.stream.ensure((size_t)T * mc.N * 32 + 64))
     return fail(AFM_ECUDA, "cudaMalloc of the PSO workspace failed");
   double* x = (double*)g_ws.swarm.p;
@@ -611,12 +613,34 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
   int done = 0;
   for (int it = 0; it < swarm->n_iters; ++it) {
     const bool last = (it == swarm->n_iters - 1);
-    if (f32)
+    // throughput regime, DMT laws: warp packing (afm_sort.cu).  The swarm state
+    // stays in particle order; theta = map(x) is gathered in packed order, the
+    // forward-only kernel runs on it, the misfits are scattered back and the
+    // stand-alone personal-best kernel takes the place of the fused epilogue.
+    Packed pk;
+    if ((rc = pack_inputs(cfg, x, nullptr, per, T, &box, &pk, st))) return rc;
+    int n_cand = bpt;
+    if (pk.order) {
+      IntegrateIO iof = io;
+      iof.params = pk.params;
+      iof.J = pk.J;
+      iof.mode = 0;
+      if (f32)
+        LAUNCHED(launch_integrate_f32(mf, iof, block, ppt, st));
+      else
+        LAUNCHED(launch_integrate_f64(mc, iof, block,
+                                      pick_variant(iof.per, iof.n_traces, ppt), st));
+      LAUNCHED(launch_pack_scatter(pk.order, pk.J, PT, J, st));
+      n_cand = blocks_per_trace(per, 128);
+      LAUNCHED(launch_pso_best(D, per, T, J, x, pbest, pbestJ, (Cand*)g_ws.cand.p, 128,
+                               st));
+    } else if (f32) {
       LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
-    else
+    } else {
       LAUNCHED(launch_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st));
+    }
     LAUNCHED(launch_pso_gbest(
-        box, D, T, bpt, (Cand*)g_ws.cand.p, pbest, gbest, gbestJ,
+        box, D, T, n_cand, (Cand*)g_ws.cand.p, pbest, gbest, gbestJ,
         gbest_hist ? gbest_hist + (size_t)it * T * (D + 1) : nullptr, th_dev,
         Js_dev, st));
     bool stop = last;

@@ -181,7 +181,7 @@ int launch_pack_order(const double* params, const double* z0v0, int D, int64_t p
                       uint32_t* order, cudaStream_t st);
 int launch_pack_gather(const uint32_t* order, const double* params,
                        const double* z0v0, int D, int64_t PT, double* params_s,
-                       double* z0v0_s, cudaStream_t st);
+                       double* z0v0_s, const BoxDev* map, cudaStream_t st);
 int launch_pack_scatter(const uint32_t* order, const double* J_s, int64_t PT,
                         double* J, cudaStream_t st);
 int launch_philox(const uint32_t* ctr, int64_t n, uint32_t k0, uint32_t k1,

@@ -13,6 +13,8 @@
 // toolkit); the key kernel is ours.
 #include <cub/device/device_radix_sort.cuh>
 
+#include <string.h>
+
 #include "afm_internal.h"
 
 namespace afm {
@@ -42,9 +44,12 @@ __global__ void pack_key_kernel(const double* __restrict__ params,
   if (D > 0) {
     long long b = __double_as_longlong(params[gp * D + (D >= 2 ? 1 : 0)]);
     b ^= (b >> 63) & 0x7fffffffffffffffLL;              // monotone in the value
-    stiff = ((uint64_t)b ^ 0x8000000000000000ULL) >> 50;  // top 14 bits, unsigned
+    stiff = (uint64_t)b ^ 0x8000000000000000ULL;  // unsigned, monotone
   }
-  keys[gp] = ((uint64_t)(gp / per) << 28) | (stiff << 14) | (uint64_t)ph;
+  // a common start (z0v0 == nullptr, e.g. inside the PSO): no phase to order by,
+  // all 28 bits go to the stiffness parameter
+  const uint64_t low = z0v0 ? (((stiff >> 50) << 14) | (uint64_t)ph) : (stiff >> 36);
+  keys[gp] = ((uint64_t)(gp / per) << 28) | low;
   idx[gp] = (uint32_t)gp;
 }
 
@@ -80,15 +85,23 @@ int launch_pack_order(const double* params, const double* z0v0, int D, int64_t p
   return 1;
 }
 
+// With map_coords the inputs are PSO coordinates and the packed copy receives
+// the physical parameters (row a1 of SURVEY.md 8(a): theta_j = 10^x_j where the
+// coordinate is logarithmic), exactly as the integrate kernel's own prologue
+// computes them.
 __global__ void pack_gather_kernel(const uint32_t* __restrict__ order,
                                    const double* __restrict__ params,
                                    const double* __restrict__ z0v0, int D,
                                    int64_t PT, double* __restrict__ params_s,
-                                   double* __restrict__ z0v0_s) {
+                                   double* __restrict__ z0v0_s, int map_coords,
+                                   BoxDev box) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= PT) return;
   const int64_t gp = order[i];
-  for (int j = 0; j < D; ++j) params_s[i * D + j] = params[gp * D + j];
+  for (int j = 0; j < D; ++j) {
+    const double xv = params[gp * D + j];
+    params_s[i * D + j] = (map_coords && box.lg[j]) ? pow(10.0, xv) : xv;
+  }
   if (z0v0 != nullptr) {
     z0v0_s[2 * i] = z0v0[2 * gp];
     z0v0_s[2 * i + 1] = z0v0[2 * gp + 1];
@@ -104,10 +117,13 @@ __global__ void pack_scatter_kernel(const uint32_t* __restrict__ order,
 
 int launch_pack_gather(const uint32_t* order, const double* params,
                        const double* z0v0, int D, int64_t PT, double* params_s,
-                       double* z0v0_s, cudaStream_t st) {
+                       double* z0v0_s, const BoxDev* map, cudaStream_t st) {
   const int threads = 256;
+  BoxDev box;
+  memset(&box, 0, sizeof(box));
+  if (map) box = *map;
   pack_gather_kernel<<<(unsigned)((PT + threads - 1) / threads), threads, 0, st>>>(
-      order, params, z0v0, D, PT, params_s, z0v0_s);
+      order, params, z0v0, D, PT, params_s, z0v0_s, map ? 1 : 0, box);
   return 1;
 }
 
