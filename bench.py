@@ -47,11 +47,11 @@ FLOPS_PER_STEP = {wlm.LAW_DMT: 57.0, wlm.LAW_DMT_VISC: 57.0, wlm.LAW_LJ_EXP: 93.
 # FP64 FMA peak of the lane model: 148 SMs x 64 lanes x 2 flops x clock
 N_SM, FP64_LANES, FP32_LANES = 148, 64, 128
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the integrate kernel
-# on configs[1], from the ncu --set full captures in profiles/r1b_ncu.md (bytes),
-# and the pipe utilisation ncu measured in the same captures.
-NCU_TRAFFIC = {"f64": 3920640 + 0, "f32": 2991872 + 0}
-NCU_PIPE = {"f64": {"sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active": 59.63},
-            "f32": {"sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active": 47.92}}
+# on configs[1], from the ncu --set full captures in profiles/r1c_cfg1_packed.md
+# (bytes), and the pipe utilisation ncu measured in the same captures.
+NCU_TRAFFIC = {"f64": 3763200 + 0, "f32": 2942720 + 0}
+NCU_PIPE = {"f64": {"sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active": 59.26},
+            "f32": {"sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active": 48.22}}
 
 
 def _peaks():
@@ -302,7 +302,7 @@ def run_ours(args):
             "config": {"workload": "configs[1]: 65536 DMT theta x 200 cycles x 256 RK4 "
                                    "steps, misfit over last 100 cycles (per GPU)",
                        "particles_per_gpu": P, "rk4_steps": N, "window": wl["n_window"],
-                       "step": "afm_forward_batch + afm_pso_step",
+                       "step": "afm_forward_batch (with warp packing) + afm_pso_step",
                        "l2": "256 MB buffer zeroed between timed iterations"},
             "e2e": {"value": e2e_value, "unit": UNIT,
                     "h2d_bytes_per_step": int(hp.nbytes + ht.nbytes + hz.nbytes),
@@ -313,7 +313,7 @@ def run_ours(args):
             "roofline": {"bound": "alu", "kernel": "integrate_misfit_%s" % args.precision,
                          "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                          "frac": achieved / peak, "traffic": NCU_TRAFFIC[args.precision],
-                         "traffic_source": "profiles/r1b_ncu.md (ncu --set full, one launch)",
+                         "traffic_source": "profiles/r1c_cfg1_packed.md (ncu --set full, one launch)",
                          "algorithmic_bytes": int(P * (8 * D + 16 + 8) + N * 32),
                          "ncu_pipe_utilisation_pct": NCU_PIPE[args.precision],
                          "flops_per_particle_step": FLOPS_PER_STEP[wl["law"]],
