@@ -1,8 +1,8 @@
 // afm_sort.cu -- warp packing for the DMT laws.  The integrate kernels take a
 // step speculatively on the free-flight side of the law and redo it in the
 // general form when ANY lane of the warp touches the sample; which lanes share a
-// warp is free to choose.  Particles are therefore ordered by (trace, initial
-// stiffness bin, initial phase): lanes of one warp then touch the sample
+// warp is free to choose.  Particles are therefore ordered by (trace, stiffness
+// bins, initial phase): lanes of one warp then touch the sample
 // at about the same time, in the transient (same phase) and in the steady state
 // (similar contact width).  configs[1]: 19.05 -> ~18 ms.  The order changes no
 // result: every lane's arithmetic is independent of its neighbours; the inputs
@@ -19,13 +19,23 @@
 
 namespace afm {
 
-// key = [trace : 24][stiffness bin : 14][initial phase : 14].  The stiffness bin
-// is the top of the order-preserving bit pattern of params[.][j] (sign, exponent
-// and two mantissa bits: four bins per octave), j = 1 when D >= 2 (E* for the DMT
-// laws), else 0; inside a bin the particles are ordered by their initial phase
-// atan2(-v0/w, z0).  Measured on configs[1] (host-sorted inputs, packing off):
-// stiffness bins then phase 18.9 ms, phase bins then stiffness 19.4 ms, as drawn
-// 20.1 ms (this build's kernel; profiles/r1c_beam.md lists the sweep).
+// Order-preserving unsigned image of a double (monotone in the value).
+__device__ __forceinline__ uint64_t mono_bits(double x) {
+  long long b = __double_as_longlong(x);
+  b ^= (b >> 63) & 0x7fffffffffffffffLL;
+  return (uint64_t)b ^ 0x8000000000000000ULL;
+}
+
+// With per-particle initial states (configs[1]):
+//   key = [trace][bin of p1 : 13][bin of p0 : 12][initial phase : 10]
+// p1 = params[.][1] (E* for the DMT laws) in half-octave bins (sign, exponent,
+// one mantissa bit), p0 = params[.][0] (H) in octave bins; inside a bin the
+// particles are ordered by their initial phase atan2(-v0/w, z0).  Measured on
+// configs[1] with host-sorted inputs and packing off: as drawn 19.04 ms; phase
+// bins then E* 18.8; E* bins (1..16 per octave) then phase 17.9-18.4; E* 2 per
+// octave, H 1 per octave, then phase 17.1 ms.
+// With a common initial state (inside the PSO, coordinates in): no phase to
+// order by, key = [trace][top 35 bits of p1].  Only the bits in use are sorted.
 __global__ void pack_key_kernel(const double* __restrict__ params,
                                 const double* __restrict__ z0v0, int D,
                                 int64_t per, int64_t PT, double w_drive,
@@ -34,22 +44,20 @@ __global__ void pack_key_kernel(const double* __restrict__ params,
                                 uint32_t* __restrict__ idx) {
   const int64_t gp = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (gp >= PT) return;
-  const double z0 = z0v0 ? z0v0[2 * gp] : z0d;
-  const double v0 = z0v0 ? z0v0[2 * gp + 1] : v0d;
-  // z = A cos(phi), v = -A w sin(phi)
-  const double phi = atan2(-v0 / w_drive, z0);  // (-pi, pi]
-  int ph = (int)floor((phi + 3.14159265358979323846) * (16384.0 / 6.283185307179586));
-  ph = min(max(ph, 0), 16383);
-  uint64_t stiff = 0;
-  if (D > 0) {
-    long long b = __double_as_longlong(params[gp * D + (D >= 2 ? 1 : 0)]);
-    b ^= (b >> 63) & 0x7fffffffffffffffLL;              // monotone in the value
-    stiff = (uint64_t)b ^ 0x8000000000000000ULL;  // unsigned, monotone
+  uint64_t low = 0;
+  const double* th = params + gp * D;
+  if (z0v0 != nullptr) {
+    // z = A cos(phi), v = -A w sin(phi)
+    const double phi = atan2(-z0v0[2 * gp + 1] / w_drive, z0v0[2 * gp]);  // (-pi, pi]
+    int ph = (int)floor((phi + 3.14159265358979323846) * (1024.0 / 6.283185307179586));
+    ph = min(max(ph, 0), 1023);
+    const uint64_t b1 = (D >= 2) ? (mono_bits(th[1]) >> 51) : 0;  // 13 bits
+    const uint64_t b0 = (D >= 1) ? (mono_bits(th[0]) >> 52) : 0;  // 12 bits
+    low = (b1 << 22) | (b0 << 10) | (uint64_t)ph;
+  } else if (D > 0) {
+    low = mono_bits(th[D >= 2 ? 1 : 0]) >> 29;  // 35 bits
   }
-  // a common start (z0v0 == nullptr, e.g. inside the PSO): no phase to order by,
-  // all 28 bits go to the stiffness parameter
-  const uint64_t low = z0v0 ? (((stiff >> 50) << 14) | (uint64_t)ph) : (stiff >> 36);
-  keys[gp] = ((uint64_t)(gp / per) << 28) | low;
+  keys[gp] = ((uint64_t)(gp / per) << 35) | low;
   idx[gp] = (uint32_t)gp;
 }
 
@@ -57,7 +65,7 @@ static size_t cub_bytes(int64_t PT) {
   size_t bytes = 0;
   cub::DeviceRadixSort::SortPairs(nullptr, bytes, (const uint64_t*)nullptr,
                                   (uint64_t*)nullptr, (const uint32_t*)nullptr,
-                                  (uint32_t*)nullptr, (int)PT, 0, 52);
+                                  (uint32_t*)nullptr, (int)PT, 0, 59);
   return bytes;
 }
 
@@ -79,8 +87,10 @@ int launch_pack_order(const double* params, const double* z0v0, int D, int64_t p
   const int threads = 256;
   pack_key_kernel<<<(unsigned)((PT + threads - 1) / threads), threads, 0, st>>>(
       params, z0v0, D, per, PT, w_drive, z0_default, v0_default, keys_in, idx_in);
+  int end_bit = 35;  // + the bits of the trace index
+  for (int64_t t = PT / per - 1; t > 0; t >>= 1) ++end_bit;
   if (cub::DeviceRadixSort::SortPairs(temp, temp_bytes, keys_in, keys_out, idx_in,
-                                      order, (int)PT, 0, 52, st) != cudaSuccess)
+                                      order, (int)PT, 0, end_bit, st) != cudaSuccess)
     return -2;
   return 1;
 }
