@@ -331,7 +331,9 @@ void afm_reset_launch_count(void);
  * kernel: 32, 64 or 128; 0 = auto), "tile" (steps per time tile; 0 = auto),
  * "ppt" (particles per thread: 1 or 2; 0 = auto), "form" (FP64 kernel form:
  * 1 = throughput, fewest FP64 instructions; 2 = latency, shortest dependent
- * chains; 0 = auto by warps per SM sub-partition), "pack" (order the particles
+ * chains; 0 = auto by warps per SM sub-partition), "lanes" (latency form of the
+ * DMT laws: particles per warp, a power of two up to 32; 0 = auto, as many as
+ * spread the batch over all SM sub-partitions), "pack" (order the particles
  * of a DMT-law batch by trace, initial phase and stiffness so that the lanes of a
  * warp touch the sample together: 1 = never, 2 = always, 0 = auto in the
  * throughput regime; results do not depend on it).

@@ -54,6 +54,7 @@ int g_opt_block = 0;  // 0 = auto
 int g_opt_tile = 0;   // 0 = auto
 int g_opt_ppt = 0;    // 0 = auto
 int g_opt_form = 0;   // 0 = auto, 1 = throughput form, 2 = latency form
+int g_opt_lanes = 0;  // 0 = auto; latency form: particles per warp
 int g_opt_pack = 0;   // 0 = auto, 1 = never, 2 = always (DMT laws only)
 int g_n_sm = 148;
 
@@ -341,6 +342,26 @@ int pack_inputs(const afm_cfg* cfg, const double* params, const double* z0v0,
   return AFM_OK;
 }
 
+// Latency form: particles per warp, so that the warps spread over all SM
+// sub-partitions (DMT laws; the other laws have no warp-wide mode to protect).
+int pick_lanes(const afm_cfg* cfg, int64_t per, int n_traces) {
+  if (g_opt_lanes > 0) return g_opt_lanes;
+  const bool dmt = (cfg->law == AFM_LAW_DMT || cfg->law == AFM_LAW_DMT_VISC);
+  if (!dmt) return 32;
+  // fewest particles per warp that still leaves at most one warp per SM
+  // sub-partition (two warps sharing a dispatch port cost more than they save:
+  // configs[2] 745 ms at 2 per warp, 898 ms at 1 per warp)
+  int lanes = 1;
+  while (lanes < 32 && ((per + lanes - 1) / lanes) * n_traces > (int64_t)4 * g_n_sm)
+    lanes *= 2;
+  return lanes;
+}
+
+// CTAs per trace of the FP64 integrate kernel for a launch decision.
+int integrate_bpt(int64_t per, int block, int ppt, int variant, int lanes) {
+  return variant == 1 ? blocks_per_trace(per, lanes) : blocks_per_trace(per, block * ppt);
+}
+
 BoxDev make_box(const afm_bounds* b, int D) {
   BoxDev bd;
   memset(&bd, 0, sizeof(bd));
@@ -403,6 +424,7 @@ int forward_locked(const double* params, int64_t P, const double* trace,
   io.per = per;
   io.n_traces = cfg->n_traces;
   io.mode = 0;
+  io.lanes = pick_lanes(cfg, per, cfg->n_traces);
   Packed pk;
   if ((rc = pack_inputs(cfg, params, z0v0, per, cfg->n_traces, nullptr, &pk, st)))
     return rc;
@@ -561,7 +583,9 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
   const int64_t PT = per * T;
   const int block = pick_block(per, T);
   const int ppt = pick_ppt(per, T);
-  const int bpt = blocks_per_trace(per, block * ppt);
+  const int lanes = pick_lanes(cfg, per, T);
+  const int bpt = f32 ? blocks_per_trace(per, block * ppt)
+                      : integrate_bpt(per, block, ppt, pick_variant(per, T, ppt), lanes);
   ModelConsts mc;
   ModelConstsF32 mf;
   make_consts(cfg, block, &mc);
@@ -609,6 +633,7 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
   io.per = per;
   io.n_traces = T;
   io.mode = 1;
+  io.lanes = lanes;
 
   int done = 0;
   for (int it = 0; it < swarm->n_iters; ++it) {
@@ -740,7 +765,9 @@ int afm_pso_shard_eval(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   const int64_t per = swarm->n_particles;
   const int block = pick_block(per, T);
   const int ppt = pick_ppt(per, T);
-  const int bpt = blocks_per_trace(per, block * ppt);
+  const int lanes = pick_lanes(cfg, per, T);
+  const int bpt = f32 ? blocks_per_trace(per, block * ppt)
+                      : integrate_bpt(per, block, ppt, pick_variant(per, T, ppt), lanes);
   ModelConsts mc;
   ModelConstsF32 mf;
   make_consts(cfg, block, &mc);
@@ -765,6 +792,7 @@ int afm_pso_shard_eval(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   io.per = per;
   io.n_traces = T;
   io.mode = 1;
+  io.lanes = lanes;
   if (f32)
     LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
   else
@@ -1184,6 +1212,13 @@ int afm_set_option(const char* name, int64_t value) {
   if (!strcmp(name, "form")) {
     if (value < 0 || value > 2) return fail(AFM_EINVAL, "form must be 0, 1 or 2");
     g_opt_form = (int)value;
+    return AFM_OK;
+  }
+  if (!strcmp(name, "lanes")) {
+    if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8 &&
+        value != 16 && value != 32)
+      return fail(AFM_EINVAL, "lanes must be 0 or a power of two up to 32");
+    g_opt_lanes = (int)value;
     return AFM_OK;
   }
   if (!strcmp(name, "pack")) {

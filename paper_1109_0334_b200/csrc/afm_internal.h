@@ -118,6 +118,8 @@ struct IntegrateIO {
   int64_t per;            // particles per trace
   int32_t n_traces;
   int32_t mode;           // 0 forward, 1 PSO
+  int32_t lanes;          // latency form: particles per warp (power of two, 1..32)
+  int32_t pad_;
 };
 
 int blocks_per_trace(int64_t per, int block);

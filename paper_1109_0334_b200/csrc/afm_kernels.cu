@@ -154,14 +154,19 @@ __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
 
   const int tid = threadIdx.x;
   const int s = blockIdx.x / blocks_per_tr;  // trace (segment) of this CTA
+  // Latency form: only io.lanes lanes of the (single) warp carry particles, the
+  // others shadow them.  With one warp or less per SM sub-partition nothing is
+  // gained by filling warps, and a warp of few particles leaves the free-flight
+  // form only when ITS particles touch the sample, not when any of 32 does.
   const int64_t base =
-      (int64_t)(blockIdx.x - s * blocks_per_tr) * blockDim.x * PPT + tid;
+      LAT ? (int64_t)(blockIdx.x - s * blocks_per_tr) * io.lanes + (tid & (io.lanes - 1))
+          : (int64_t)(blockIdx.x - s * blocks_per_tr) * blockDim.x * PPT + tid;
   bool active[PPT];
   int64_t gp[PPT];
 #pragma unroll
   for (int q = 0; q < PPT; ++q) {
     const int64_t li = base + (int64_t)q * blockDim.x;
-    active[q] = li < io.per;
+    active[q] = (li < io.per) && (!LAT || tid < io.lanes);
     // an inactive slot of a ragged last CTA integrates a copy of the segment's
     // last particle (keeps every vote and barrier uniform) and writes nothing
     gp[q] = (int64_t)s * io.per + (active[q] ? li : io.per - 1);
@@ -571,7 +576,9 @@ int launch_build_stream(const ModelConsts& mc, const double* trace, int n_traces
 template <int LAW, int MODE, int PPT, bool LAT>
 static int launch_integrate_t(const ModelConsts& mc, const IntegrateIO& io,
                               int block, cudaStream_t st) {
-  const int bpt = blocks_per_trace(io.per, block * PPT);
+  const int bpt = LAT ? blocks_per_trace(io.per, io.lanes)
+                      : blocks_per_trace(io.per, block * PPT);
+  if (LAT) block = 32;  // one warp per CTA
   const unsigned grid = (unsigned)(bpt * io.n_traces);
   const size_t smem = (size_t)mc.T * 32 * 2 + 64;  // + barriers + over-read pad
   auto kern = integrate_misfit_f64<LAW, MODE, PPT, LAT>;

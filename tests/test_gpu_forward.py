@@ -290,3 +290,30 @@ def test_warp_packing_changes_no_result(afm, precision):
     if precision == 0:
         Jo = _oracle_forward(wl, params, trace, z0v0)
         assert rel_err(out[2], Jo).max() < TOL_F64
+
+
+@pytest.mark.parametrize("lanes", [1, 2, 8, 32])
+def test_latency_form_lanes_per_warp(afm, lanes):
+    """Latency form with 1..32 particles per warp (the other lanes shadow them):
+    bit-identical misfits and swarm, ragged counts included."""
+    import torch
+    wl = wlm.scaled(wlm.config(2), n_cycles=10, n_skip_cycles=5, n_particles=77, n_iters=4)
+    trace = oracle_trace(wl)
+    params = wlm.draw_params(wl, 77, seed=61)
+    out = {}
+    for l in (32, lanes):
+        afm.afm_set_option("lanes", l)
+        afm.afm_set_option("form", 2)
+        try:
+            J = _gpu_forward(afm, wl, params, trace)
+            g = afm.afm_pso_invert(afm.bounds_from(wl), afm.swarm_from(wl), 0,
+                                   torch.as_tensor(trace, device="cuda"), afm.cfg_from(wl),
+                                   dump=True)
+            out[l] = (J, g["dump"].cpu().numpy(), g["theta_star"])
+        finally:
+            afm.afm_set_option("lanes", 0)
+            afm.afm_set_option("form", 0)
+    assert np.array_equal(out[32][0], out[lanes][0])
+    assert np.array_equal(out[32][1], out[lanes][1])
+    assert np.array_equal(out[32][2], out[lanes][2])
+    assert rel_err(out[lanes][0], _oracle_forward(wl, params, trace)).max() < TOL_F64
