@@ -49,9 +49,9 @@ N_SM, FP64_LANES, FP32_LANES = 148, 64, 128
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the integrate kernel
 # on configs[1], from the ncu --set full captures in profiles/r1c_cfg1_packed.md
 # (bytes), and the pipe utilisation ncu measured in the same captures.
-NCU_TRAFFIC = {"f64": 3763200 + 0, "f32": 2942720 + 0}
-NCU_PIPE = {"f64": {"sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active": 59.26},
-            "f32": {"sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active": 48.22}}
+NCU_TRAFFIC = {"f64": 3762688 + 0, "f32": 2942720 + 0}
+NCU_PIPE = {"f64": {"sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active": 58.63},
+            "f32": {"sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active": 48.63}}
 
 
 def _peaks():
