@@ -112,3 +112,39 @@ def test_product_package_never_imports_the_oracle():
                 if f.endswith((".py", ".cu", ".cuh", ".h")):
                     text = open(os.path.join(dirpath, f)).read()
                     assert not pat.search(text), (f, pat.search(text).group(0))
+
+
+def test_new_entry_points_validate_before_touching_the_device(lib):
+    """Beam model, sharded swarm, probes, options: bad arguments are AFM_EINVAL
+    without any CUDA call (this runs on a box with no GPU)."""
+    wl = wlm.beam_workload()
+    p16 = C.c_void_p(16)
+    for field, val in (("n_modes", 3), ("n_points", 500), ("n_points", 1), ("Q", 0.0),
+                       ("n_params", 3), ("law", 9), ("n_skip_cycles", 80), ("n_traces", 0),
+                       ("L", -1.0), ("A_ref", 0.0)):
+        cfg = afm.beam_cfg_from(wl, **{field: val})
+        rc = lib.afm_beam_forward_batch(p16, 4, p16, C.byref(cfg), None, p16, None)
+        assert rc == afm.EINVAL, (field, val)
+        assert lib.afm_beam_modes(C.byref(cfg), None, None, None, None, None, None) == afm.EINVAL
+        assert lib.afm_beam_trajectory(p16, C.byref(cfg), None, None, None) == afm.EINVAL
+    cfg = afm.beam_cfg_from(wl)
+    assert lib.afm_beam_forward_batch(p16, 3, p16, C.byref(afm.beam_cfg_from(wl, n_traces=2)),
+                                      None, p16, None) == afm.EINVAL
+    assert lib.afm_beam_forward_batch(None, 4, p16, C.byref(cfg), None, p16, None) == afm.EINVAL
+    w0 = wlm.config(0)
+    b, sw, c0 = afm.bounds_from(w0), afm.swarm_from(w0), afm.cfg_from(w0)
+    assert lib.afm_pso_shard_init(C.byref(b), C.byref(sw), 2, 1, 0, -1, p16, p16, p16, p16,
+                                  p16, p16, None) == afm.EINVAL
+    assert lib.afm_pso_shard_eval(C.byref(b), C.byref(sw), p16, C.byref(c0), -5, p16, p16,
+                                  p16, p16, p16, None) == afm.EINVAL
+    assert lib.afm_pso_shard_move(C.byref(b), C.byref(sw), 2, 1, 0, 0, 1, 0, p16, 0, p16, p16,
+                                  p16, p16, p16, None, None, None) == afm.EINVAL
+    out = C.c_double(0.0)
+    assert lib.afm_fma_peak(7, 0.1, C.byref(out), None) == afm.EINVAL
+    assert lib.afm_fma_peak(0, 100.0, C.byref(out), None) == afm.EINVAL
+    assert lib.afm_dispatch_probe(9, 1, C.byref(out), None) == afm.EINVAL
+    assert lib.afm_dispatch_probe(0, 0, C.byref(out), None) == afm.EINVAL
+    for name, bad in (("form", 3), ("lanes", 3), ("pack", 5), ("ppt", 4), ("tile", -1)):
+        with pytest.raises(afm.AfmError):
+            afm.afm_set_option(name, bad)
+        assert afm.afm_set_option(name, 0) is None
