@@ -431,6 +431,21 @@ def extras(afm, torch, dev, main_prec):
             ex["cfg2_batches_to_cutoff"] = int(r["n_iters_done"])
             ex["cfg2_cutoff_theta_star_rel_err_vs_truth"] = [
                 float(abs(a - t) / abs(t)) for a, t in zip(r["theta_star"][0], wl["truth"])]
+            # the same inversion with a swarm that fills the machine: 1 024 particles
+            # are 32 warps on 592 SM sub-partitions, and a batch of 16 384 takes the
+            # same time (the time loop is a latency chain), so the swarm can be 16x
+            # wider for free and needs far fewer batches
+            for tag, kw in (("to_cutoff", dict(j_target=jt, n_particles=16384)),
+                            ("30_batches", dict(n_particles=16384, n_iters=30))):
+                sc = afm.swarm_from(wl, **kw)
+                afm.afm_pso_invert(b, sc, wl["pso_seed"], trace, cfg)
+                t0 = time.perf_counter()
+                r = afm.afm_pso_invert(b, sc, wl["pso_seed"], trace, cfg)
+                ex["cfg2_wide16384_%s_ms" % tag] = (time.perf_counter() - t0) * 1e3
+                ex["cfg2_wide16384_%s_batches" % tag] = int(r["n_iters_done"])
+                ex["cfg2_wide16384_%s_theta_star_rel_err_vs_truth" % tag] = [
+                    float(abs(a - t) / abs(t))
+                    for a, t in zip(r["theta_star"][0], wl["truth"])]
     return ex
 
 
