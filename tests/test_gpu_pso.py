@@ -174,3 +174,14 @@ def test_pso_step_on_supplied_misfits(afm):
         assert np.array_equal(st["pbestJ"].cpu().numpy(), o["dump"][it, :, 10]), it
         assert np.array_equal(st["gbest"].cpu().numpy()[0], o["gbest_hist"][it, 0, :3]), it
         assert st["gbestJ"].cpu().numpy()[0] == o["gbest_hist"][it, 0, 3]
+
+
+@pytest.mark.parametrize("per,T", [(1, 9), (33, 7), (1, 1)])
+def test_degenerate_swarm_shapes(afm, per, T):
+    """One particle per swarm, ragged swarms over several traces, a single particle
+    in total: the swarm still replays the oracle."""
+    wl = wlm.scaled(wlm.config(4), n_cycles=6, n_skip_cycles=3, n_traces=T, n_particles=per,
+                    n_iters=4)
+    trace = oracle_trace(wl, truths=wlm.pixel_truths(wl))
+    g, o = _both(afm, wl, trace)
+    _compare_runs(g, o, wl["n_params"])
