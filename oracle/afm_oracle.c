@@ -409,11 +409,27 @@ void orc_pso_core(orc_eval_fn eval, const void* ctx, int64_t W, int32_t D,
       double r1[4], r2[4];
       s = (int32_t)(gp / P);
       orc_pso_uniforms(seed, (uint64_t)gp, (uint32_t)it, 1u, D, r1, r2);
+      const double* social = gbest + s * D;
+      if (Sw->topology == 1) {
+        /* ring of three inside the swarm of trace s */
+        int64_t p = gp - (int64_t)s * P;
+        int64_t cand[3], best, c;
+        cand[0] = (p + P - 1) % P;
+        cand[1] = p;
+        cand[2] = (p + 1) % P;
+        best = cand[0];
+        for (c = 1; c < 3; ++c) {
+          double Jc = pbestJ[(int64_t)s * P + cand[c]];
+          double Jb = pbestJ[(int64_t)s * P + best];
+          if (Jc < Jb || (Jc == Jb && cand[c] < best)) best = cand[c];
+        }
+        social = pbest + ((int64_t)s * P + best) * D;
+      }
       for (j = 0; j < D; ++j) {
         double xi = x[gp * D + j];
         double vi = Sw->w * vel[gp * D + j] +
                     Sw->c1 * r1[j] * (pbest[gp * D + j] - xi) +
-                    Sw->c2 * r2[j] * (gbest[s * D + j] - xi);
+                    Sw->c2 * r2[j] * (social[j] - xi);
         xi = xi + vi;
         if (xi < B->lo[j]) {
           xi = B->lo[j];

@@ -85,6 +85,12 @@ typedef struct {
   int32_t n_particles; /* per trace                                          */
   int32_t n_iters;     /* number of forward batches (iteration 0 = x0)       */
   double w, c1, c2;    /* Eq. 8 weights                                      */
+  int32_t topology;    /* 0: global best (the paper's "g_b");
+                          1: ring of three (R23): the social attractor
+                          of particle p is the best personal best among
+                          p-1, p, p+1 (indices wrap inside the swarm; lowest
+                          index among equal minima)                          */
+  int32_t pad_;
 } orc_swarm;
 
 void   orc_constants(const orc_model* M, orc_consts* C);

@@ -38,7 +38,8 @@ class Box(C.Structure):
 
 class Swarm(C.Structure):
     _fields_ = [("n_particles", C.c_int32), ("n_iters", C.c_int32),
-                ("w", C.c_double), ("c1", C.c_double), ("c2", C.c_double)]
+                ("w", C.c_double), ("c1", C.c_double), ("c2", C.c_double),
+                ("topology", C.c_int32), ("pad_", C.c_int32)]
 
 
 class Beam(C.Structure):
@@ -158,11 +159,12 @@ def box_from(wl):
     return b
 
 
-def swarm_from(wl, n_particles=None, n_iters=None):
+def swarm_from(wl, n_particles=None, n_iters=None, topology=None):
     s = wl["swarm"]
     return Swarm(n_particles=s["n_particles"] if n_particles is None else n_particles,
                  n_iters=s["n_iters"] if n_iters is None else n_iters,
-                 w=s["w"], c1=s["c1"], c2=s["c2"])
+                 w=s["w"], c1=s["c1"], c2=s["c2"],
+                 topology=s.get("topology", 0) if topology is None else topology, pad_=0)
 
 
 # ---- thin calls -------------------------------------------------------------

@@ -154,3 +154,36 @@ def test_pso_recovers_ground_truth_from_noise_free_trace():
     rel = np.abs(out["theta_star"][0] / np.array(wl["truth"]) - 1.0)
     assert np.all(rel < 1e-3), (out["theta_star"], rel)
     assert out["J_star"][0] < 1e-6 * np.sum(clean ** 2)
+
+
+def test_ring_topology_by_hand_replay():
+    """topology = 1 (R23): the social attractor of
+    particle p is the best personal best among p-1, p, p+1 (wrapping inside the
+    swarm, lowest index among equal minima).  Replayed here in numpy from the
+    oracle's own dump: same uniforms, same Eq. 8, only the attractor differs;
+    the reported result is still the best over the whole swarm."""
+    wl = wlm.scaled(wlm.config(0), n_cycles=6, n_skip_cycles=3, n_particles=9, n_iters=5)
+    M = orc.model_from(wl)
+    bad, win = orc.window(M, wl["truth"], wl["z0"], wl["v0"])
+    sw = orc.swarm_from(wl, topology=1)
+    o = orc.pso_invert(M, orc.box_from(wl), sw, 3, win[None, :], wl["z0"], wl["v0"], dump=True)
+    g = orc.pso_invert(M, orc.box_from(wl), orc.swarm_from(wl), 3, win[None, :], wl["z0"],
+                       wl["v0"], dump=True)
+    d, D, P = o["dump"], 2, 9
+    lo, hi = np.array(wl["bounds"]["lo"]), np.array(wl["bounds"]["hi"])
+    assert np.array_equal(d[0], g["dump"][0])           # same start, same first batch
+    assert not np.array_equal(d[2], g["dump"][2])       # another swarm afterwards
+    for it in range(4):
+        x, v, pb, pbJ = d[it, :, 0:2], d[it, :, 2:4], d[it, :, 4:6], d[it, :, 7]
+        for p in range(P):
+            cand = [(p - 1) % P, p, (p + 1) % P]
+            best = min(cand, key=lambda c: (pbJ[c], c))
+            r1, r2 = orc.pso_uniforms(3, p, it, 1, D)
+            vn = sw.w * v[p] + sw.c1 * r1 * (pb[p] - x[p]) + sw.c2 * r2 * (pb[best] - x[p])
+            xn = x[p] + vn
+            low, high = xn < lo, xn > hi
+            xn = np.where(low, lo, np.where(high, hi, xn))
+            vn = np.where(low | high, 0.0, vn)
+            assert np.array_equal(d[it + 1, p, 0:2], xn), (it, p)
+            assert np.array_equal(d[it + 1, p, 2:4], vn), (it, p)
+    assert o["J_star"][0] == d[:, :, 6].min()
