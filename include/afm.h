@@ -126,6 +126,13 @@ typedef struct {
   int32_t n_iters;
   double w, c1, c2;
   double j_target;
+  int32_t topology;   /* 0: global best (the paper's g_b);
+                         1: ring of three (R23): the social attractor
+                         of particle p is the best personal best among p-1, p,
+                         p+1, wrapping inside the swarm, lowest index among
+                         equal minima.  theta*, J* are the swarm's best either
+                         way.  Not available for a sharded swarm. */
+  int32_t reserved_;  /* must be 0 */
 } afm_swarm_cfg;
 
 /* ---- forward problem + cost (Eq. 5) -------------

@@ -85,7 +85,8 @@ class Bounds(C.Structure):
 class SwarmCfg(C.Structure):
     _fields_ = [("n_particles", C.c_int32), ("n_iters", C.c_int32),
                 ("w", C.c_double), ("c1", C.c_double), ("c2", C.c_double),
-                ("j_target", C.c_double)]
+                ("j_target", C.c_double), ("topology", C.c_int32),
+                ("reserved_", C.c_int32)]
 
 
 _lib = None
@@ -187,7 +188,8 @@ def bounds_from(wl):
 def swarm_from(wl, j_target=0.0, **over):
     s = wl["swarm"]
     sc = SwarmCfg(n_particles=s["n_particles"], n_iters=s["n_iters"], w=s["w"],
-                  c1=s["c1"], c2=s["c2"], j_target=j_target)
+                  c1=s["c1"], c2=s["c2"], j_target=j_target,
+                  topology=s.get("topology", 0), reserved_=0)
     for k, v in over.items():
         setattr(sc, k, v)
     return sc

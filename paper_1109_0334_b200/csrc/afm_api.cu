@@ -388,6 +388,9 @@ int validate_swarm(const afm_swarm_cfg* s) {
     return fail(AFM_EINVAL, "n_particles and n_iters must be >= 1");
   if (!isfinite(s->w) || !isfinite(s->c1) || !isfinite(s->c2))
     return fail(AFM_EINVAL, "w, c1, c2 must be finite");
+  if (s->topology != 0 && s->topology != 1)
+    return fail(AFM_EINVAL, "topology must be 0 (global best) or 1 (ring of three)");
+  if (s->reserved_ != 0) return fail(AFM_EINVAL, "swarm reserved_ must be 0");
   return AFM_OK;
 }
 
@@ -558,7 +561,7 @@ int afm_pso_step(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   if (g_ws.cand.ensure((size_t)bpt * n_traces * sizeof(Cand)))
     return fail(AFM_ECUDA, "cudaMalloc of candidates failed");
   BoxDev box = make_box(bounds, n_dims);
-  SwarmDev sw = {swarm->w, swarm->c1, swarm->c2};
+  SwarmDev sw = {swarm->w, swarm->c1, swarm->c2, swarm->topology, 0};
   LAUNCHED(launch_pso_best(n_dims, per, n_traces, J, x, pbest, pbestJ,
                            (Cand*)g_ws.cand.p, block, st));
   LAUNCHED(launch_pso_gbest(box, n_dims, n_traces, bpt, (Cand*)g_ws.cand.p,
@@ -612,7 +615,7 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
   if ((rc = ensure_pinned((size_t)T * 8))) return rc;
 
   BoxDev box = make_box(bounds, D);
-  SwarmDev sw = {swarm->w, swarm->c1, swarm->c2};
+  SwarmDev sw = {swarm->w, swarm->c1, swarm->c2, swarm->topology, 0};
 
   if (f32)
     LAUNCHED(launch_build_stream_f32(mf, trace, T, (float*)g_ws.stream.p, st));
@@ -817,12 +820,16 @@ int afm_pso_shard_move(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   int rc = validate_bounds(bounds, n_dims);
   if (rc) return rc;
   if ((rc = validate_swarm(swarm))) return rc;
+  if (swarm->topology != 0)
+    return fail(AFM_EUNSUPPORTED,
+                "the ring topology needs its neighbours' personal bests: not "
+                "available for a sharded swarm");
   if (!gathered || !x || !v || !pbest || !gbest || !gbestJ)
     return fail(AFM_EINVAL, "NULL swarm array");
   if ((rc = check_device())) return rc;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   BoxDev box = make_box(bounds, n_dims);
-  SwarmDev sw = {swarm->w, swarm->c1, swarm->c2};
+  SwarmDev sw = {swarm->w, swarm->c1, swarm->c2, swarm->topology, 0};
   LAUNCHED(launch_pso_shard_gbest(box, n_dims, n_traces, n_ranks, gathered, gbest,
                                   gbestJ, theta_star, J_star, st));
   if (do_move)
@@ -1017,7 +1024,7 @@ int afm_beam_pso_invert(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   double* Js_dev = th_dev + (size_t)T * D;
   if ((rc = ensure_pinned((size_t)T * 8))) return rc;
   BoxDev box = make_box(bounds, D);
-  SwarmDev sw = {swarm->w, swarm->c1, swarm->c2};
+  SwarmDev sw = {swarm->w, swarm->c1, swarm->c2, swarm->topology, 0};
   LAUNCHED(launch_pso_init(box, D, per, T, seed, 0, x, v, pbest, pbestJ, gbest,
                            gbestJ, st));
   IntegrateIO io;

@@ -92,6 +92,8 @@ struct BoxDev {
 
 struct SwarmDev {
   double w, c1, c2;
+  int32_t topology;  // 0 global best, 1 ring of three
+  int32_t pad_;
 };
 
 // One block-level (pbestJ, particle index) candidate of the global-best search.

@@ -531,10 +531,26 @@ __global__ void pso_move_kernel(BoxDev box, SwarmDev sw, int D, int64_t per,
   if (!do_move) return;
   double r1[4], r2[4];
   pso_uniforms(seed, (uint64_t)(first + gp), it, 1u, D, r1, r2);
+  // social attractor: the swarm's best, or (ring of three, R23) the best
+  // personal best among p-1, p, p+1 inside the swarm of trace s
+  const double* social = gbest + s * D;
+  if (sw.topology == 1) {
+    const int64_t p = gp - s * per;
+    const int64_t c0 = (p + per - 1) % per, c2 = (p + 1) % per;
+    int64_t best = c0;
+    double Jb = pbestJ[s * per + c0];
+    const double J1 = pbestJ[gp], J2 = pbestJ[s * per + c2];
+    if (J1 < Jb || (J1 == Jb && p < best)) {
+      best = p;
+      Jb = J1;
+    }
+    if (J2 < Jb || (J2 == Jb && c2 < best)) best = c2;
+    social = pbest + (s * per + best) * D;
+  }
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
     if (j < D) {
-      const double gb = gbest[s * D + j];
+      const double gb = social[j];
       const double t0 = __dmul_rn(sw.w, vi[j]);
       const double t1 =
           __dmul_rn(__dmul_rn(sw.c1, r1[j]), __dsub_rn(pb[j], xi[j]));

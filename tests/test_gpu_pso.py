@@ -185,3 +185,22 @@ def test_degenerate_swarm_shapes(afm, per, T):
     trace = oracle_trace(wl, truths=wlm.pixel_truths(wl))
     g, o = _both(afm, wl, trace)
     _compare_runs(g, o, wl["n_params"])
+
+
+@pytest.mark.parametrize("cfg_i,T", [(2, 1), (4, 3)])
+def test_ring_topology_replays_the_oracle(afm, cfg_i, T):
+    """topology = 1 (ring of three, R23): same dump as the oracle's ring swarm, and
+    a different swarm from the global-best one."""
+    over = dict(n_cycles=8, n_skip_cycles=4, n_particles=45, n_iters=6)
+    if cfg_i == 4:
+        over["n_traces"] = T
+    wl = wlm.scaled(wlm.config(cfg_i), **over)
+    wl["swarm"]["topology"] = 1
+    truths = None if wl["truth"] is not None else wlm.pixel_truths(wl)
+    trace = oracle_trace(wl, truths=truths)
+    g, o = _both(afm, wl, trace)
+    _compare_runs(g, o, wl["n_params"])
+    wl0 = wlm.scaled(wl)
+    wl0["swarm"]["topology"] = 0
+    g0, _ = _both(afm, wl0, trace)
+    assert not np.array_equal(g0["dump"].cpu().numpy()[3], g["dump"].cpu().numpy()[3])
