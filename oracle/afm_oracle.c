@@ -320,99 +320,42 @@ void orc_theta_of_x(const orc_box* B, int32_t D, const double* x,
  *   up to and including batch i;
  *   n_iters forward batches; the result is the global best after the last.
  * Each trace (pixel) owns an independent swarm of n_particles.
+ *
+ * Cost cutoff (R24; "generations to convergence", 236
+ * "convergence cutoff", 264 "cutoff convergence threshold of J_L2"): with
+ * j_target > 0 the run ends after the first batch at which every trace's
+ * global-best J is <= j_target; that batch is not followed by a move.  The
+ * return value is the number of batches run.
+ *
+ * Asynchronous swarm (R25; the paper is silent): with
+ * 0 < async_chunk = B < n_particles the particles of every swarm are taken in
+ * chunks [c, c + B) in index order.  A chunk is evaluated, its personal bests
+ * and the swarm's best are updated from it, and it moves at once (Eq. 8 with
+ * the best known at that moment; same random numbers as the synchronous
+ * swarm), so later chunks of the same batch see what earlier chunks found.
+ * The chunks of the last batch (n_iters reached) do not move; the cutoff is
+ * still tested once per batch, after its last chunk.  B >= n_particles or 0 is
+ * the synchronous swarm: the whole swarm is one chunk and moves after the
+ * cutoff test.
  * ---------------------------------------------------------------------- */
-void orc_pso_core(orc_eval_fn eval, const void* ctx, int64_t W, int32_t D,
-                  const orc_box* B, const orc_swarm* Sw, uint64_t seed,
-                  const double* trace, int32_t n_traces, double* theta_star,
-                  double* J_star, double* dump, double* gbest_hist) {
+
+/* Eq. 8 + position update + bound rule for particles [p0, p1) of every swarm. */
+static void pso_move_range(int32_t D, const orc_box* B, const orc_swarm* Sw,
+                           uint64_t seed, int32_t it, int32_t n_traces,
+                           int64_t p0, int64_t p1, double* x, double* vel,
+                           const double* pbest, const double* pbestJ,
+                           const double* gbest) {
   const int64_t P = Sw->n_particles;
-  const int64_t PT = P * (int64_t)n_traces;
-  const int64_t rec = 3 * D + 2;
-  double* x = (double*)malloc((size_t)(PT * D) * sizeof(double));
-  double* vel = (double*)malloc((size_t)(PT * D) * sizeof(double));
-  double* pbest = (double*)malloc((size_t)(PT * D) * sizeof(double));
-  double* pbestJ = (double*)malloc((size_t)PT * sizeof(double));
-  double* J = (double*)malloc((size_t)PT * sizeof(double));
-  double* gbest = (double*)malloc((size_t)(n_traces * D) * sizeof(double));
-  double* gbestJ = (double*)malloc((size_t)n_traces * sizeof(double));
-  int64_t gp;
-  int32_t it, j, s;
-
-  /* initialisation: uniform positions and velocities in the search space */
-  for (gp = 0; gp < PT; ++gp) {
-    double a[4], b[4];
-    orc_pso_uniforms(seed, (uint64_t)gp, 0u, 0u, D, a, b);
-    for (j = 0; j < D; ++j) {
-      double x0 = B->lo[j] + a[j] * (B->hi[j] - B->lo[j]);
-      double y0 = B->lo[j] + b[j] * (B->hi[j] - B->lo[j]);
-      x[gp * D + j] = x0;
-      vel[gp * D + j] = 0.5 * (y0 - x0);
-      pbest[gp * D + j] = x0;
-    }
-    pbestJ[gp] = INFINITY;
-  }
+  int32_t s, j;
+  int64_t p;
   for (s = 0; s < n_traces; ++s) {
-    gbestJ[s] = INFINITY;
-    for (j = 0; j < D; ++j) gbest[s * D + j] = x[(int64_t)s * P * D + j];
-  }
-
-  for (it = 0; it < Sw->n_iters; ++it) {
-    /* forward batch on every particle */
-#ifdef ORC_OPENMP /* parity-only build; never the timed baseline */
-#pragma omp parallel for schedule(dynamic, 4)
-#endif
-    for (gp = 0; gp < PT; ++gp) {
-      double theta[4];
-      orc_theta_of_x(B, D, x + gp * D, theta);
-      J[gp] = eval(ctx, theta, trace + (gp / P) * W);
-    }
-    /* personal best (strict <; NaN and +Inf never win) */
-    for (gp = 0; gp < PT; ++gp) {
-      if (J[gp] < pbestJ[gp]) {
-        pbestJ[gp] = J[gp];
-        for (j = 0; j < D; ++j) pbest[gp * D + j] = x[gp * D + j];
-      }
-    }
-    /* global best per swarm: lowest index among equal minima */
-    for (s = 0; s < n_traces; ++s) {
-      int64_t p;
-      for (p = 0; p < P; ++p) {
-        gp = (int64_t)s * P + p;
-        if (pbestJ[gp] < gbestJ[s]) {
-          gbestJ[s] = pbestJ[gp];
-          for (j = 0; j < D; ++j) gbest[s * D + j] = pbest[gp * D + j];
-        }
-      }
-    }
-    if (dump) {
-      for (gp = 0; gp < PT; ++gp) {
-        double* r = dump + ((int64_t)it * PT + gp) * rec;
-        for (j = 0; j < D; ++j) {
-          r[j] = x[gp * D + j];
-          r[D + j] = vel[gp * D + j];
-          r[2 * D + j] = pbest[gp * D + j];
-        }
-        r[3 * D] = J[gp];
-        r[3 * D + 1] = pbestJ[gp];
-      }
-    }
-    if (gbest_hist) {
-      for (s = 0; s < n_traces; ++s) {
-        double* r = gbest_hist + ((int64_t)it * n_traces + s) * (D + 1);
-        for (j = 0; j < D; ++j) r[j] = gbest[s * D + j];
-        r[D] = gbestJ[s];
-      }
-    }
-    if (it == Sw->n_iters - 1) break;
-    /* move: Eq. 8, then x <- x + v, then the bound rule */
-    for (gp = 0; gp < PT; ++gp) {
+    for (p = p0; p < p1; ++p) {
+      const int64_t gp = (int64_t)s * P + p;
       double r1[4], r2[4];
-      s = (int32_t)(gp / P);
-      orc_pso_uniforms(seed, (uint64_t)gp, (uint32_t)it, 1u, D, r1, r2);
       const double* social = gbest + s * D;
+      orc_pso_uniforms(seed, (uint64_t)gp, (uint32_t)it, 1u, D, r1, r2);
       if (Sw->topology == 1) {
         /* ring of three inside the swarm of trace s */
-        int64_t p = gp - (int64_t)s * P;
         int64_t cand[3], best, c;
         cand[0] = (p + P - 1) % P;
         cand[1] = p;
@@ -444,6 +387,125 @@ void orc_pso_core(orc_eval_fn eval, const void* ctx, int64_t W, int32_t D,
       }
     }
   }
+}
+
+int32_t orc_pso_core(orc_eval_fn eval, const void* ctx, int64_t W, int32_t D,
+                     const orc_box* B, const orc_swarm* Sw, uint64_t seed,
+                     const double* trace, int32_t n_traces, double* theta_star,
+                     double* J_star, double* dump, double* gbest_hist) {
+  const int64_t P = Sw->n_particles;
+  const int64_t PT = P * (int64_t)n_traces;
+  const int64_t rec = 3 * D + 2;
+  const int64_t chunk =
+      (Sw->async_chunk > 0 && Sw->async_chunk < P) ? Sw->async_chunk : P;
+  const int asynchronous = chunk < P;
+  double* x = (double*)malloc((size_t)(PT * D) * sizeof(double));
+  double* vel = (double*)malloc((size_t)(PT * D) * sizeof(double));
+  double* pbest = (double*)malloc((size_t)(PT * D) * sizeof(double));
+  double* pbestJ = (double*)malloc((size_t)PT * sizeof(double));
+  double* J = (double*)malloc((size_t)PT * sizeof(double));
+  double* gbest = (double*)malloc((size_t)(n_traces * D) * sizeof(double));
+  double* gbestJ = (double*)malloc((size_t)n_traces * sizeof(double));
+  int64_t gp, i, c0;
+  int32_t it, j, s, done = 0;
+
+  if (dump)
+    for (i = 0; i < (int64_t)Sw->n_iters * PT * rec; ++i) dump[i] = NAN;
+  if (gbest_hist)
+    for (i = 0; i < (int64_t)Sw->n_iters * n_traces * (D + 1); ++i)
+      gbest_hist[i] = NAN;
+
+  /* initialisation: uniform positions and velocities in the search space */
+  for (gp = 0; gp < PT; ++gp) {
+    double a[4], b[4];
+    orc_pso_uniforms(seed, (uint64_t)gp, 0u, 0u, D, a, b);
+    for (j = 0; j < D; ++j) {
+      double x0 = B->lo[j] + a[j] * (B->hi[j] - B->lo[j]);
+      double y0 = B->lo[j] + b[j] * (B->hi[j] - B->lo[j]);
+      x[gp * D + j] = x0;
+      vel[gp * D + j] = 0.5 * (y0 - x0);
+      pbest[gp * D + j] = x0;
+    }
+    pbestJ[gp] = INFINITY;
+  }
+  for (s = 0; s < n_traces; ++s) {
+    gbestJ[s] = INFINITY;
+    for (j = 0; j < D; ++j) gbest[s * D + j] = x[(int64_t)s * P * D + j];
+  }
+
+  for (it = 0; it < Sw->n_iters; ++it) {
+    const int last = (it == Sw->n_iters - 1);
+    int reached;
+    for (c0 = 0; c0 < P; c0 += chunk) {
+      const int64_t c1 = (c0 + chunk < P) ? c0 + chunk : P;
+      const int64_t cn = c1 - c0;
+      /* forward batch on the particles of this chunk */
+#ifdef ORC_OPENMP /* parity-only build; never the timed baseline */
+#pragma omp parallel for schedule(dynamic, 4)
+#endif
+      for (i = 0; i < cn * n_traces; ++i) {
+        const int64_t q = (i / cn) * P + c0 + (i % cn);
+        double theta[4];
+        orc_theta_of_x(B, D, x + q * D, theta);
+        J[q] = eval(ctx, theta, trace + (q / P) * W);
+      }
+      for (s = 0; s < n_traces; ++s) {
+        int64_t p;
+        /* personal best (strict <; NaN and +Inf never win) */
+        for (p = c0; p < c1; ++p) {
+          gp = (int64_t)s * P + p;
+          if (J[gp] < pbestJ[gp]) {
+            pbestJ[gp] = J[gp];
+            for (j = 0; j < D; ++j) pbest[gp * D + j] = x[gp * D + j];
+          }
+        }
+        /* global best per swarm: lowest index among equal minima */
+        for (p = c0; p < c1; ++p) {
+          gp = (int64_t)s * P + p;
+          if (pbestJ[gp] < gbestJ[s]) {
+            gbestJ[s] = pbestJ[gp];
+            for (j = 0; j < D; ++j) gbest[s * D + j] = pbest[gp * D + j];
+          }
+        }
+        if (dump) {
+          for (p = c0; p < c1; ++p) {
+            double* r;
+            gp = (int64_t)s * P + p;
+            r = dump + ((int64_t)it * PT + gp) * rec;
+            for (j = 0; j < D; ++j) {
+              r[j] = x[gp * D + j];
+              r[D + j] = vel[gp * D + j];
+              r[2 * D + j] = pbest[gp * D + j];
+            }
+            r[3 * D] = J[gp];
+            r[3 * D + 1] = pbestJ[gp];
+          }
+        }
+      }
+      /* asynchronous swarm: the chunk moves before the next one is evaluated */
+      if (asynchronous && !last)
+        pso_move_range(D, B, Sw, seed, it, n_traces, c0, c1, x, vel, pbest,
+                       pbestJ, gbest);
+    }
+    if (gbest_hist) {
+      for (s = 0; s < n_traces; ++s) {
+        double* r = gbest_hist + ((int64_t)it * n_traces + s) * (D + 1);
+        for (j = 0; j < D; ++j) r[j] = gbest[s * D + j];
+        r[D] = gbestJ[s];
+      }
+    }
+    done = it + 1;
+    if (last) break;
+    /* cost cutoff: every trace's best is at or below the target */
+    reached = (Sw->j_target > 0.0);
+    for (s = 0; s < n_traces; ++s)
+      if (!(gbestJ[s] <= Sw->j_target)) reached = 0;
+    if (reached) break;
+    /* synchronous swarm: move after the whole batch (Eq. 8, x <- x + v, bounds) */
+    if (!asynchronous)
+      pso_move_range(D, B, Sw, seed, it, n_traces, 0, P, x, vel, pbest, pbestJ,
+                     gbest);
+  }
 
   for (s = 0; s < n_traces; ++s) {
     orc_theta_of_x(B, D, gbest + s * D, theta_star + s * D);
@@ -456,6 +518,7 @@ void orc_pso_core(orc_eval_fn eval, const void* ctx, int64_t W, int32_t D,
   free(J);
   free(gbest);
   free(gbestJ);
+  return done;
 }
 
 /* The point-mass forward solve as the PSO's cost function. */
@@ -469,16 +532,17 @@ static double pm_eval(const void* ctx, const double* theta, const double* U) {
   return orc_misfit(c->M, theta, c->z0, c->v0, U);
 }
 
-void orc_pso_invert(const orc_model* M, const orc_box* B, const orc_swarm* Sw,
-                    uint64_t seed, const double* trace, int32_t n_traces,
-                    double z0, double v0, double* theta_star, double* J_star,
-                    double* dump, double* gbest_hist) {
+int32_t orc_pso_invert(const orc_model* M, const orc_box* B,
+                       const orc_swarm* Sw, uint64_t seed, const double* trace,
+                       int32_t n_traces, double z0, double v0,
+                       double* theta_star, double* J_star, double* dump,
+                       double* gbest_hist) {
   orc_consts C;
   pm_ctx ctx;
   orc_constants(M, &C);
   ctx.M = M;
   ctx.z0 = z0;
   ctx.v0 = v0;
-  orc_pso_core(pm_eval, &ctx, C.W, M->n_theta, B, Sw, seed, trace, n_traces,
-               theta_star, J_star, dump, gbest_hist);
+  return orc_pso_core(pm_eval, &ctx, C.W, M->n_theta, B, Sw, seed, trace,
+                      n_traces, theta_star, J_star, dump, gbest_hist);
 }

@@ -22,11 +22,14 @@
  *   RK4 tableau, linear closed forms, step-halving order, force-law hand
  *   values, energy balance, misfit identities, Philox known answers, PSO
  *   invariants and a hand-computed PSO step, scipy DOP853 on the nonlinear
- *   problem.
+ *   problem; the cost cutoff and the asynchronous swarm on a hand-made cost
+ *   callback whose stopping batch and result are written down by hand
+ *   (tests/test_oracle_pso_rules.py).
  * PARITY UNPINNED (design choices with nothing outside this file to check
  * against): the PSO bound rule (clamp + zero
  * velocity), the initial-velocity rule v0 = (U(lo,hi) - x0)/2, the
- * lowest-index tie-break, and the Philox counter layout.
+ * lowest-index tie-break, the Philox counter layout, the ring of three (R23)
+ * and the chunked reading of "asynchronous" (R25).
  */
 #ifndef AFM_ORACLE_H
 #define AFM_ORACLE_H
@@ -85,12 +88,25 @@ typedef struct {
   int32_t n_particles; /* per trace                                          */
   int32_t n_iters;     /* number of forward batches (iteration 0 = x0)       */
   double w, c1, c2;    /* Eq. 8 weights                                      */
+  double j_target;     /* cost cutoff ("convergence cutoff",
+                          264 "cutoff convergence threshold of J_L2 = 0.0005";
+                          DESIGN.md R24): > 0: the run ends after the first
+                          batch at which EVERY trace's global-best J is
+                          <= j_target, and no move follows that batch;
+                          <= 0: off, all n_iters batches are run            */
   int32_t topology;    /* 0: global best (the paper's "g_b");
                           1: ring of three (R23): the social attractor
                           of particle p is the best personal best among
                           p-1, p, p+1 (indices wrap inside the swarm; lowest
                           index among equal minima)                          */
-  int32_t pad_;
+  int32_t async_chunk; /* 0 (or >= n_particles): synchronous swarm, the paper's
+                          generation-by-generation PSO.  B in 1..n_particles-1:
+                          asynchronous swarm (R25):
+                          every swarm is processed in chunks of B particles in
+                          index order; a chunk is evaluated, its personal bests
+                          and the swarm's best are updated, and the chunk moves
+                          at once with the best known at that moment, so later
+                          chunks of the same batch already see it           */
 } orc_swarm;
 
 void   orc_constants(const orc_model* M, orc_consts* C);
@@ -144,12 +160,16 @@ void   orc_pso_uniforms(uint64_t seed, uint64_t gp, uint32_t it,
 void   orc_theta_of_x(const orc_box* B, int32_t D, const double* x,
                       double* theta);
 
-/* Synchronous global-best PSO around the forward batch.
+/* PSO around the forward batch (synchronous global best unless Sw says
+ * otherwise).
  * dump (or NULL): [n_iters][n_traces*P][3D+2] = x, v, pbest, J, pbestJ,
  * recorded after the personal-best update of each iteration and before the
  * move.  gbest_hist (or NULL): [n_iters][n_traces][D+1] = gbest x, gbestJ.
- * Outputs theta_star [n_traces][D], J_star [n_traces]. */
-void   orc_pso_invert(const orc_model* M, const orc_box* B,
+ * Rows of batches that the cost cutoff left unrun are NaN.
+ * Outputs theta_star [n_traces][D], J_star [n_traces].
+ * Returns the number of forward batches run (n_iters unless j_target cut the
+ * run short): the paper's "generations to convergence". */
+int32_t orc_pso_invert(const orc_model* M, const orc_box* B,
                       const orc_swarm* Sw, uint64_t seed, const double* trace,
                       int32_t n_traces, double z0, double v0,
                       double* theta_star, double* J_star, double* dump,
@@ -159,7 +179,7 @@ void   orc_pso_invert(const orc_model* M, const orc_box* B,
  * point-mass misfit above, or the beam misfit of afm_oracle_beam.h). */
 typedef double (*orc_eval_fn)(const void* ctx, const double* theta,
                               const double* trace_s);
-void   orc_pso_core(orc_eval_fn eval, const void* ctx, int64_t W, int32_t D,
+int32_t orc_pso_core(orc_eval_fn eval, const void* ctx, int64_t W, int32_t D,
                     const orc_box* B, const orc_swarm* Sw, uint64_t seed,
                     const double* trace, int32_t n_traces, double* theta_star,
                     double* J_star, double* dump, double* gbest_hist);

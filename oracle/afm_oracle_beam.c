@@ -235,12 +235,13 @@ static double beam_eval(const void* ctx, const double* theta, const double* U) {
   return orc_beam_misfit((const orc_beam*)ctx, theta, U);
 }
 
-void orc_beam_pso_invert(const orc_beam* B, const orc_box* Bx,
-                         const orc_swarm* Sw, uint64_t seed, const double* trace,
-                         int32_t n_traces, double* theta_star, double* J_star,
-                         double* dump, double* gbest_hist) {
+int32_t orc_beam_pso_invert(const orc_beam* B, const orc_box* Bx,
+                            const orc_swarm* Sw, uint64_t seed,
+                            const double* trace, int32_t n_traces,
+                            double* theta_star, double* J_star, double* dump,
+                            double* gbest_hist) {
   orc_beam_modes Mo;
   orc_beam_setup(B, &Mo);
-  orc_pso_core(beam_eval, B, Mo.W, B->n_theta, Bx, Sw, seed, trace, n_traces,
-               theta_star, J_star, dump, gbest_hist);
+  return orc_pso_core(beam_eval, B, Mo.W, B->n_theta, Bx, Sw, seed, trace,
+                      n_traces, theta_star, J_star, dump, gbest_hist);
 }

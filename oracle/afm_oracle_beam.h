@@ -73,12 +73,13 @@ double orc_beam_misfit(const orc_beam* B, const double* theta,
 void   orc_beam_forward_batch(const orc_beam* B, const double* params,
                               int64_t P, const double* trace, int32_t n_traces,
                               double* misfit);
-/* The PSO of afm_oracle.h around the beam forward batch (same streams). */
-void   orc_beam_pso_invert(const orc_beam* B, const orc_box* Bx,
-                           const orc_swarm* Sw, uint64_t seed,
-                           const double* trace, int32_t n_traces,
-                           double* theta_star, double* J_star, double* dump,
-                           double* gbest_hist);
+/* The PSO of afm_oracle.h around the beam forward batch (same streams, same
+ * cutoff and chunk rules); returns the number of batches run. */
+int32_t orc_beam_pso_invert(const orc_beam* B, const orc_box* Bx,
+                            const orc_swarm* Sw, uint64_t seed,
+                            const double* trace, int32_t n_traces,
+                            double* theta_star, double* J_star, double* dump,
+                            double* gbest_hist);
 
 #ifdef __cplusplus
 }

@@ -39,7 +39,13 @@ class Box(C.Structure):
 class Swarm(C.Structure):
     _fields_ = [("n_particles", C.c_int32), ("n_iters", C.c_int32),
                 ("w", C.c_double), ("c1", C.c_double), ("c2", C.c_double),
-                ("topology", C.c_int32), ("pad_", C.c_int32)]
+                ("j_target", C.c_double), ("topology", C.c_int32),
+                ("async_chunk", C.c_int32)]
+
+
+# cost callback of orc_pso_core: double eval(ctx, theta[D], trace_s[W])
+EVAL_FN = C.CFUNCTYPE(C.c_double, C.c_void_p, C.POINTER(C.c_double),
+                      C.POINTER(C.c_double))
 
 
 class Beam(C.Structure):
@@ -112,7 +118,11 @@ def lib(openmp=False):
                                      C.POINTER(Swarm), C.c_uint64, _dp,
                                      C.c_int32, C.c_double, C.c_double, _dp,
                                      _dp, _dp, _dp]
-        L.orc_pso_invert.restype = None
+        L.orc_pso_invert.restype = C.c_int32
+        L.orc_pso_core.argtypes = [EVAL_FN, C.c_void_p, C.c_int64, C.c_int32,
+                                   C.POINTER(Box), C.POINTER(Swarm), C.c_uint64,
+                                   _dp, C.c_int32, _dp, _dp, _dp, _dp]
+        L.orc_pso_core.restype = C.c_int32
         L.orc_beam_setup.argtypes = [C.POINTER(Beam), C.POINTER(BeamModes)]
         L.orc_beam_setup.restype = None
         L.orc_beam_shape.argtypes = [C.POINTER(Beam), C.POINTER(BeamModes), C.c_int32,
@@ -130,7 +140,7 @@ def lib(openmp=False):
         L.orc_beam_pso_invert.argtypes = [C.POINTER(Beam), C.POINTER(Box),
                                           C.POINTER(Swarm), C.c_uint64, _dp, C.c_int32,
                                           _dp, _dp, _dp, _dp]
-        L.orc_beam_pso_invert.restype = None
+        L.orc_beam_pso_invert.restype = C.c_int32
         _libs[key] = L
     return _libs[key]
 
@@ -159,12 +169,14 @@ def box_from(wl):
     return b
 
 
-def swarm_from(wl, n_particles=None, n_iters=None, topology=None):
+def swarm_from(wl, n_particles=None, n_iters=None, topology=None, j_target=0.0,
+               async_chunk=0):
     s = wl["swarm"]
     return Swarm(n_particles=s["n_particles"] if n_particles is None else n_particles,
                  n_iters=s["n_iters"] if n_iters is None else n_iters,
-                 w=s["w"], c1=s["c1"], c2=s["c2"],
-                 topology=s.get("topology", 0) if topology is None else topology, pad_=0)
+                 w=s["w"], c1=s["c1"], c2=s["c2"], j_target=j_target,
+                 topology=s.get("topology", 0) if topology is None else topology,
+                 async_chunk=async_chunk)
 
 
 # ---- thin calls -------------------------------------------------------------
@@ -256,7 +268,7 @@ def theta_of_x(B, D, x):
 def pso_invert(M, B, Sw, seed, trace, z0, v0, n_traces=1, dump=False,
                openmp=False):
     """Returns dict(theta_star [T][D], J_star [T], dump [it][PT][3D+2] or None,
-    gbest_hist [it][T][D+1])."""
+    gbest_hist [it][T][D+1], n_iters_done); rows of unrun batches are NaN."""
     D = M.n_theta
     PT = Sw.n_particles * n_traces
     tr = _f64(trace)
@@ -265,10 +277,31 @@ def pso_invert(M, B, Sw, seed, trace, z0, v0, n_traces=1, dump=False,
     Js = np.empty(n_traces)
     dmp = np.empty((Sw.n_iters, PT, 3 * D + 2)) if dump else None
     gh = np.empty((Sw.n_iters, n_traces, D + 1))
-    lib(openmp).orc_pso_invert(C.byref(M), C.byref(B), C.byref(Sw), seed,
-                               _ptr(tr), n_traces, z0, v0, _ptr(th), _ptr(Js),
-                               _ptr(dmp), _ptr(gh))
-    return dict(theta_star=th, J_star=Js, dump=dmp, gbest_hist=gh)
+    done = lib(openmp).orc_pso_invert(C.byref(M), C.byref(B), C.byref(Sw), seed,
+                                      _ptr(tr), n_traces, z0, v0, _ptr(th), _ptr(Js),
+                                      _ptr(dmp), _ptr(gh))
+    return dict(theta_star=th, J_star=Js, dump=dmp, gbest_hist=gh, n_iters_done=int(done))
+
+
+def pso_core(cost, D, B, Sw, seed, trace, n_traces=1):
+    """The oracle's PSO loop around a PYTHON cost function cost(theta[D], U_s[W]) ->
+    float (the pins of the cutoff and chunk rules use hand-made costs).  trace is
+    [n_traces][W].  Single-threaded.  Same outputs as pso_invert, dump included."""
+    tr = _f64(trace).reshape(n_traces, -1)
+    Wn = tr.shape[1]
+    PT = Sw.n_particles * n_traces
+
+    def _cb(_ctx, th, U):
+        return float(cost(np.array([th[j] for j in range(D)]),
+                          np.ctypeslib.as_array(U, shape=(Wn,))))
+
+    th = np.empty((n_traces, D))
+    Js = np.empty(n_traces)
+    dmp = np.empty((Sw.n_iters, PT, 3 * D + 2))
+    gh = np.empty((Sw.n_iters, n_traces, D + 1))
+    done = lib().orc_pso_core(EVAL_FN(_cb), None, Wn, D, C.byref(B), C.byref(Sw), seed,
+                              _ptr(tr), n_traces, _ptr(th), _ptr(Js), _ptr(dmp), _ptr(gh))
+    return dict(theta_star=th, J_star=Js, dump=dmp, gbest_hist=gh, n_iters_done=int(done))
 
 
 # ---- the multi-mode Euler-Bernoulli beam (afm_oracle_beam.h) ------------------
@@ -331,6 +364,7 @@ def beam_pso_invert(B, Bx, Sw, seed, trace, n_traces=1, dump=False, openmp=False
     Js = np.empty(n_traces)
     dmp = np.empty((Sw.n_iters, PT, 3 * D + 2)) if dump else None
     gh = np.empty((Sw.n_iters, n_traces, D + 1))
-    lib(openmp).orc_beam_pso_invert(C.byref(B), C.byref(Bx), C.byref(Sw), seed, _ptr(tr),
-                                    n_traces, _ptr(th), _ptr(Js), _ptr(dmp), _ptr(gh))
-    return dict(theta_star=th, J_star=Js, dump=dmp, gbest_hist=gh)
+    done = lib(openmp).orc_beam_pso_invert(C.byref(B), C.byref(Bx), C.byref(Sw), seed,
+                                           _ptr(tr), n_traces, _ptr(th), _ptr(Js),
+                                           _ptr(dmp), _ptr(gh))
+    return dict(theta_star=th, J_star=Js, dump=dmp, gbest_hist=gh, n_iters_done=int(done))

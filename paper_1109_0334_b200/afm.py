@@ -276,7 +276,8 @@ def afm_forward_batch_host(params, trace, cfg, z0v0=None, misfit=None, stream=No
 def afm_pso_invert(bounds, swarm, seed, trace, cfg, dump=False, hist=False,
                    stream=None):
     """Returns dict(theta_star [T][D], J_star [T], n_iters_done, dump, gbest_hist);
-    dump / gbest_hist are device tensors or None."""
+    dump / gbest_hist are device tensors or None; rows of batches a cost cutoff left
+    unrun are not written."""
     torch = _torch()
     trace = _dev_f64(trace, "trace")
     if trace.numel() != cfg.n_traces * cfg.n_window:
@@ -285,8 +286,13 @@ def afm_pso_invert(bounds, swarm, seed, trace, cfg, dump=False, hist=False,
     PT = swarm.n_particles * T
     th = np.empty((T, D), dtype=np.float64)
     Js = np.empty(T, dtype=np.float64)
-    dmp = (torch.empty((swarm.n_iters, PT, 3 * D + 2), dtype=torch.float64,
-                       device=trace.device) if dump else None)
+    if isinstance(dump, torch.Tensor):          # caller-owned [n_iters][PT][3D+2]
+        dmp = _dev_f64(dump, "dump")
+        if dmp.numel() != swarm.n_iters * PT * (3 * D + 2):
+            raise ValueError("dump must be [n_iters][PT][3D+2]")
+    else:
+        dmp = (torch.empty((swarm.n_iters, PT, 3 * D + 2), dtype=torch.float64,
+                           device=trace.device) if dump else None)
     gh = (torch.empty((swarm.n_iters, T, D + 1), dtype=torch.float64,
                       device=trace.device) if hist else None)
     done = C.c_int32(0)

@@ -137,20 +137,92 @@ def test_noise_free_truth_recovery(afm):
     assert g["J_star"][0] < 1e-6 * wl["n_window"] * wl["sigma"] ** 2
 
 
-def test_j_target_stops_early(afm):
+def _cut_target(hist, after):
+    """A cutoff strictly between two successive, distinct values of a best-cost
+    history (geometric mean), first crossed at batch k >= after: the ~1e-11 relative
+    difference between the two forward solvers cannot move the crossing."""
+    for k in range(max(after, 1), len(hist)):
+        if hist[k] < hist[k - 1] * (1 - 1e-6):
+            return float(np.sqrt(hist[k] * hist[k - 1])), k
+    raise AssertionError("no strict improvement after batch %d" % after)
+
+
+def _both_cut(afm, wl, trace, seed, j_target):
+    import torch
+    g = afm.afm_pso_invert(afm.bounds_from(wl), afm.swarm_from(wl, j_target=j_target), seed,
+                           torch.as_tensor(np.ascontiguousarray(trace), device="cuda"),
+                           afm.cfg_from(wl), dump=True, hist=True)
+    o = orc.pso_invert(orc.model_from(wl), orc.box_from(wl),
+                       orc.swarm_from(wl, j_target=j_target), seed, trace, wl["z0"],
+                       wl["v0"], n_traces=wl["n_traces"], dump=True, openmp=True)
+    return g, o
+
+
+def _compare_cut_runs(g, o, D):
+    """Batches run, theta*, J* and every recorded row up to the stop."""
+    n = o["n_iters_done"]
+    assert g["n_iters_done"] == n
+    gc = dict(g, dump=g["dump"][:n], gbest_hist=g["gbest_hist"][:n])
+    oc = dict(o, dump=o["dump"][:n], gbest_hist=o["gbest_hist"][:n])
+    _compare_runs(gc, oc, D)
+    assert np.all(np.isnan(o["dump"][n:]))              # the oracle ran no further batch
+
+
+def test_j_target_single_trace_against_the_oracle(afm):
+    """Cost cutoff (R24): the target is taken from
+    the ORACLE's own uncut history; both sides must stop after the same batch with
+    the same swarm, and no move follows the stopping batch (the dump row of that
+    batch holds the positions evaluated in it; the caller's later rows are left
+    untouched)."""
     import torch
     wl = wlm.scaled(wlm.config(0), n_iters=60)
     trace = oracle_trace(wl)
-    t = torch.as_tensor(trace, device="cuda")
-    full = afm.afm_pso_invert(afm.bounds_from(wl), afm.swarm_from(wl), 0, t,
-                              afm.cfg_from(wl), hist=True)
-    hist = full["gbest_hist"].cpu().numpy()[:, 0, 2]
-    target = hist[25] * (1 + 1e-12)
-    first = int(np.argmax(hist <= target))
-    cut = afm.afm_pso_invert(afm.bounds_from(wl), afm.swarm_from(wl, j_target=target), 0, t,
-                             afm.cfg_from(wl))
-    assert cut["n_iters_done"] == first + 1 <= 26
-    assert cut["J_star"][0] == hist[first]
+    full = orc.pso_invert(orc.model_from(wl), orc.box_from(wl), orc.swarm_from(wl), 0, trace,
+                          wl["z0"], wl["v0"], openmp=True)
+    target, k = _cut_target(full["gbest_hist"][:, 0, 2], 20)
+    g, o = _both_cut(afm, wl, trace, 0, target)
+    assert o["n_iters_done"] == k + 1 < 60
+    _compare_cut_runs(g, o, 2)
+    assert g["J_star"][0] <= target < full["gbest_hist"][k - 1, 0, 2]
+    # a target nobody reaches runs every batch; a target met by the very first batch
+    # stops after one
+    g, o = _both_cut(afm, wl, trace, 0, 1e-30)
+    assert g["n_iters_done"] == o["n_iters_done"] == 60
+    g, o = _both_cut(afm, wl, trace, 0, 1.0)
+    assert g["n_iters_done"] == o["n_iters_done"] == 1
+    _compare_cut_runs(g, o, 2)
+    # rows after the stop are not written
+    sentinel = torch.full((60, 64, 8), -7.0, dtype=torch.float64, device="cuda")
+    th = afm.afm_pso_invert(afm.bounds_from(wl), afm.swarm_from(wl, j_target=1.0), 0,
+                            torch.as_tensor(trace, device="cuda"), afm.cfg_from(wl),
+                            dump=sentinel)
+    assert th["n_iters_done"] == 1
+    assert bool((sentinel[1:] == -7.0).all()) and not bool((sentinel[0] == -7.0).any())
+
+
+def test_j_target_waits_for_every_trace(afm):
+    """Three pixels with their own traces and swarms cross the same cutoff at
+    different batches; the run ends after the LAST of them has crossed (every
+    trace's best <= target), the early pixels keep improving meanwhile."""
+    wl = wlm.scaled(wlm.config(4), n_cycles=10, n_skip_cycles=5, n_traces=3,
+                    n_particles=48, n_iters=40)
+    trace = oracle_trace(wl, truths=wlm.pixel_truths(wl))
+    full = orc.pso_invert(orc.model_from(wl), orc.box_from(wl), orc.swarm_from(wl), 5, trace,
+                          wl["z0"], wl["v0"], n_traces=3, openmp=True)
+    h = full["gbest_hist"][:, :, 3]                      # [batch][trace]
+    # cutoff from the trace that is slowest to get there, between two of its values
+    slow = int(np.argmax(h[20]))
+    target, _ = _cut_target(h[:, slow], 12)
+    cross = [int(np.argmax(h[:, s] <= target)) for s in range(3)]
+    assert all(h[c, s] <= target for s, c in enumerate(cross))
+    assert len(set(cross)) > 1, cross                    # the pixels do differ
+    for s in range(3):                                   # no crossing is a near tie
+        assert np.min(np.abs(h[:, s] / target - 1.0)) > 1e-6
+    g, o = _both_cut(afm, wl, trace, 5, target)
+    assert o["n_iters_done"] == max(cross) + 1 < 40
+    _compare_cut_runs(g, o, 3)
+    first = int(np.argmin(cross))
+    assert o["J_star"][first] <= h[cross[first], first]
 
 
 def test_pso_step_on_supplied_misfits(afm):
