@@ -343,7 +343,13 @@ void afm_reset_launch_count(void);
  * spread the batch over all SM sub-partitions), "pack" (order the particles
  * of a DMT-law batch by trace, initial phase and stiffness so that the lanes of a
  * warp touch the sample together: 1 = never, 2 = always, 0 = auto in the
- * throughput regime; results do not depend on it).
+ * throughput regime; results do not depend on it), "queue" (segment-queue
+ * scheduling of the FP64 throughput form: the time loop of every warp of
+ * particles is cut into segments that persistent workers hand on through a
+ * ticket queue, which balances a batch of a few warps per SM sub-partition;
+ * 1 = never, 2 = always, 0 = auto; results do not depend on it), "segs"
+ * (segments per trajectory, 0 = auto, about 450 steps each), "workers" (queue
+ * workers per SM sub-partition, 1..8, 0 = auto).
  * Returns AFM_EINVAL for an unknown name or value. */
 int afm_set_option(const char* name, int64_t value);
 

@@ -56,6 +56,9 @@ int g_opt_ppt = 0;    // 0 = auto
 int g_opt_form = 0;   // 0 = auto, 1 = throughput form, 2 = latency form
 int g_opt_lanes = 0;  // 0 = auto; latency form: particles per warp
 int g_opt_pack = 0;   // 0 = auto, 1 = never, 2 = always (DMT laws only)
+int g_opt_queue = 0;  // 0 = auto, 1 = never, 2 = always: segment-queue scheduling
+int g_opt_segs = 0;   // 0 = auto (~450 steps each): time segments per chain of the queue kernel
+int g_opt_workers = 0;  // 0 = auto: queue workers per SM sub-partition
 int g_n_sm = 148;
 
 // ---- grow-only device workspace ------------------------------------------------
@@ -92,6 +95,7 @@ struct Workspace {
   Buffer h_params, h_trace, h_z0v0, h_misfit;  // staging for the *_host calls
   Buffer scratch;                      // theta for afm_trajectory
   Buffer sort;                         // warp-packing keys, order, radix-sort temp
+  Buffer segq;                         // segment queue: control words, slots, checkpoints
   cudaEvent_t last_use = nullptr;      // orders reuse across streams
   cudaStream_t last_stream = nullptr;
   bool checked_device = false;
@@ -362,6 +366,64 @@ int integrate_bpt(int64_t per, int block, int ppt, int variant, int lanes) {
   return variant == 1 ? blocks_per_trace(per, lanes) : blocks_per_trace(per, block * ppt);
 }
 
+// The FP64 integrate launch.  In the throughput form a batch of a few warps per
+// SM sub-partition goes through the segment queue (integrate_misfit_f64_q):
+// floor(r) + 1 persistent one-warp workers per sub-partition for r chains per
+// sub-partition, so that the spare worker slots rotate over the whole device.
+// Lock held.
+int run_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block,
+                      int variant, cudaStream_t st) {
+  const int64_t chains = (int64_t)blocks_per_trace(io.per, 32) * io.n_traces;
+  const int64_t subparts = (int64_t)4 * g_n_sm;
+  bool use_q = (variant == 0 && block == 32 && g_opt_queue != 1 && chains < (1 << 20));
+  if (use_q && g_opt_queue == 0)
+    use_q = (2 * chains >= 3 * subparts && chains <= 6 * subparts && mc.n_tiles >= 64);
+  if (!use_q) {
+    LAUNCHED(launch_integrate_f64(mc, io, block, variant, st));
+    return AFM_OK;
+  }
+  int per_sub = g_opt_workers > 0 ? g_opt_workers : (int)(chains / subparts) + 1;
+  if (per_sub > 8) per_sub = 8;
+  int workers = (int)(per_sub * subparts);
+  if (workers > chains) workers = (int)chains;
+  SegQueue q;
+  // segments of about 450 steps (130 us at 3-4 warps per sub-partition: long
+  // against the 2-3 us a hand-over costs, short against the whole solve;
+  // measured on configs[1]: 8 segments 16.4 ms, 32: 15.7, 115: 14.9, 400: 15.3)
+  int segs = g_opt_segs > 0 ? g_opt_segs : (mc.n_tiles * mc.T + 447) / 448;
+  if (segs > mc.n_tiles) segs = mc.n_tiles;
+  if (segs > 2047) segs = 2047;
+  if (segs < 1) segs = 1;
+  q.tiles_per_seg = (mc.n_tiles + segs - 1) / segs;
+  q.n_segs = (mc.n_tiles + q.tiles_per_seg - 1) / q.tiles_per_seg;
+  q.n_chains = (int32_t)chains;
+  q.n_tasks = q.n_chains * q.n_segs;
+  q.timeout_cycles = 40000000000LL;  // ~20 s: only a corrupted queue gets there
+  const size_t slot_bytes = ((size_t)q.n_tasks * 4 + 255) & ~(size_t)255;
+  const size_t need = 256 + slot_bytes + (size_t)chains * 128 * 8;
+  const bool fresh = need > g_ws.segq.cap;
+  if (g_ws.segq.ensure(need))
+    return fail(AFM_ECUDA, "cudaMalloc of the segment queue failed");
+  if (fresh) CUDA_TRY(cudaMemsetAsync(g_ws.segq.p, 0, 256, st));
+  q.ctrl = (unsigned*)g_ws.segq.p;
+  q.slots = (int*)((char*)g_ws.segq.p + 256);
+  q.ckpt = (double*)((char*)g_ws.segq.p + 256 + slot_bytes);
+  LAUNCHED(launch_integrate_f64_q(mc, io, q, workers, st));
+  return AFM_OK;
+}
+
+// After a stream synchronisation: did a queue worker give up waiting (a
+// corrupted queue; see segq_pop)?  The flag is sticky until read here.
+int check_queue_flag(cudaStream_t st) {
+  if (!g_ws.segq.p) return AFM_OK;
+  unsigned flag = 0;
+  CUDA_TRY(cudaMemcpyAsync(&flag, (char*)g_ws.segq.p + 8, 4, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  if (!flag) return AFM_OK;
+  CUDA_TRY(cudaMemsetAsync((char*)g_ws.segq.p + 8, 0, 4, st));
+  return fail(AFM_ECUDA, "segment queue timed out: results of the last batch are invalid");
+}
+
 BoxDev make_box(const afm_bounds* b, int D) {
   BoxDev bd;
   memset(&bd, 0, sizeof(bd));
@@ -438,8 +500,8 @@ int forward_locked(const double* params, int64_t P, const double* trace,
   }
   if (f32)
     LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
-  else
-    LAUNCHED(launch_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st));
+  else if ((rc = run_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st)))
+    return rc;
   if (pk.order) LAUNCHED(launch_pack_scatter(pk.order, pk.J, P, misfit, st));
   return release_ws(st);
 }
@@ -507,7 +569,7 @@ int afm_forward_batch_host(const double* params, int64_t n_particles,
   if (rc) return rc;
   CUDA_TRY(cudaMemcpyAsync(misfit, g_ws.h_misfit.p, mb, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
-  return AFM_OK;
+  return check_queue_flag(st);
 }
 
 int afm_pso_shard_init(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
@@ -655,17 +717,18 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
       iof.mode = 0;
       if (f32)
         LAUNCHED(launch_integrate_f32(mf, iof, block, ppt, st));
-      else
-        LAUNCHED(launch_integrate_f64(mc, iof, block,
-                                      pick_variant(iof.per, iof.n_traces, ppt), st));
+      else if ((rc = run_integrate_f64(mc, iof, block,
+                                       pick_variant(iof.per, iof.n_traces, ppt), st)))
+        return rc;
       LAUNCHED(launch_pack_scatter(pk.order, pk.J, PT, J, st));
       n_cand = blocks_per_trace(per, 128);
       LAUNCHED(launch_pso_best(D, per, T, J, x, pbest, pbestJ, (Cand*)g_ws.cand.p, 128,
                                st));
     } else if (f32) {
       LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
-    } else {
-      LAUNCHED(launch_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st));
+    } else if ((rc = run_integrate_f64(mc, io, block,
+                                       pick_variant(io.per, io.n_traces, ppt), st))) {
+      return rc;
     }
     LAUNCHED(launch_pso_gbest(
         box, D, T, n_cand, (Cand*)g_ws.cand.p, pbest, gbest, gbestJ,
@@ -694,6 +757,7 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
   CUDA_TRY(cudaMemcpyAsync(J_star, Js_dev, (size_t)T * 8, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
   if (n_iters_done) *n_iters_done = done;
+  if ((rc = check_queue_flag(st))) return rc;
   return release_ws(st);
 }
 
@@ -798,8 +862,8 @@ int afm_pso_shard_eval(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   io.lanes = lanes;
   if (f32)
     LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
-  else
-    LAUNCHED(launch_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st));
+  else if ((rc = run_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st)))
+    return rc;
   LAUNCHED(launch_pso_shard_cand(D, T, bpt, first_particle, (Cand*)g_ws.cand.p,
                                  pbest, cand_out, st));
   return release_ws(st);
@@ -1233,6 +1297,21 @@ int afm_set_option(const char* name, int64_t value) {
     g_opt_pack = (int)value;
     return AFM_OK;
   }
+  if (!strcmp(name, "queue")) {
+    if (value < 0 || value > 2) return fail(AFM_EINVAL, "queue must be 0, 1 or 2");
+    g_opt_queue = (int)value;
+    return AFM_OK;
+  }
+  if (!strcmp(name, "workers")) {
+    if (value < 0 || value > 8) return fail(AFM_EINVAL, "workers must be in 0..8");
+    g_opt_workers = (int)value;
+    return AFM_OK;
+  }
+  if (!strcmp(name, "segs")) {
+    if (value < 0 || value > 2047) return fail(AFM_EINVAL, "segs must be in 0..2047");
+    g_opt_segs = (int)value;
+    return AFM_OK;
+  }
   if (!strcmp(name, "tile")) {
     if (value < 0 || value > 2048)
       return fail(AFM_EINVAL, "tile must be in 0..2048");
@@ -1256,6 +1335,7 @@ void afm_shutdown(void) {
   g_ws.h_misfit.release();
   g_ws.scratch.release();
   g_ws.sort.release();
+  g_ws.segq.release();
   if (g_ws.pinned) cudaFreeHost(g_ws.pinned);
   g_ws.pinned = nullptr;
   g_ws.pinned_cap = 0;

@@ -124,7 +124,22 @@ struct IntegrateIO {
   int32_t pad_;
 };
 
+// Segment queue of integrate_misfit_f64_q (afm_kernels.cu): tasks are
+// (chain, segment) = (warp of 32 particles, run of tiles_per_seg time tiles).
+struct SegQueue {
+  int* slots;            // [n_tasks]  (segment << 20) | chain, or -1 = not yet published
+  unsigned* ctrl;        // [0] consume ticket, [1] publish index, [2] time-out flag
+  double* ckpt;          // [n_chains][4][32]: d, w, J, diverged flag of a chain at rest
+  long long timeout_cycles;
+  int32_t n_chains;
+  int32_t n_segs;
+  int32_t n_tasks;       // n_chains * n_segs
+  int32_t tiles_per_seg;
+};
+
 int blocks_per_trace(int64_t per, int block);
+int launch_integrate_f64_q(const ModelConsts& mc, const IntegrateIO& io,
+                           const SegQueue& q, int workers, cudaStream_t st);
 
 int launch_build_stream(const ModelConsts& mc, const double* trace, int n_traces,
                         double* stream, cudaStream_t st);

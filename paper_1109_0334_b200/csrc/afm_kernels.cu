@@ -285,6 +285,217 @@ __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
   }
 }
 
+// ============================================================================
+// integrate-and-misfit, FP64, segment queue (throughput form, one warp per CTA).
+//
+// A forward batch of a few warps per SM sub-partition is unbalanced when every
+// warp is bound to one sub-partition for its whole trajectory: 2 048 warps on
+// 592 sub-partitions leave 3 on some and 4 on others, warps differ up to 3x in
+// cost (general-form steps), and the slowest sub-partition sets the time.  Here
+// the time loop of a warp of particles (a "chain") is cut into segments of
+// q.tiles_per_seg time tiles; a grid of persistent one-warp CTAs (workers, a
+// whole number per sub-partition) takes (chain, segment) tasks from a
+// multi-producer multi-consumer ticket queue in global memory.  A worker that
+// finishes a segment stores the chain's state (d, w, J, diverged flag: 32 B per
+// particle), publishes the chain's next segment at the tail of the queue and
+// takes the ticket at its head; since there are more workers than chains, the
+// published task is picked up at once by the worker that has waited longest, so
+// every chain is always running and the idle slots rotate evenly over all
+// sub-partitions.  The arithmetic of a particle is that of
+// integrate_misfit_f64<LAW, MODE, 1, false>, step for step: results are
+// bit-identical.
+// ============================================================================
+__device__ __forceinline__ int ld_acquire_s32(const int* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_s32(int* p, int v) {
+  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+__global__ void segq_init_kernel(SegQueue q) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < q.n_tasks) q.slots[i] = (i < q.n_chains) ? i : -1;  // segment 0 of chain i
+  if (i == 0) {
+    q.ctrl[0] = 0u;                    // head: next consume ticket
+    q.ctrl[1] = (unsigned)q.n_chains;  // tail: next publish slot
+  }
+}
+
+// Next task of this worker: -1 when every task has been handed out, -2 after a
+// time-out (cannot happen unless the queue is corrupted; keeps a bug from
+// hanging the device).  Called by one lane.
+__device__ __forceinline__ int segq_pop(const SegQueue& q) {
+  const unsigned t = atomicAdd(&q.ctrl[0], 1u);
+  if (t >= (unsigned)q.n_tasks) return -1;
+  const long long t_start = clock64();
+  int v;
+  while ((v = ld_acquire_s32(&q.slots[t])) < 0) {
+    __nanosleep(200);
+    if (clock64() - t_start > q.timeout_cycles) {
+      atomicExch(&q.ctrl[2], 1u);
+      return -2;
+    }
+  }
+  return v;
+}
+
+template <int LAW, int MODE>
+__global__ void __launch_bounds__(32)
+integrate_misfit_f64_q(ModelConsts mc, IntegrateIO io, int blocks_per_tr, SegQueue q) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double4* tile0 = reinterpret_cast<double4*>(smem_raw);
+  double4* tile1 = tile0 + mc.T;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tile1 + mc.T);
+  __shared__ Cand red[32];
+
+  const int tid = threadIdx.x;
+  if (tid == 0) {
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    fence_mbar_init();
+  }
+  __syncthreads();
+  uint32_t n_wait0 = 0u, n_wait1 = 0u;  // completed phases of the two stages
+  const long long a0_bits = __double_as_longlong(mc.a0);
+  DivergeTest T;
+  T.key_max = order_key(mc.d_max);
+  T.key_min = order_key(mc.d_min);
+  T.safe_hi = __double2hiint(mc.d_safe);
+
+  for (;;) {
+    int task = 0;
+    if (tid == 0) task = segq_pop(q);
+    task = __shfl_sync(0xffffffffu, task, 0);
+    if (task < 0) break;
+    const int chain = task & 0xfffff;
+    const int seg = task >> 20;
+    const int s = chain / blocks_per_tr;  // trace of this chain
+    const int64_t li = (int64_t)(chain - s * blocks_per_tr) * 32 + tid;
+    const bool active = li < io.per;
+    const int64_t gp = (int64_t)s * io.per + (active ? li : io.per - 1);
+    const double* stream = io.stream + (int64_t)s * mc.N * 4;
+    const int tile_begin = seg * q.tiles_per_seg;
+    const int tile_end = min(tile_begin + q.tiles_per_seg, mc.n_tiles);
+
+    if (tid == 0) {
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        const int tile = tile_begin + k;
+        if (tile < tile_end) {
+          const int st = tile & 1;
+          const int nb = tile * mc.T;
+          const uint32_t bytes = (uint32_t)min(mc.T, mc.N - nb) * 32u;
+          fence_proxy_async();
+          mbar_arrive_expect_tx(&bars[st], bytes);
+          bulk_g2s(st ? tile1 : tile0, stream + (int64_t)nb * 4, bytes, &bars[st]);
+        }
+      }
+    }
+
+    // a1: parameter map (every segment: the chain may have come from another SM)
+    double xloc[4];
+    Particle64 P[1];
+    double d[1], w[1], J[1];
+    bool bad[1];
+    {
+      double th[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        xloc[j] = 0.0;
+        if (j < mc.D) {
+          const double xv = io.params[gp * mc.D + j];
+          xloc[j] = xv;
+          th[j] = (MODE == 1 && io.box.lg[j]) ? pow(10.0, xv) : xv;
+        }
+      }
+      load_particle(P[0], LAW, th, mc.alpha, mc.beta, mc.a0, mc.inv_a0sq, mc.c_vdw,
+                    mc.c_hertz, mc.c_visc, mc.c_force, mc.zc, mc.c_damp);
+    }
+    double* ck = q.ckpt + (int64_t)chain * 128 + tid;
+    if (seg == 0) {
+      double z0 = mc.z0, v0 = mc.v0;
+      if (io.z0v0 != nullptr) {
+        z0 = io.z0v0[2 * gp];
+        v0 = io.z0v0[2 * gp + 1];
+      }
+      d[0] = z0 + mc.zc;
+      w[0] = v0 * mc.h;
+      J[0] = 0.0;
+      bad[0] = false;
+    } else {
+      d[0] = __ldcg(ck);
+      w[0] = __ldcg(ck + 32);
+      J[0] = __ldcg(ck + 64);
+      bad[0] = __ldcg(ck + 96) != 0.0;
+    }
+    int mode = 0;
+
+    for (int tile = tile_begin; tile < tile_end; ++tile) {
+      const int st = tile & 1;
+      const double4* sp = st ? tile1 : tile0;
+      mbar_wait(&bars[st], (st ? n_wait1 : n_wait0) & 1u);
+      if (st) ++n_wait1; else ++n_wait0;
+      const int n_begin = tile * mc.T;
+      const int n_steps = min(mc.T, mc.N - n_begin);
+      const int k0 = max(0, min(n_steps, mc.n0 - n_begin));
+      run_steps<LAW, 1, false, false>(sp, 0, k0, P, a0_bits, T, d, w, J, bad, mode);
+      run_steps<LAW, 1, false, true>(sp, k0, n_steps, P, a0_bits, T, d, w, J, bad, mode);
+      __syncthreads();
+      if (tid == 0 && tile + 2 < tile_end) {
+        const int nb = (tile + 2) * mc.T;
+        const uint32_t bytes = (uint32_t)min(mc.T, mc.N - nb) * 32u;
+        fence_proxy_async();
+        mbar_arrive_expect_tx(&bars[st], bytes);
+        bulk_g2s(st ? tile1 : tile0, stream + (int64_t)nb * 4, bytes, &bars[st]);
+      }
+    }
+
+    if (tile_end < mc.n_tiles) {
+      // hand the chain on: state first, then the task (release / acquire)
+      __stcg(ck, d[0]);
+      __stcg(ck + 32, w[0]);
+      __stcg(ck + 64, J[0]);
+      __stcg(ck + 96, bad[0] ? 1.0 : 0.0);
+      __threadfence();
+      __syncwarp();
+      if (tid == 0) {
+        const unsigned slot = atomicAdd(&q.ctrl[1], 1u);
+        st_release_s32(&q.slots[slot], ((seg + 1) << 20) | chain);
+      }
+      continue;
+    }
+
+    // last segment: the epilogue of integrate_misfit_f64
+    const long long kw = __double_as_longlong(w[0]) & 0x7fffffffffffffffLL;
+    bad[0] |= (kw >= 0x7ff0000000000000LL);
+    if (bad[0] || !(J[0] == J[0])) J[0] = CUDART_INF;
+    if (active) io.J[gp] = J[0];
+    if (MODE == 1) {
+      double pb = CUDART_INF;
+      long long idx = 0x7fffffffffffffffLL;
+      if (active) {
+        double pq = io.pbestJ[gp];
+        if (J[0] < pq) {
+          pq = J[0];
+          io.pbestJ[gp] = J[0];
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            if (j < mc.D) io.pbest[gp * mc.D + j] = xloc[j];
+        }
+        pb = pq;
+        idx = gp;
+      }
+      block_argmin(pb, idx, red);
+      if (tid == 0) {
+        io.cand[chain].J = pb;
+        io.cand[chain].idx = idx;
+      }
+    }
+  }
+}
+
 // Trajectory of one particle through the same rk4_step (tests/diagnostics).
 template <int LAW>
 __global__ void trajectory_kernel(ModelConsts mc, const double* __restrict__ th,
@@ -630,6 +841,40 @@ int launch_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block
       return -1;
   }
 #undef AFM_DISPATCH
+}
+
+template <int LAW, int MODE>
+static int launch_integrate_q_t(const ModelConsts& mc, const IntegrateIO& io,
+                                const SegQueue& q, int workers, cudaStream_t st) {
+  const int bpt = blocks_per_trace(io.per, 32);
+  const size_t smem = (size_t)mc.T * 32 * 2 + 64;
+  auto kern = integrate_misfit_f64_q<LAW, MODE>;
+  if (smem > 48 * 1024)
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  segq_init_kernel<<<(unsigned)((q.n_tasks + 255) / 256), 256, 0, st>>>(q);
+  kern<<<(unsigned)workers, 32, smem, st>>>(mc, io, bpt, q);
+  return 2;
+}
+
+// Segment-queue form of the throughput kernel (one warp per CTA, `workers`
+// persistent CTAs); q.n_chains must be blocks_per_trace(io.per, 32) * n_traces.
+int launch_integrate_f64_q(const ModelConsts& mc, const IntegrateIO& io,
+                           const SegQueue& q, int workers, cudaStream_t st) {
+#define AFM_DISPATCH_Q(LAWV)                                                   \
+  case LAWV:                                                                   \
+    return io.mode ? launch_integrate_q_t<LAWV, 1>(mc, io, q, workers, st)     \
+                   : launch_integrate_q_t<LAWV, 0>(mc, io, q, workers, st);
+  switch (mc.law) {
+    AFM_DISPATCH_Q(AFM_LAW_NONE)
+    AFM_DISPATCH_Q(AFM_LAW_DMT)
+    AFM_DISPATCH_Q(AFM_LAW_DMT_VISC)
+    AFM_DISPATCH_Q(AFM_LAW_LJ_EXP)
+    AFM_DISPATCH_Q(AFM_LAW_HOOKE)
+    AFM_DISPATCH_Q(AFM_LAW_KELVIN_VOIGT)
+    default:
+      return -1;
+  }
+#undef AFM_DISPATCH_Q
 }
 
 int launch_trajectory(const ModelConsts& mc, const double* theta_dev,

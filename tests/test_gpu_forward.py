@@ -292,6 +292,49 @@ def test_warp_packing_changes_no_result(afm, precision):
         assert rel_err(out[2], Jo).max() < TOL_F64
 
 
+@pytest.mark.parametrize("cfg_i,segs,workers", [(1, 0, 0), (1, 5, 1), (2, 3, 8), (3, 7, 2),
+                                                (4, 1, 4), (4, 2047, 3)])
+def test_segment_queue_changes_no_result(afm, cfg_i, segs, workers):
+    """afm_set_option("queue"): the time loop of every warp of particles is cut into
+    segments handed between persistent workers through a ticket queue in global
+    memory (integrate_misfit_f64_q).  Misfits, and the swarm of an inversion, must be
+    bit-identical to the one-CTA-per-warp kernel: ragged particle counts, several
+    traces, every segment count from one to one tile per segment, fewer workers than
+    chains, all law families; and they must match the oracle."""
+    import torch
+    over = dict(n_cycles=12, n_skip_cycles=6)
+    if cfg_i == 4:
+        over["n_traces"] = 3
+    wl = wlm.scaled(wlm.config(cfg_i), **over)
+    T = wl["n_traces"]
+    truths = None if wl["truth"] is not None else wlm.pixel_truths(wl)
+    trace = oracle_trace(wl, truths=truths)
+    # (1, 5, 1): 626 chains on 592 workers, so chains also wait for a free worker
+    n = 20013 if (cfg_i, workers) == (1, 1) else T * (300 + 13)
+    params = wlm.draw_params(wl, n, seed=61)
+    z0v0 = wlm.draw_initial_states(wl, n, seed=62) if cfg_i == 1 else None
+    wp = wlm.scaled(wl, n_particles=77, n_iters=4)
+    out = {}
+    for queue in (1, 2):
+        afm.afm_set_option("queue", queue)
+        afm.afm_set_option("segs", segs)
+        afm.afm_set_option("workers", workers)
+        afm.afm_set_option("form", 1)           # the queue serves the throughput form
+        try:
+            out[queue] = _gpu_forward(afm, wl, params, trace, z0v0)
+            g = afm.afm_pso_invert(afm.bounds_from(wp), afm.swarm_from(wp), 3,
+                                   torch.as_tensor(trace, device="cuda"), afm.cfg_from(wp),
+                                   dump=True)
+            out[queue, "pso"] = g["dump"].cpu().numpy()
+        finally:
+            for name in ("queue", "segs", "workers", "form"):
+                afm.afm_set_option(name, 0)
+    assert np.array_equal(out[1], out[2])
+    assert np.array_equal(out[1, "pso"], out[2, "pso"])
+    Jo = _oracle_forward(wl, params, trace, z0v0)
+    assert rel_err(out[2], Jo).max() < TOL_F64
+
+
 @pytest.mark.parametrize("lanes", [1, 2, 8, 32])
 def test_latency_form_lanes_per_warp(afm, lanes):
     """Latency form with 1..32 particles per warp (the other lanes shadow them):
