@@ -366,49 +366,74 @@ int integrate_bpt(int64_t per, int block, int ppt, int variant, int lanes) {
   return variant == 1 ? blocks_per_trace(per, lanes) : blocks_per_trace(per, block * ppt);
 }
 
-// The FP64 integrate launch.  In the throughput form a batch of a few warps per
-// SM sub-partition goes through the segment queue (integrate_misfit_f64_q):
-// floor(r) + 1 persistent one-warp workers per sub-partition for r chains per
-// sub-partition, so that the spare worker slots rotate over the whole device.
-// Lock held.
-int run_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block,
-                      int variant, cudaStream_t st) {
-  const int64_t chains = (int64_t)blocks_per_trace(io.per, 32) * io.n_traces;
+// Segment-queue scheduling (integrate_misfit_f64_q / _f32_q) serves a batch of a
+// few warps of particles ("chains") per SM sub-partition: floor(r) + 1 persistent
+// one-warp workers per sub-partition for r chains per sub-partition, so that the
+// spare worker slots rotate over the whole device.  *use is false when the plain
+// kernel should run.  Lock held.
+int make_queue(int64_t per, int n_traces, int n_tiles, int T, bool eligible,
+               SegQueue* q, int* workers, bool* use, cudaStream_t st) {
+  const int64_t chains = (int64_t)blocks_per_trace(per, 32) * n_traces;
   const int64_t subparts = (int64_t)4 * g_n_sm;
-  bool use_q = (variant == 0 && block == 32 && g_opt_queue != 1 && chains < (1 << 20));
-  if (use_q && g_opt_queue == 0)
-    use_q = (2 * chains >= 3 * subparts && chains <= 6 * subparts && mc.n_tiles >= 64);
-  if (!use_q) {
-    LAUNCHED(launch_integrate_f64(mc, io, block, variant, st));
-    return AFM_OK;
-  }
+  *use = eligible && g_opt_queue != 1 && chains < (1 << 20);
+  if (*use && g_opt_queue == 0)
+    *use = (2 * chains >= 3 * subparts && chains <= 6 * subparts && n_tiles >= 64);
+  if (!*use) return AFM_OK;
   int per_sub = g_opt_workers > 0 ? g_opt_workers : (int)(chains / subparts) + 1;
   if (per_sub > 8) per_sub = 8;
-  int workers = (int)(per_sub * subparts);
-  if (workers > chains) workers = (int)chains;
-  SegQueue q;
-  // segments of about 450 steps (130 us at 3-4 warps per sub-partition: long
+  *workers = (int)(per_sub * subparts);
+  if (*workers > chains) *workers = (int)chains;
+  // segments of about 450 steps (130 us at 3-4 FP64 warps per sub-partition: long
   // against the 2-3 us a hand-over costs, short against the whole solve;
   // measured on configs[1]: 8 segments 16.4 ms, 32: 15.7, 115: 14.9, 400: 15.3)
-  int segs = g_opt_segs > 0 ? g_opt_segs : (mc.n_tiles * mc.T + 447) / 448;
-  if (segs > mc.n_tiles) segs = mc.n_tiles;
+  int segs = g_opt_segs > 0 ? g_opt_segs : (n_tiles * T + 447) / 448;
+  if (segs > n_tiles) segs = n_tiles;
   if (segs > 2047) segs = 2047;
   if (segs < 1) segs = 1;
-  q.tiles_per_seg = (mc.n_tiles + segs - 1) / segs;
-  q.n_segs = (mc.n_tiles + q.tiles_per_seg - 1) / q.tiles_per_seg;
-  q.n_chains = (int32_t)chains;
-  q.n_tasks = q.n_chains * q.n_segs;
-  q.timeout_cycles = 40000000000LL;  // ~20 s: only a corrupted queue gets there
-  const size_t slot_bytes = ((size_t)q.n_tasks * 4 + 255) & ~(size_t)255;
+  q->tiles_per_seg = (n_tiles + segs - 1) / segs;
+  q->n_segs = (n_tiles + q->tiles_per_seg - 1) / q->tiles_per_seg;
+  q->n_chains = (int32_t)chains;
+  q->n_tasks = q->n_chains * q->n_segs;
+  q->timeout_cycles = 40000000000LL;  // ~20 s: only a corrupted queue gets there
+  const size_t slot_bytes = ((size_t)q->n_tasks * 4 + 255) & ~(size_t)255;
   const size_t need = 256 + slot_bytes + (size_t)chains * 128 * 8;
   const bool fresh = need > g_ws.segq.cap;
   if (g_ws.segq.ensure(need))
     return fail(AFM_ECUDA, "cudaMalloc of the segment queue failed");
   if (fresh) CUDA_TRY(cudaMemsetAsync(g_ws.segq.p, 0, 256, st));
-  q.ctrl = (unsigned*)g_ws.segq.p;
-  q.slots = (int*)((char*)g_ws.segq.p + 256);
-  q.ckpt = (double*)((char*)g_ws.segq.p + 256 + slot_bytes);
-  LAUNCHED(launch_integrate_f64_q(mc, io, q, workers, st));
+  q->ctrl = (unsigned*)g_ws.segq.p;
+  q->slots = (int*)((char*)g_ws.segq.p + 256);
+  q->ckpt = (double*)((char*)g_ws.segq.p + 256 + slot_bytes);
+  return AFM_OK;
+}
+
+int run_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block,
+                      int variant, cudaStream_t st) {
+  SegQueue q;
+  int workers = 0;
+  bool use_q = false;
+  int rc = make_queue(io.per, io.n_traces, mc.n_tiles, mc.T, variant == 0 && block == 32,
+                      &q, &workers, &use_q, st);
+  if (rc) return rc;
+  if (use_q)
+    LAUNCHED(launch_integrate_f64_q(mc, io, q, workers, st));
+  else
+    LAUNCHED(launch_integrate_f64(mc, io, block, variant, st));
+  return AFM_OK;
+}
+
+int run_integrate_f32(const ModelConstsF32& mf, const IntegrateIO& io, int block,
+                      int ppt, cudaStream_t st) {
+  SegQueue q;
+  int workers = 0;
+  bool use_q = false;
+  int rc = make_queue(io.per, io.n_traces, mf.n_tiles, mf.T, ppt == 1 && block == 32, &q,
+                      &workers, &use_q, st);
+  if (rc) return rc;
+  if (use_q)
+    LAUNCHED(launch_integrate_f32_q(mf, io, q, workers, st));
+  else
+    LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
   return AFM_OK;
 }
 
@@ -499,9 +524,10 @@ int forward_locked(const double* params, int64_t P, const double* trace,
     io.J = pk.J;
   }
   if (f32)
-    LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
-  else if ((rc = run_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st)))
-    return rc;
+    rc = run_integrate_f32(mf, io, block, ppt, st);
+  else
+    rc = run_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st);
+  if (rc) return rc;
   if (pk.order) LAUNCHED(launch_pack_scatter(pk.order, pk.J, P, misfit, st));
   return release_ws(st);
 }
@@ -716,19 +742,20 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
       iof.J = pk.J;
       iof.mode = 0;
       if (f32)
-        LAUNCHED(launch_integrate_f32(mf, iof, block, ppt, st));
-      else if ((rc = run_integrate_f64(mc, iof, block,
-                                       pick_variant(iof.per, iof.n_traces, ppt), st)))
-        return rc;
+        rc = run_integrate_f32(mf, iof, block, ppt, st);
+      else
+        rc = run_integrate_f64(mc, iof, block, pick_variant(iof.per, iof.n_traces, ppt), st);
+      if (rc) return rc;
       LAUNCHED(launch_pack_scatter(pk.order, pk.J, PT, J, st));
       n_cand = blocks_per_trace(per, 128);
       LAUNCHED(launch_pso_best(D, per, T, J, x, pbest, pbestJ, (Cand*)g_ws.cand.p, 128,
                                st));
-    } else if (f32) {
-      LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
-    } else if ((rc = run_integrate_f64(mc, io, block,
-                                       pick_variant(io.per, io.n_traces, ppt), st))) {
-      return rc;
+    } else {
+      if (f32)
+        rc = run_integrate_f32(mf, io, block, ppt, st);
+      else
+        rc = run_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st);
+      if (rc) return rc;
     }
     LAUNCHED(launch_pso_gbest(
         box, D, T, n_cand, (Cand*)g_ws.cand.p, pbest, gbest, gbestJ,
@@ -861,9 +888,10 @@ int afm_pso_shard_eval(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   io.mode = 1;
   io.lanes = lanes;
   if (f32)
-    LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
-  else if ((rc = run_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st)))
-    return rc;
+    rc = run_integrate_f32(mf, io, block, ppt, st);
+  else
+    rc = run_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st);
+  if (rc) return rc;
   LAUNCHED(launch_pso_shard_cand(D, T, bpt, first_particle, (Cand*)g_ws.cand.p,
                                  pbest, cand_out, st));
   return release_ws(st);

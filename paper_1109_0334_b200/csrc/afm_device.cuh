@@ -233,6 +233,36 @@ __device__ __forceinline__ bool diverged_step(double d, const DivergeTest& T) {
   return false;
 }
 
+// One free-flight step taken speculatively, without the vote: new state in
+// (dn, wn); returns whether THIS lane's four stage gaps stayed above a0 and the
+// new gap is a positive number below the divergence filter (the conditions
+// under which rk4_step keeps a speculative step).  Same arithmetic as the
+// mode-0 branch of rk4_step.
+template <bool LAT>
+__device__ __forceinline__ bool free_step(const Particle64& P, double s0, double sh,
+                                          double s1, long long a0_bits,
+                                          const DivergeTest& T, double d, double w,
+                                          double& dn, double& wn) {
+  const double sixth = 1.0 / 6.0;
+  const double dw = d + w;
+  const double d2 = fma(0.5, w, d);
+  const double k1 = accel_free<LAT>(P, s0, d, w);
+  const double w2 = fma(0.5, k1, w);
+  const double k2 = accel_free<LAT>(P, sh, d2, w2);
+  const double w3 = fma(0.5, k2, w);
+  const double d3 = fma(0.5, w2, d);
+  const double k3 = accel_free<LAT>(P, sh, d3, w3);
+  const double d4 = d + w3;
+  const double k4 = accel_free<LAT>(P, s1, d4, w + k3);
+  const int m = min(min(__double2hiint(d), __double2hiint(d2)),
+                    min(__double2hiint(d3), __double2hiint(d4)));
+  const double t23 = k2 + k3;
+  const double s3 = k1 + t23;
+  dn = fma(s3, sixth, dw);
+  wn = fma((s3 + t23) + k4, sixth, w);
+  return (m > (int)(a0_bits >> 32)) & ((unsigned)__double2hiint(dn) < (unsigned)T.safe_hi);
+}
+
 template <int LAW, int PPT, bool LAT>
 __device__ __forceinline__ void rk4_step(const Particle64 (&P)[PPT], double s0,
                                          double sh, double s1,

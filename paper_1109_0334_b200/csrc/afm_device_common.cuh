@@ -57,6 +57,45 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
       : "memory");
 }
 
+// ---- segment queue of the *_q integrate kernels (see afm_kernels.cu) ----------
+__device__ __forceinline__ int ld_relaxed_s32(const int* p) {
+  int v;
+  asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_s32(int* p, int v) {
+  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// Next task of this worker: -1 when every task has been handed out, -2 after a
+// time-out (cannot happen unless the queue is corrupted; keeps a bug from
+// hanging the device).  Called by one lane.
+__device__ __forceinline__ int segq_pop(const SegQueue& q) {
+  const unsigned t = atomicAdd(&q.ctrl[0], 1u);
+  if (t >= (unsigned)q.n_tasks) return -1;
+  const long long t_start = clock64();
+  int v;
+  unsigned ns = 250;  // poll with back-off: a waiting worker shares its issue port
+  while ((v = ld_relaxed_s32(&q.slots[t])) < 0) {
+    __nanosleep(ns);
+    if (ns < 4000) ns *= 2;
+    if (clock64() - t_start > q.timeout_cycles) {
+      atomicExch(&q.ctrl[2], 1u);
+      return -2;
+    }
+  }
+  __threadfence();  // acquire: the chain's checkpoint was written before the slot
+  return v;
+}
+
+
+// Publish segment `seg` of `chain` at the tail of the queue.  The caller has
+// stored the chain's checkpoint, fenced and synchronised its warp.  One lane.
+__device__ __forceinline__ void segq_push(const SegQueue& q, int chain, int seg) {
+  const unsigned slot = atomicAdd(&q.ctrl[1], 1u);
+  st_release_s32(&q.slots[slot], (seg << 20) | chain);
+}
+
 __device__ __forceinline__ bool cand_less(double Ja, long long ia, double Jb,
                                           long long ib) {
   return (Ja < Jb) || (Ja == Jb && ia < ib);

@@ -129,7 +129,8 @@ struct IntegrateIO {
 struct SegQueue {
   int* slots;            // [n_tasks]  (segment << 20) | chain, or -1 = not yet published
   unsigned* ctrl;        // [0] consume ticket, [1] publish index, [2] time-out flag
-  double* ckpt;          // [n_chains][4][32]: d, w, J, diverged flag of a chain at rest
+  double* ckpt;          // [n_chains][4][32] doubles: d, w, J, diverged flag of a chain at
+                         // rest (FP32 kernel: [n_chains][8][32] floats, same size)
   long long timeout_cycles;
   int32_t n_chains;
   int32_t n_segs;
@@ -138,7 +139,10 @@ struct SegQueue {
 };
 
 int blocks_per_trace(int64_t per, int block);
+int launch_segq_init(const SegQueue& q, cudaStream_t st);
 int launch_integrate_f64_q(const ModelConsts& mc, const IntegrateIO& io,
+                           const SegQueue& q, int workers, cudaStream_t st);
+int launch_integrate_f32_q(const ModelConstsF32& mf, const IntegrateIO& io,
                            const SegQueue& q, int workers, cudaStream_t st);
 
 int launch_build_stream(const ModelConsts& mc, const double* trace, int n_traces,

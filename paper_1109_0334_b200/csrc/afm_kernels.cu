@@ -122,6 +122,41 @@ __device__ __forceinline__ void run_steps(const double4* sp, int i0, int i1,
                                           double (&J)[PPT], bool (&bad)[PPT],
                                           int& mode) {
   if (i0 >= i1) return;
+#ifdef AFM_PAIR
+  if (IsDmt<LAW>::value && PPT == 1) {
+    // DMT laws: in free flight two steps are taken speculatively before the
+    // warp votes once on both; a failed pair redoes its first step in the
+    // general form (rk4_step with mode 1), which also finds the way back.
+    int i = i0;
+    while (i < i1) {
+      if (mode == 0 && i + 1 < i1) {
+        const double4 ra = sp[i], rb = sp[i + 1];
+        double d1, w1, d2, w2;
+        const bool ok1 = free_step<LAT>(P[0], ra.x, ra.y, ra.z, a0_bits, T, d[0], w[0], d1, w1);
+        const bool ok2 = free_step<LAT>(P[0], rb.x, rb.y, rb.z, a0_bits, T, d1, w1, d2, w2);
+        if (__all_sync(0xffffffffu, ok1 & ok2)) {
+          if (WIN) {
+            const double e1 = d1 - ra.w, e2 = d2 - rb.w;
+            J[0] = fma(e2, e2, fma(e1, e1, J[0]));
+          }
+          d[0] = d2;
+          w[0] = w2;
+          i += 2;
+          continue;
+        }
+        mode = 1;
+      }
+      const double4 r = sp[i];
+      rk4_step<LAW, PPT, LAT>(P, r.x, r.y, r.z, a0_bits, d, w, mode, bad, T);
+      if (WIN) {
+        const double res = d[0] - r.w;
+        J[0] = fma(res, res, J[0]);
+      }
+      ++i;
+    }
+    return;
+  }
+#endif
   double4 r = sp[i0];
 #pragma unroll 2
   for (int i = i0; i < i1; ++i) {
@@ -305,15 +340,6 @@ __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
 // integrate_misfit_f64<LAW, MODE, 1, false>, step for step: results are
 // bit-identical.
 // ============================================================================
-__device__ __forceinline__ int ld_acquire_s32(const int* p) {
-  int v;
-  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-__device__ __forceinline__ void st_release_s32(int* p, int v) {
-  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-
 __global__ void segq_init_kernel(SegQueue q) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < q.n_tasks) q.slots[i] = (i < q.n_chains) ? i : -1;  // segment 0 of chain i
@@ -321,24 +347,6 @@ __global__ void segq_init_kernel(SegQueue q) {
     q.ctrl[0] = 0u;                    // head: next consume ticket
     q.ctrl[1] = (unsigned)q.n_chains;  // tail: next publish slot
   }
-}
-
-// Next task of this worker: -1 when every task has been handed out, -2 after a
-// time-out (cannot happen unless the queue is corrupted; keeps a bug from
-// hanging the device).  Called by one lane.
-__device__ __forceinline__ int segq_pop(const SegQueue& q) {
-  const unsigned t = atomicAdd(&q.ctrl[0], 1u);
-  if (t >= (unsigned)q.n_tasks) return -1;
-  const long long t_start = clock64();
-  int v;
-  while ((v = ld_acquire_s32(&q.slots[t])) < 0) {
-    __nanosleep(200);
-    if (clock64() - t_start > q.timeout_cycles) {
-      atomicExch(&q.ctrl[2], 1u);
-      return -2;
-    }
-  }
-  return v;
 }
 
 template <int LAW, int MODE>
@@ -460,10 +468,7 @@ integrate_misfit_f64_q(ModelConsts mc, IntegrateIO io, int blocks_per_tr, SegQue
       __stcg(ck + 96, bad[0] ? 1.0 : 0.0);
       __threadfence();
       __syncwarp();
-      if (tid == 0) {
-        const unsigned slot = atomicAdd(&q.ctrl[1], 1u);
-        st_release_s32(&q.slots[slot], ((seg + 1) << 20) | chain);
-      }
+      if (tid == 0) segq_push(q, chain, seg + 1);
       continue;
     }
 
@@ -843,6 +848,11 @@ int launch_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block
 #undef AFM_DISPATCH
 }
 
+int launch_segq_init(const SegQueue& q, cudaStream_t st) {
+  segq_init_kernel<<<(unsigned)((q.n_tasks + 255) / 256), 256, 0, st>>>(q);
+  return 1;
+}
+
 template <int LAW, int MODE>
 static int launch_integrate_q_t(const ModelConsts& mc, const IntegrateIO& io,
                                 const SegQueue& q, int workers, cudaStream_t st) {
@@ -851,7 +861,7 @@ static int launch_integrate_q_t(const ModelConsts& mc, const IntegrateIO& io,
   auto kern = integrate_misfit_f64_q<LAW, MODE>;
   if (smem > 48 * 1024)
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  segq_init_kernel<<<(unsigned)((q.n_tasks + 255) / 256), 256, 0, st>>>(q);
+  launch_segq_init(q, st);
   kern<<<(unsigned)workers, 32, smem, st>>>(mc, io, bpt, q);
   return 2;
 }

@@ -247,6 +247,209 @@ __global__ void integrate_misfit_f32(ModelConstsF32 mf, IntegrateIO io,
   }
 }
 
+// ============================================================================
+// Segment-queue form (see integrate_misfit_f64_q in afm_kernels.cu): persistent
+// one-warp workers take (chain, segment) tasks; between segments a chain rests as
+// { d hi, d lo, w hi, w lo, J hi, J lo, diverged } (the per-tile partial sum is
+// folded at every tile end, and the carried stream value s_prev is re-read from
+// the row before the segment).  Same arithmetic per particle as
+// integrate_misfit_f32<LAW, MODE, 1>: bit-identical results.
+// ============================================================================
+template <int LAW, int MODE>
+__global__ void __launch_bounds__(32)
+integrate_misfit_f32_q(ModelConstsF32 mf, IntegrateIO io, int blocks_per_tr, SegQueue q) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  float4* tile0 = reinterpret_cast<float4*>(smem_raw);
+  float4* tile1 = tile0 + mf.T;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tile1 + mf.T);
+  __shared__ Cand red[32];
+
+  const int tid = threadIdx.x;
+  if (tid == 0) {
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    fence_mbar_init();
+  }
+  __syncthreads();
+  uint32_t n_wait0 = 0u, n_wait1 = 0u;
+
+  Model32 M;
+  {
+    const float a6f = (float)mf.a6, b6f = (float)mf.b6;
+    M.nalpha = -a6f;
+    M.nbeta = -b6f;
+    M.nalpha_lo = -(float)(mf.a6 - (double)a6f);
+    M.nbeta_lo = -(float)(mf.b6 - (double)b6f);
+    M.a0 = (float)mf.a0;
+    M.d_safe = (float)mf.d_safe;
+    M.d_max = (float)mf.d_max;
+    M.d_min = (float)mf.d_min;
+  }
+
+  for (;;) {
+    int task = 0;
+    if (tid == 0) task = segq_pop(q);
+    task = __shfl_sync(0xffffffffu, task, 0);
+    if (task < 0) break;
+    const int chain = task & 0xfffff;
+    const int seg = task >> 20;
+    const int s = chain / blocks_per_tr;
+    const int64_t li = (int64_t)(chain - s * blocks_per_tr) * 32 + tid;
+    const bool active = li < io.per;
+    const int64_t gp = (int64_t)s * io.per + (active ? li : io.per - 1);
+    const float4* stream = reinterpret_cast<const float4*>(io.stream) + (int64_t)s * mf.N;
+    const int tile_begin = seg * q.tiles_per_seg;
+    const int tile_end = min(tile_begin + q.tiles_per_seg, mf.n_tiles);
+
+    if (tid == 0) {
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        const int tile = tile_begin + k;
+        if (tile < tile_end) {
+          const int st = tile & 1;
+          const int nb = tile * mf.T;
+          const uint32_t bytes = (uint32_t)min(mf.T, mf.N - nb) * 16u;
+          fence_proxy_async();
+          mbar_arrive_expect_tx(&bars[st], bytes);
+          bulk_g2s(st ? tile1 : tile0, stream + nb, bytes, &bars[st]);
+        }
+      }
+    }
+
+    double xloc[4];
+    Particle32 P[1];
+    State32 S[1];
+    float Jt[1], Jh, Jl, s_prev;
+    bool bad[1];
+    {
+      double th[4] = {0.0, 0.0, 0.0, 1.0};
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        xloc[j] = 0.0;
+        if (j < mf.D) {
+          const double xv = io.params[gp * mf.D + j];
+          xloc[j] = xv;
+          th[j] = (MODE == 1 && io.box.lg[j]) ? pow(10.0, xv) : xv;
+        }
+      }
+      P[0].c0 = P[0].c1 = P[0].c2 = P[0].c3 = P[0].thr = 0.0f;
+      if (LAW == AFM_LAW_DMT || LAW == AFM_LAW_DMT_VISC) {
+        const double kappa = th[0] * mf.c_vdw;
+        P[0].c0 = (float)(-kappa);
+        P[0].c1 = (float)(th[1] * mf.c_hertz);
+        P[0].c2 = (float)(-kappa / (mf.a0 * mf.a0));
+        if (LAW == AFM_LAW_DMT_VISC) P[0].c3 = (float)(-(th[2] * mf.c_visc));
+      } else if (LAW == AFM_LAW_LJ_EXP) {
+        P[0].c0 = (float)(th[0] * mf.c_rep);
+        P[0].c1 = (float)(-(th[1] * mf.c_att));
+        P[0].c2 = (float)(-(th[2] * mf.c_fad));
+        P[0].c3 = (float)(-mf.c_lam / th[3]);
+      } else if (LAW == AFM_LAW_HOOKE) {
+        P[0].c1 = (float)(th[0] * mf.c_ks);
+        P[0].thr = (float)(mf.zc - th[1] / mf.len);
+      } else if (LAW == AFM_LAW_KELVIN_VOIGT) {
+        P[0].c1 = (float)(th[0] * mf.c_ks);
+        P[0].c3 = (float)(-mf.a6 - th[1] * mf.c_zeta);
+      }
+    }
+    float* ck = reinterpret_cast<float*>(q.ckpt) + (int64_t)chain * 256 + tid;
+    if (seg == 0) {
+      double z0 = mf.z0, v0 = mf.v0;
+      if (io.z0v0 != nullptr) {
+        z0 = io.z0v0[2 * gp];
+        v0 = io.z0v0[2 * gp + 1];
+      }
+      const double d0 = z0 / mf.len + mf.zc;
+      const double w0 = v0 * mf.h / mf.len;
+      S[0].dh = (float)d0;
+      S[0].dl = (float)(d0 - (double)S[0].dh);
+      S[0].wh = (float)w0;
+      S[0].wl = (float)(w0 - (double)S[0].wh);
+      Jh = Jl = 0.0f;
+      bad[0] = false;
+      s_prev = (float)(mf.drive6 + mf.b6_zc);  // s6(0): cos(0) = 1
+    } else {
+      S[0].dh = __ldcg(ck);
+      S[0].dl = __ldcg(ck + 32);
+      S[0].wh = __ldcg(ck + 64);
+      S[0].wl = __ldcg(ck + 96);
+      Jh = __ldcg(ck + 128);
+      Jl = __ldcg(ck + 160);
+      bad[0] = __ldcg(ck + 192) != 0.0f;
+      s_prev = stream[tile_begin * mf.T - 1].y;  // s1 of the step before this segment
+    }
+    Jt[0] = 0.0f;
+    int mode = 0;
+
+    for (int tile = tile_begin; tile < tile_end; ++tile) {
+      const int st = tile & 1;
+      const float4* sp = st ? tile1 : tile0;
+      mbar_wait(&bars[st], (st ? n_wait1 : n_wait0) & 1u);
+      if (st) ++n_wait1; else ++n_wait0;
+      const int n_begin = tile * mf.T;
+      const int n_steps = min(mf.T, mf.N - n_begin);
+      const int k0 = max(0, min(n_steps, mf.n0 - n_begin));
+      run_steps32<LAW, 1, false>(sp, 0, k0, M, P, S, Jt, bad, mode, s_prev);
+      run_steps32<LAW, 1, true>(sp, k0, n_steps, M, P, S, Jt, bad, mode, s_prev);
+      {
+        float e;
+        two_sum32(Jh, Jt[0], Jh, e);
+        Jl = __fadd_rn(Jl, e);
+        Jt[0] = 0.0f;
+      }
+      __syncthreads();
+      if (tid == 0 && tile + 2 < tile_end) {
+        const int nb = (tile + 2) * mf.T;
+        const uint32_t bytes = (uint32_t)min(mf.T, mf.N - nb) * 16u;
+        fence_proxy_async();
+        mbar_arrive_expect_tx(&bars[st], bytes);
+        bulk_g2s(st ? tile1 : tile0, stream + nb, bytes, &bars[st]);
+      }
+    }
+
+    if (tile_end < mf.n_tiles) {
+      __stcg(ck, S[0].dh);
+      __stcg(ck + 32, S[0].dl);
+      __stcg(ck + 64, S[0].wh);
+      __stcg(ck + 96, S[0].wl);
+      __stcg(ck + 128, Jh);
+      __stcg(ck + 160, Jl);
+      __stcg(ck + 192, bad[0] ? 1.0f : 0.0f);
+      __threadfence();
+      __syncwarp();
+      if (tid == 0) segq_push(q, chain, seg + 1);
+      continue;
+    }
+
+    const double to_si = mf.len * mf.len;
+    double J = ((double)Jh + (double)Jl) * to_si;
+    bad[0] |= !(fabsf(S[0].wh) <= 3.0e38f);  // last velocity finite too (R12)
+    if (bad[0] || !(J == J)) J = CUDART_INF;
+    if (active) io.J[gp] = J;
+    if (MODE == 1) {
+      double pb = CUDART_INF;
+      long long idx = 0x7fffffffffffffffLL;
+      if (active) {
+        double pq = io.pbestJ[gp];
+        if (J < pq) {
+          pq = J;
+          io.pbestJ[gp] = J;
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            if (j < mf.D) io.pbest[gp * mf.D + j] = xloc[j];
+        }
+        pb = pq;
+        idx = gp;
+      }
+      block_argmin(pb, idx, red);
+      if (tid == 0) {
+        io.cand[chain].J = pb;
+        io.cand[chain].idx = idx;
+      }
+    }
+  }
+}
+
 // ---- launchers ------------------------------------------------------------------
 int launch_build_stream_f32(const ModelConstsF32& mf, const double* trace,
                             int n_traces, float* stream, cudaStream_t st) {
@@ -292,6 +495,38 @@ int launch_integrate_f32(const ModelConstsF32& mf, const IntegrateIO& io,
       return -1;
   }
 #undef AFM_DISPATCH32
+}
+
+template <int LAW, int MODE>
+static int launch_integrate32_q_t(const ModelConstsF32& mf, const IntegrateIO& io,
+                                  const SegQueue& q, int workers, cudaStream_t st) {
+  const int bpt = blocks_per_trace(io.per, 32);
+  const size_t smem = (size_t)mf.T * 16 * 2 + 64;
+  auto kern = integrate_misfit_f32_q<LAW, MODE>;
+  if (smem > 48 * 1024)
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  launch_segq_init(q, st);
+  kern<<<(unsigned)workers, 32, smem, st>>>(mf, io, bpt, q);
+  return 2;
+}
+
+int launch_integrate_f32_q(const ModelConstsF32& mf, const IntegrateIO& io,
+                           const SegQueue& q, int workers, cudaStream_t st) {
+#define AFM_DISPATCH32_Q(LAWV)                                                 \
+  case LAWV:                                                                   \
+    return io.mode ? launch_integrate32_q_t<LAWV, 1>(mf, io, q, workers, st)   \
+                   : launch_integrate32_q_t<LAWV, 0>(mf, io, q, workers, st);
+  switch (mf.law) {
+    AFM_DISPATCH32_Q(AFM_LAW_NONE)
+    AFM_DISPATCH32_Q(AFM_LAW_DMT)
+    AFM_DISPATCH32_Q(AFM_LAW_DMT_VISC)
+    AFM_DISPATCH32_Q(AFM_LAW_LJ_EXP)
+    AFM_DISPATCH32_Q(AFM_LAW_HOOKE)
+    AFM_DISPATCH32_Q(AFM_LAW_KELVIN_VOIGT)
+    default:
+      return -1;
+  }
+#undef AFM_DISPATCH32_Q
 }
 
 }  // namespace afm

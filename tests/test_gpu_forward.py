@@ -292,12 +292,13 @@ def test_warp_packing_changes_no_result(afm, precision):
         assert rel_err(out[2], Jo).max() < TOL_F64
 
 
+@pytest.mark.parametrize("precision", [0, 1])
 @pytest.mark.parametrize("cfg_i,segs,workers", [(1, 0, 0), (1, 5, 1), (2, 3, 8), (3, 7, 2),
                                                 (4, 1, 4), (4, 2047, 3)])
-def test_segment_queue_changes_no_result(afm, cfg_i, segs, workers):
+def test_segment_queue_changes_no_result(afm, cfg_i, segs, workers, precision):
     """afm_set_option("queue"): the time loop of every warp of particles is cut into
     segments handed between persistent workers through a ticket queue in global
-    memory (integrate_misfit_f64_q).  Misfits, and the swarm of an inversion, must be
+    memory (integrate_misfit_f64_q, integrate_misfit_f32_q).  Misfits, and the swarm of an inversion, must be
     bit-identical to the one-CTA-per-warp kernel: ragged particle counts, several
     traces, every segment count from one to one tile per segment, fewer workers than
     chains, all law families; and they must match the oracle."""
@@ -321,18 +322,19 @@ def test_segment_queue_changes_no_result(afm, cfg_i, segs, workers):
         afm.afm_set_option("workers", workers)
         afm.afm_set_option("form", 1)           # the queue serves the throughput form
         try:
-            out[queue] = _gpu_forward(afm, wl, params, trace, z0v0)
+            out[queue] = _gpu_forward(afm, wl, params, trace, z0v0, precision=precision)
             g = afm.afm_pso_invert(afm.bounds_from(wp), afm.swarm_from(wp), 3,
-                                   torch.as_tensor(trace, device="cuda"), afm.cfg_from(wp),
-                                   dump=True)
+                                   torch.as_tensor(trace, device="cuda"),
+                                   afm.cfg_from(wp, precision=precision), dump=True)
             out[queue, "pso"] = g["dump"].cpu().numpy()
         finally:
             for name in ("queue", "segs", "workers", "form"):
                 afm.afm_set_option(name, 0)
     assert np.array_equal(out[1], out[2])
     assert np.array_equal(out[1, "pso"], out[2, "pso"])
-    Jo = _oracle_forward(wl, params, trace, z0v0)
-    assert rel_err(out[2], Jo).max() < TOL_F64
+    if precision == 0:
+        Jo = _oracle_forward(wl, params, trace, z0v0)
+        assert rel_err(out[2], Jo).max() < TOL_F64
 
 
 @pytest.mark.parametrize("lanes", [1, 2, 8, 32])
