@@ -11,8 +11,9 @@ hot path over that batch: afm_forward_batch (a1-a4: parameter map, RK4, misfit)
 followed by afm_pso_step (a5-a7: personal best, global best, Eq. 8 move) on a
 65,536-particle swarm holding the same coordinates.  Inputs are synthetic
 (paper_1109_0334_b200.workloads, seeded), resident in HBM for `value`, and
-start in pinned host memory for `e2e` (afm_forward_batch_host: H2D of theta,
-z0v0 and trace, D2H of the misfits, inside the timed region).
+start in pinned host memory for `e2e` (afm_forward_batch_host +
+afm_pso_step_host: H2D of theta, z0v0, the trace, the misfits and the swarm
+state, D2H of the misfits and the swarm state, inside the timed region).
 
 N > 1 (torchrun): every rank runs its own batch of the same shape (different
 seeds); there is no data-path collective; scaling is
@@ -46,12 +47,43 @@ FLOPS_PER_STEP = {wlm.LAW_DMT: 57.0, wlm.LAW_DMT_VISC: 57.0, wlm.LAW_LJ_EXP: 93.
                   wlm.LAW_NONE: 49.0}
 # FP64 FMA peak of the lane model: 148 SMs x 64 lanes x 2 flops x clock
 N_SM, FP64_LANES, FP32_LANES = 148, 64, 128
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the integrate kernel
-# on configs[1], from the ncu --set full captures in profiles/r1c_cfg1_packed.md
-# (bytes), and the pipe utilisation ncu measured in the same captures.
-NCU_TRAFFIC = {"f64": 3762688 + 0, "f32": 2942720 + 0}
-NCU_PIPE = {"f64": {"sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active": 58.63},
-            "f32": {"sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active": 48.63}}
+# ncu figures of the dominant kernel (DRAM traffic per launch, pipe utilisation) are
+# read from the machine-written summary profiles/<PROFILE>_ncu.csv
+# (python -m paper_1109_0334_b200.ncu_summary) and reported only while the library
+# source is the one that summary was made from; otherwise they are null.
+PROFILE = {"f64": "r2_cfg1_f64", "f32": "r2_cfg1_f32"}
+PIPE_METRIC = {"f64": "sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_",
+               "f32": "sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_"}
+
+
+def _ncu_profile(precision):
+    """dict(traffic, pipe_active_pct, pipe_elapsed_pct, ...) from the committed ncu
+    summary of this precision's integrate kernel, or the reason it is not usable."""
+    import csv
+    from paper_1109_0334_b200 import ncu_summary
+    path = os.path.join(ROOT, "profiles", PROFILE[precision] + "_ncu.csv")
+    out = {"file": os.path.relpath(path, ROOT), "traffic": None, "pipe_active_pct": None,
+           "pipe_elapsed_pct": None}
+    if not os.path.exists(path):
+        out["status"] = "no summary committed"
+        return out
+    kv = dict((r[0], r[1]) for r in csv.reader(open(path)) if len(r) == 2)
+    out["kernel"] = kv.get("kernel", "").split("(")[0]
+    out["registers_per_thread"] = kv.get("launch__registers_per_thread")
+    sha = ncu_summary.source_sha()
+    if kv.get("source_sha") != sha:
+        out["status"] = "stale: summary made from source %s, running %s" % (
+            kv.get("source_sha"), sha)
+        return out
+    if ("integrate_misfit_%s" % precision) not in out["kernel"]:
+        out["status"] = "summary is of another kernel"
+        return out
+    out["status"] = "fresh"
+    out["traffic"] = int(float(kv["dram_bytes_read"]) + float(kv["dram_bytes_write"]))
+    out["pipe_active_pct"] = float(kv[PIPE_METRIC[precision] + "active"])
+    out["pipe_elapsed_pct"] = float(kv[PIPE_METRIC[precision] + "elapsed"])
+    out["kernel_ms_under_ncu"] = float(kv["duration_ms"])
+    return out
 
 
 def _peaks():
@@ -245,6 +277,9 @@ def run_ours(args):
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True),
            torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     afm.afm_reset_launch_count()
+    # the library brackets every integrate-kernel launch with its own event pair
+    # on the launching stream: roofline.kernel_ms is that kernel alone
+    afm.afm_set_option("kernel_events", 1)
     barrier()
     for i in range(args.steps):
         flush.zero_()                      # L2 flush between timed iterations (untimed)
@@ -256,25 +291,35 @@ def run_ours(args):
         ev[i][2].record()
     barrier()
     launches = afm.afm_launch_count()
+    kernel_times = afm.afm_kernel_times(min(args.steps, 64))
+    afm.afm_set_option("kernel_events", 0)
     step_ms = [e[0].elapsed_time(e[2]) for e in ev]
     fwd_ms = [e[0].elapsed_time(e[1]) for e in ev]
     total_ms = float(sum(step_ms))
     clocks = sampler.stop() if sampler else None
 
-    # ---- e2e: host buffers in, host misfits out, through the C ABI ----------
-    h_params = torch.as_tensor(params_np).pin_memory()
-    h_trace = torch.as_tensor(trace_np).pin_memory()
-    h_z0v0 = torch.as_tensor(z0v0_np).pin_memory()
-    h_out = torch.empty(P, dtype=torch.float64).pin_memory()
-    hp, ht, hz, ho = (h_params.numpy(), h_trace.numpy(), h_z0v0.numpy(), h_out.numpy())
-    afm.afm_forward_batch_host(hp, ht, cfg, z0v0=hz, misfit=ho)
+    # ---- e2e: the same step through the C ABI with HOST buffers: theta, z0v0, the
+    # trace, the misfits and the whole swarm state start and end in (pinned) host
+    # memory; every copy is inside the timed region -------------------------------
+    def pinned(a):
+        return torch.as_tensor(np.ascontiguousarray(a)).pin_memory().numpy()
+    hp, ht, hz = pinned(params_np), pinned(trace_np), pinned(z0v0_np)
+    ho = pinned(np.empty(P))
+    hst = {k: pinned(v.cpu().numpy()) for k, v in state.items()}
+
+    def e2e_step(it):
+        afm.afm_forward_batch_host(hp, ht, cfg, z0v0=hz, misfit=ho)
+        afm.afm_pso_step_host(bounds, swarm, D, 1, wl["pso_seed"], it, True, ho, hst)
+
+    e2e_step(0)
     barrier()
     t0 = time.perf_counter()
     for i in range(args.steps):
-        afm.afm_forward_batch_host(hp, ht, cfg, z0v0=hz, misfit=ho)
+        e2e_step(1 + i)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     finite = int(np.isfinite(ho).sum())
+    state_bytes = int(sum(v.nbytes for v in hst.values()))
 
     t = torch.tensor([total_ms, e2e_s * 1e3, float(sum(fwd_ms))], dtype=torch.float64,
                      device=dev)
@@ -288,11 +333,12 @@ def run_ours(args):
 
     if rank == 0:
         pk = _peaks()
-        kern_ms = fwd_total_ms / args.steps
+        kern_ms = float(np.mean(kernel_times))
         flops = FLOPS_PER_STEP[wl["law"]] * P * N
         achieved = flops / (kern_ms * 1e-3) / 1e12
         peak = pk["fp32_tflops"] if prec == afm.F32 else pk["fp64_tflops"]
         peak_meas = afm.afm_fma_peak(prec, 0.25)
+        ncu = _ncu_profile(args.precision)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup,
@@ -302,22 +348,34 @@ def run_ours(args):
             "config": {"workload": "configs[1]: 65536 DMT theta x 200 cycles x 256 RK4 "
                                    "steps, misfit over last 100 cycles (per GPU)",
                        "particles_per_gpu": P, "rk4_steps": N, "window": wl["n_window"],
-                       "step": "afm_forward_batch (with warp packing) + afm_pso_step",
+                       "step": "afm_forward_batch (warp packing, segment queue) + "
+                               "afm_pso_step",
                        "l2": "256 MB buffer zeroed between timed iterations"},
             "e2e": {"value": e2e_value, "unit": UNIT,
-                    "h2d_bytes_per_step": int(hp.nbytes + ht.nbytes + hz.nbytes),
-                    "d2h_bytes_per_step": int(ho.nbytes),
-                    "api": "afm_forward_batch_host", "finite_misfits": finite},
+                    "h2d_bytes_per_step": int(hp.nbytes + ht.nbytes + hz.nbytes + ho.nbytes
+                                              + state_bytes),
+                    "d2h_bytes_per_step": int(ho.nbytes + state_bytes),
+                    "api": "afm_forward_batch_host + afm_pso_step_host",
+                    "finite_misfits": finite},
             "gpu_launches": int(launches),
             "clocks": clocks,
-            "roofline": {"bound": "alu", "kernel": "integrate_misfit_%s" % args.precision,
+            "forward_ms": fwd_total_ms / args.steps,
+            "roofline": {"bound": "alu",
+                         "kernel": "integrate_misfit_%s_q" % args.precision,
                          "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                         "frac": achieved / peak, "traffic": NCU_TRAFFIC[args.precision],
-                         "traffic_source": "profiles/r1c_cfg1_packed.md (ncu --set full, one launch)",
-                         "algorithmic_bytes": int(P * (8 * D + 16 + 8) + N * 32),
-                         "ncu_pipe_utilisation_pct": NCU_PIPE[args.precision],
-                         "flops_per_particle_step": FLOPS_PER_STEP[wl["law"]],
+                         "frac": achieved / peak,
                          "kernel_ms": kern_ms,
+                         "kernel_ms_source": "CUDA events recorded by the library around "
+                                             "each integrate launch on its stream, mean of "
+                                             "%d timed launches" % len(kernel_times),
+                         "flops_per_particle_step": FLOPS_PER_STEP[wl["law"]],
+                         "algorithmic_bytes": int(P * (8 * D + 16 + 8) + N * 32),
+                         "traffic": ncu["traffic"],
+                         "frac_pipe_active": (None if ncu["pipe_active_pct"] is None
+                                              else ncu["pipe_active_pct"] / 100.0),
+                         "frac_pipe_elapsed": (None if ncu["pipe_elapsed_pct"] is None
+                                               else ncu["pipe_elapsed_pct"] / 100.0),
+                         "ncu": ncu,
                          "peak_source": "lane model 148 SM x %d lanes x 2 x %s (%s)" % (
                              FP32_LANES if prec == afm.F32 else FP64_LANES,
                              pk["clock_mhz"], pk["clock_source"]),
@@ -335,11 +393,31 @@ def run_ours(args):
                 "sample": "%d of 65536 particles x %d RK4 steps, single thread, %.1f s"
                           % (n_s, N, dt),
                 "host_cores": os.cpu_count()}
+            out["north_star_targets"] = _targets(out, ncu, args.precision)
         print(json.dumps(out))
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
     return 0
+
+
+def _targets(out, ncu, precision):
+    """BASELINE.json:north_star's three targets as plain pass/fail (None: not
+    measured by this run)."""
+    ex = out.get("extras", {})
+    other = _ncu_profile("f32" if precision == "f64" else "f64")
+    by = {precision: ncu, ("f32" if precision == "f64" else "f64"): other}
+
+    def pipe(p, bar):
+        v = by[p]["pipe_active_pct"]
+        return {"pipe_active_pct": v, "pipe_elapsed_pct": by[p]["pipe_elapsed_pct"],
+                "bar_pct": bar, "met": None if v is None else bool(v >= bar),
+                "source": by[p]["file"], "status": by[p]["status"]}
+    ms = ex.get("cfg2_inversion_ms")
+    return {"fp64_pipe_ge_60pct_configs1": pipe("f64", 60.0),
+            "fp32_pipe_ge_50pct_configs1": pipe("f32", 50.0),
+            "configs2_inversion_lt_100ms": {"ms": ms, "met": None if ms is None
+                                            else bool(ms < 100.0)}}
 
 
 def _event_ms(torch, fn, reps):
@@ -354,13 +432,31 @@ def _event_ms(torch, fn, reps):
     return e0.elapsed_time(e1) / reps
 
 
+def _wall_ms(fn, warmups, runs):
+    """Host wall clock, call to return: `warmups` untimed calls, then the median and
+    the best of `runs` timed ones (SURVEY.md 8(d) "Timing").  Returns (median, best,
+    last result)."""
+    r = None
+    for _ in range(warmups):
+        r = fn()
+    ts = []
+    for _ in range(runs):
+        t0 = time.perf_counter()
+        r = fn()
+        ts.append((time.perf_counter() - t0) * 1e3)
+    return float(np.median(ts)), float(min(ts)), r
+
+
 def extras(afm, torch, dev, main_prec):
     """Secondary figures of BASELINE.json:metric (not the headline): measured FMA
-    peaks, configs[1] in the other precision, one forward batch of configs[3]
-    and [4] at full size, and the inversion wall time (host clock, call to
-    return) of configs[0] and [2]."""
+    peaks, configs[1] in the other precision, one forward batch and the full
+    inversion of configs[3] and [4] at full size, and the inversion wall time (host
+    clock, call to return, median of 5 after 3 warm-ups) of configs[0] and [2]."""
     ex = {"fma_peak_measured_tflops": {"f64": afm.afm_fma_peak(afm.F64, 0.25),
-                                       "f32": afm.afm_fma_peak(afm.F32, 0.25)}}
+                                       "f32": afm.afm_fma_peak(afm.F32, 0.25)},
+          "timing": "inversions: host wall clock, call to return; cfg0/cfg2: 3 warm-ups, "
+                    "median of 5; cfg3/cfg4 full inversions: 1 warm-up, median of 3 "
+                    "(cfg3 f64: 1 run)"}
 
     def trace_of(wl, truths=None):
         cfg = afm.cfg_from(wl)
@@ -369,6 +465,9 @@ def extras(afm, torch, dev, main_prec):
         rows = [afm.afm_trajectory(tl[s], cfg, wl["z0"], wl["v0"])[0][-wl["n_window"]:]
                 for s in range(T)]
         return torch.as_tensor(np.stack(rows) + wlm.trace_noise(wl), device=dev)
+
+    def rel(r, wl):
+        return [float(abs(a - t) / abs(t)) for a, t in zip(r["theta_star"][0], wl["truth"])]
 
     # configs[1] in the other precision (kernel only, CUDA events)
     wl = wlm.config(1)
@@ -385,7 +484,8 @@ def extras(afm, torch, dev, main_prec):
     ex["cfg1_%s_forward_ms" % name] = ms
     ex["cfg1_%s_particle_steps_per_s" % name] = P * wl["n_steps"] / (ms * 1e-3)
 
-    # one full-size forward batch of configs[3] (both precisions) and configs[4]
+    # configs[3] (both precisions) and configs[4]: one full-size forward batch and the
+    # full inversion, measured (not extrapolated)
     for ci, precs in ((3, (afm.F64, afm.F32)), (4, (afm.F64,))):
         wl = wlm.config(ci)
         T, per = wl["n_traces"], wl["swarm"]["n_particles"]
@@ -393,6 +493,7 @@ def extras(afm, torch, dev, main_prec):
         tr = trace_of(wl, truths)
         params = torch.as_tensor(wlm.draw_params(wl, T * per, seed=1), device=dev)
         out = torch.empty(T * per, dtype=torch.float64, device=dev)
+        b, sw = afm.bounds_from(wl), afm.swarm_from(wl)
         for prec in precs:
             cfg = afm.cfg_from(wl, precision=prec)
             ms = _event_ms(torch, lambda: afm.afm_forward_batch(params, tr, cfg,
@@ -401,51 +502,54 @@ def extras(afm, torch, dev, main_prec):
             ex["cfg%d_%s_batch_ms" % (ci, name)] = ms
             ex["cfg%d_%s_particle_steps_per_s" % (ci, name)] = \
                 T * per * wl["n_steps"] / (ms * 1e-3)
-            ex["cfg%d_%s_full_inversion_s_extrapolated" % (ci, name)] = \
-                ms * 1e-3 * wl["swarm"]["n_iters"]
+            slow = (ci == 3 and prec == afm.F64)
+            med, best, r = _wall_ms(lambda: afm.afm_pso_invert(b, sw, wl["pso_seed"], tr, cfg),
+                                    0 if slow else 1, 1 if slow else 3)
+            ex["cfg%d_%s_full_inversion_s" % (ci, name)] = med * 1e-3
+            ex["cfg%d_%s_full_inversion_particle_steps_per_s" % (ci, name)] = \
+                float(T) * per * wl["n_steps"] * sw.n_iters / (med * 1e-3)
+            if wl["truth"] is not None:
+                ex["cfg%d_%s_theta_star_rel_err_vs_truth" % (ci, name)] = rel(r, wl)
 
     for ci in (0, 2):
         wl = wlm.config(ci)
         cfg = afm.cfg_from(wl)
         trace = trace_of(wl)
         b, s = afm.bounds_from(wl), afm.swarm_from(wl)
-        afm.afm_pso_invert(b, s, wl["pso_seed"], trace, cfg)       # warm-up
-        t0 = time.perf_counter()
-        r = afm.afm_pso_invert(b, s, wl["pso_seed"], trace, cfg)
-        ms = (time.perf_counter() - t0) * 1e3
+        med, best, r = _wall_ms(lambda: afm.afm_pso_invert(b, s, wl["pso_seed"], trace, cfg),
+                                3, 5)
         units = wl["swarm"]["n_particles"] * wl["swarm"]["n_iters"] * wl["n_steps"]
-        ex["cfg%d_inversion_ms" % ci] = ms
-        ex["cfg%d_particle_steps_per_s" % ci] = units / (ms * 1e-3)
-        ex["cfg%d_theta_star_rel_err_vs_truth" % ci] = [
-            float(abs(a - t) / abs(t)) for a, t in zip(r["theta_star"][0], wl["truth"])]
+        ex["cfg%d_inversion_ms" % ci] = med
+        ex["cfg%d_inversion_ms_best" % ci] = best
+        ex["cfg%d_particle_steps_per_s" % ci] = units / (med * 1e-3)
+        ex["cfg%d_theta_star_rel_err_vs_truth" % ci] = rel(r, wl)
         if ci == 2:
-            # the paper's stopping rule is a cost cutoff; here
-            # the cutoff is the noise energy of the trace, W sigma^2 + 3 sd
+            # the paper's stopping rule is a cost cutoff (DESIGN.md
+            # R24); here the cutoff is the noise energy of the trace, W sigma^2 + 3 sd.
+            # tests/test_gpu_full_size.py replays this run against the oracle (same
+            # number of batches, same theta*).
             W, sg = wl["n_window"], wl["sigma"]
             jt = W * sg * sg * (1.0 + 3.0 * (2.0 / W) ** 0.5)
             sc = afm.swarm_from(wl, j_target=jt)
-            afm.afm_pso_invert(b, sc, wl["pso_seed"], trace, cfg)
-            t0 = time.perf_counter()
-            r = afm.afm_pso_invert(b, sc, wl["pso_seed"], trace, cfg)
-            ex["cfg2_time_to_cutoff_ms"] = (time.perf_counter() - t0) * 1e3
+            med, best, r = _wall_ms(
+                lambda: afm.afm_pso_invert(b, sc, wl["pso_seed"], trace, cfg), 3, 5)
+            ex["cfg2_time_to_cutoff_ms"] = med
             ex["cfg2_batches_to_cutoff"] = int(r["n_iters_done"])
-            ex["cfg2_cutoff_theta_star_rel_err_vs_truth"] = [
-                float(abs(a - t) / abs(t)) for a, t in zip(r["theta_star"][0], wl["truth"])]
+            ex["cfg2_cutoff_theta_star_rel_err_vs_truth"] = rel(r, wl)
             # the same inversion with a swarm that fills the machine: 1 024 particles
             # are 32 warps on 592 SM sub-partitions, and a batch of 16 384 takes the
             # same time (the time loop is a latency chain), so the swarm can be 16x
-            # wider for free and needs far fewer batches
+            # wider for free and needs far fewer batches.  NOT
+            # configs[2] as BASELINE.json states it: another computation, quoted as an
+            # observation only.
             for tag, kw in (("to_cutoff", dict(j_target=jt, n_particles=16384)),
                             ("30_batches", dict(n_particles=16384, n_iters=30))):
                 sc = afm.swarm_from(wl, **kw)
-                afm.afm_pso_invert(b, sc, wl["pso_seed"], trace, cfg)
-                t0 = time.perf_counter()
-                r = afm.afm_pso_invert(b, sc, wl["pso_seed"], trace, cfg)
-                ex["cfg2_wide16384_%s_ms" % tag] = (time.perf_counter() - t0) * 1e3
+                med, best, r = _wall_ms(
+                    lambda: afm.afm_pso_invert(b, sc, wl["pso_seed"], trace, cfg), 1, 3)
+                ex["cfg2_wide16384_%s_ms" % tag] = med
                 ex["cfg2_wide16384_%s_batches" % tag] = int(r["n_iters_done"])
-                ex["cfg2_wide16384_%s_theta_star_rel_err_vs_truth" % tag] = [
-                    float(abs(a - t) / abs(t))
-                    for a, t in zip(r["theta_star"][0], wl["truth"])]
+                ex["cfg2_wide16384_%s_theta_star_rel_err_vs_truth" % tag] = rel(r, wl)
     return ex
 
 

@@ -195,6 +195,16 @@ int afm_pso_step(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
                  double* x, double* v, double* pbest, double* pbestJ,
                  double* gbest, double* gbestJ, void* cuda_stream);
 
+/* afm_pso_step with the swarm state and the misfits in HOST memory: copies
+ * J, x, v, pbest, pbestJ, gbest, gbestJ to the device, steps, copies the six
+ * state arrays back and synchronises the stream (with afm_forward_batch_host the
+ * end-to-end step that bench.py times).  All pointers host. */
+int afm_pso_step_host(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                      int32_t n_dims, int32_t n_traces, uint64_t seed,
+                      int32_t iteration, int32_t do_move, const double* J,
+                      double* x, double* v, double* pbest, double* pbestJ,
+                      double* gbest, double* gbestJ, void* cuda_stream);
+
 /* Initial swarm (uniform positions and velocities in the box):
  * fills x, v, pbest [PT][D] and sets pbestJ [PT], gbestJ [n_traces] to +Inf,
  * gbest [n_traces][D] to the first particle of each trace.  Asynchronous. */
@@ -320,14 +330,14 @@ int afm_trajectory(const double* theta, const afm_cfg* cfg, double z0,
 int afm_fma_peak(int32_t precision, double seconds, double* tflops,
                  void* cuda_stream);
 
-/* Dispatch probe ("what bounds the FP64 kernel"): time per
- * DFMA warp-instruction per SM sub-partition, in ns, for
- *   mode 0: x = fma(x, a, b) with a, b reused;  1: three distinct 64-bit register
- *   operands;  2, 3: mode 1 plus 2 / 4 independent integer instructions per
- *   DFMA;  4: mode 1 with 16 of 32 lanes active,
- * at 1..8 resident warps per sub-partition.  Synchronous.  Not on the hot path. */
-int afm_dispatch_probe(int32_t mode, int32_t warps_per_subpartition,
-                       double* ns_per_dfma, void* cuda_stream);
+/* Measurement aid: after afm_set_option("kernel_events", 1)
+ * every launch of an integrate-and-misfit kernel (the dominant kernel of every
+ * compute call) is bracketed by a pair of CUDA events recorded on the stream it
+ * is launched on.  afm_kernel_times waits for the recorded launches and writes
+ * the durations of the most recent min(max_n, 64, launches recorded) of them,
+ * oldest first, in milliseconds, to ms (host); *n_out = how many.  Switching
+ * the option on or off resets the record. */
+int afm_kernel_times(double* ms, int32_t max_n, int32_t* n_out);
 
 /* Kernel launches enqueued by this library on the calling thread since the
  * last reset (bench.py's gpu_launches). */

@@ -23,10 +23,11 @@ OK, EINVAL, ECUDA, EUNSUPPORTED = 0, -1, -2, -3
 # every symbol include/afm.h declares (tests check the library exports them all)
 SYMBOLS = (
     "afm_forward_batch", "afm_forward_batch_host", "afm_pso_invert",
-    "afm_pso_invert_host", "afm_pso_step", "afm_pso_init",
+    "afm_pso_invert_host", "afm_pso_step", "afm_pso_step_host", "afm_pso_init",
+    "afm_kernel_times",
     "afm_pso_shard_init", "afm_pso_shard_eval", "afm_pso_shard_move",
     "afm_beam_modes", "afm_beam_forward_batch", "afm_beam_pso_invert",
-    "afm_beam_trajectory", "afm_philox4x32_10", "afm_trajectory", "afm_fma_peak", "afm_dispatch_probe",
+    "afm_beam_trajectory", "afm_philox4x32_10", "afm_trajectory", "afm_fma_peak",
     "afm_launch_count",
     "afm_reset_launch_count", "afm_set_option", "afm_last_error",
     "afm_version", "afm_shutdown",
@@ -112,6 +113,10 @@ def lib():
                                           C.POINTER(i32), vp]
         L.afm_pso_step.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), i32, i32,
                                    u64, i32, i32, dp, dp, dp, dp, dp, dp, dp, vp]
+        L.afm_pso_step_host.argtypes = L.afm_pso_step.argtypes
+        L.afm_pso_step_host.restype = C.c_int
+        L.afm_kernel_times.argtypes = [C.POINTER(C.c_double), i32, C.POINTER(i32)]
+        L.afm_kernel_times.restype = C.c_int
         L.afm_pso_init.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), i32, i32,
                                    u64, dp, dp, dp, dp, dp, dp, vp]
         L.afm_pso_shard_init.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), i32,
@@ -135,10 +140,9 @@ def lib():
         L.afm_trajectory.argtypes = [dp, C.POINTER(Cfg), C.c_double, C.c_double,
                                      dp, dp, vp]
         L.afm_fma_peak.argtypes = [i32, C.c_double, C.POINTER(C.c_double), vp]
-        L.afm_dispatch_probe.argtypes = [i32, i32, C.POINTER(C.c_double), vp]
-        L.afm_dispatch_probe.restype = C.c_int
         for name in ("afm_forward_batch", "afm_forward_batch_host", "afm_pso_invert",
-                     "afm_pso_invert_host", "afm_pso_step", "afm_pso_init",
+                     "afm_pso_invert_host", "afm_pso_step", "afm_pso_step_host", "afm_pso_init",
+    "afm_kernel_times",
                      "afm_philox4x32_10", "afm_trajectory", "afm_fma_peak",
                      "afm_pso_shard_init", "afm_pso_shard_eval",
                      "afm_pso_shard_move"):
@@ -346,6 +350,32 @@ def afm_pso_step(bounds, swarm, n_dims, n_traces, seed, iteration, do_move, J, s
     return st
 
 
+def afm_pso_step_host(bounds, swarm, n_dims, n_traces, seed, iteration, do_move, J, st,
+                      stream=None):
+    """afm_pso_step on HOST (numpy) state: st is a dict of contiguous float64 arrays
+    x, v, pbest [PT][D], pbestJ [PT], gbest [T][D], gbestJ [T], updated in place."""
+    for k in ("x", "v", "pbest", "pbestJ", "gbest", "gbestJ"):
+        a = st[k]
+        if not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.flags.c_contiguous):
+            raise TypeError("st[%r] must be a contiguous float64 numpy array" % k)
+    J = _host_f64(J)
+    _check(lib().afm_pso_step_host(C.byref(bounds), C.byref(swarm), n_dims, n_traces,
+                                   int(seed), int(iteration), int(bool(do_move)), _hptr(J),
+                                   _hptr(st["x"]), _hptr(st["v"]), _hptr(st["pbest"]),
+                                   _hptr(st["pbestJ"]), _hptr(st["gbest"]),
+                                   _hptr(st["gbestJ"]), _stream_ptr(stream)))
+    return st
+
+
+def afm_kernel_times(max_n=64):
+    """Durations (ms, oldest first) of the last integrate-kernel launches recorded
+    since afm_set_option("kernel_events", 1)."""
+    buf = (C.c_double * max_n)()
+    n = C.c_int32(0)
+    _check(lib().afm_kernel_times(buf, max_n, C.byref(n)))
+    return [buf[i] for i in range(n.value)]
+
+
 def afm_pso_shard_init(bounds, swarm, n_dims, n_traces, seed, first_particle,
                        stream=None):
     """Swarm state of a shard: swarm.n_particles local particles
@@ -505,14 +535,6 @@ def afm_fma_peak(precision, seconds=0.2, stream=None):
     out = C.c_double(0.0)
     _check(lib().afm_fma_peak(int(precision), float(seconds), C.byref(out),
                               _stream_ptr(stream)))
-    return out.value
-
-
-def afm_dispatch_probe(mode, warps_per_subpartition, stream=None):
-    """ns per DFMA warp-instruction per SM sub-partition (include/afm.h)."""
-    out = C.c_double(0.0)
-    _check(lib().afm_dispatch_probe(int(mode), int(warps_per_subpartition),
-                                    C.byref(out), _stream_ptr(stream)))
     return out.value
 
 

@@ -61,6 +61,27 @@ int g_opt_segs = 0;   // 0 = auto (~450 steps each): time segments per chain of 
 int g_opt_workers = 0;  // 0 = auto: queue workers per SM sub-partition
 int g_n_sm = 148;
 
+// afm_set_option("kernel_events", 1): every launch of an integrate kernel is
+// bracketed by a pair of CUDA events on its own stream (bench.py's
+// roofline.kernel_ms: the duration of the dominant kernel alone, measured live).
+constexpr int kMaxKernelEvents = 64;
+int g_opt_kernel_events = 0;
+cudaEvent_t g_kev[kMaxKernelEvents][2];
+bool g_kev_made = false;
+int64_t g_kev_count = 0;  // launches recorded since the option was switched on
+
+int kev_record(int which, cudaStream_t st) {
+  if (!g_opt_kernel_events) return AFM_OK;
+  if (!g_kev_made) {
+    for (int i = 0; i < kMaxKernelEvents; ++i)
+      for (int j = 0; j < 2; ++j) CUDA_TRY(cudaEventCreate(&g_kev[i][j]));
+    g_kev_made = true;
+  }
+  CUDA_TRY(cudaEventRecord(g_kev[g_kev_count % kMaxKernelEvents][which], st));
+  if (which == 1) ++g_kev_count;
+  return AFM_OK;
+}
+
 // ---- grow-only device workspace ------------------------------------------------
 struct Buffer {
   void* p = nullptr;
@@ -93,6 +114,7 @@ struct Workspace {
   Buffer swarm;                        // x, v, pbest, J, pbestJ, gbest, ...
   Buffer cand;                         // block candidates
   Buffer h_params, h_trace, h_z0v0, h_misfit;  // staging for the *_host calls
+  Buffer h_state;                      // staging for afm_pso_step_host
   Buffer scratch;                      // theta for afm_trajectory
   Buffer sort;                         // warp-packing keys, order, radix-sort temp
   Buffer segq;                         // segment queue: control words, slots, checkpoints
@@ -415,11 +437,12 @@ int run_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block,
   int rc = make_queue(io.per, io.n_traces, mc.n_tiles, mc.T, variant == 0 && block == 32,
                       &q, &workers, &use_q, st);
   if (rc) return rc;
+  if ((rc = kev_record(0, st))) return rc;
   if (use_q)
     LAUNCHED(launch_integrate_f64_q(mc, io, q, workers, st));
   else
     LAUNCHED(launch_integrate_f64(mc, io, block, variant, st));
-  return AFM_OK;
+  return kev_record(1, st);
 }
 
 int run_integrate_f32(const ModelConstsF32& mf, const IntegrateIO& io, int block,
@@ -430,11 +453,12 @@ int run_integrate_f32(const ModelConstsF32& mf, const IntegrateIO& io, int block
   int rc = make_queue(io.per, io.n_traces, mf.n_tiles, mf.T, ppt == 1 && block == 32, &q,
                       &workers, &use_q, st);
   if (rc) return rc;
+  if ((rc = kev_record(0, st))) return rc;
   if (use_q)
     LAUNCHED(launch_integrate_f32_q(mf, io, q, workers, st));
   else
     LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
-  return AFM_OK;
+  return kev_record(1, st);
 }
 
 // After a stream synchronisation: did a queue worker give up waiting (a
@@ -1267,29 +1291,71 @@ int afm_fma_peak(int32_t precision, double seconds, double* tflops,
   return release_ws(st);
 }
 
-int afm_dispatch_probe(int32_t mode, int32_t warps_per_subpartition,
-                       double* ns_per_dfma, void* cuda_stream) {
-  if (!ns_per_dfma) return fail(AFM_EINVAL, "ns_per_dfma is NULL");
-  if (mode < 0 || mode > 4) return fail(AFM_EINVAL, "mode must be 0..4");
-  if (warps_per_subpartition < 1 || warps_per_subpartition > 8)
-    return fail(AFM_EINVAL, "warps_per_subpartition must be 1..8");
-  int rc = check_device();
-  if (rc) return rc;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+int afm_kernel_times(double* ms, int32_t max_n, int32_t* n_out) {
+  if (!ms || !n_out || max_n < 0) return fail(AFM_EINVAL, "NULL pointer or negative max_n");
   std::lock_guard<std::mutex> lock(g_ws.mu);
-  if ((rc = acquire_ws(st))) return rc;
-  if (g_ws.scratch.ensure(1024)) return fail(AFM_ECUDA, "cudaMalloc failed");
-  double h[64];
-  for (int i = 0; i < 64; ++i) h[i] = 0.999 + 1e-6 * i;
-  CUDA_TRY(cudaMemcpyAsync(g_ws.scratch.p, h, sizeof(h), cudaMemcpyHostToDevice, st));
+  int64_t n = g_kev_count < kMaxKernelEvents ? g_kev_count : kMaxKernelEvents;
+  if (n > max_n) n = max_n;
+  // oldest first: launches g_kev_count - n .. g_kev_count - 1
+  for (int64_t k = 0; k < n; ++k) {
+    const int64_t slot = (g_kev_count - n + k) % kMaxKernelEvents;
+    CUDA_TRY(cudaEventSynchronize(g_kev[slot][1]));
+    float t = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&t, g_kev[slot][0], g_kev[slot][1]));
+    ms[k] = (double)t;
+  }
+  *n_out = (int32_t)n;
+  return AFM_OK;
+}
+
+int afm_pso_step_host(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                      int32_t n_dims, int32_t n_traces, uint64_t seed,
+                      int32_t iteration, int32_t do_move, const double* J, double* x,
+                      double* v, double* pbest, double* pbestJ, double* gbest,
+                      double* gbestJ, void* cuda_stream) {
+  if (n_dims < 1 || n_dims > 4) return fail(AFM_EINVAL, "n_dims must be 1..4");
+  if (n_traces < 1) return fail(AFM_EINVAL, "n_traces must be >= 1");
+  int rc = validate_swarm(swarm);
+  if (rc) return rc;
+  if (!J || !x || !v || !pbest || !pbestJ || !gbest || !gbestJ)
+    return fail(AFM_EINVAL, "NULL swarm array");
+  if ((rc = check_device())) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t PT = (size_t)swarm->n_particles * n_traces;
+  const size_t nd = PT * n_dims, nt = (size_t)n_traces;
+  // device image: J, x, v, pbest, pbestJ, gbest, gbestJ
+  const size_t total = PT + 3 * nd + PT + nt * n_dims + nt;
+  double* base;
+  {
+    std::lock_guard<std::mutex> lock(g_ws.mu);
+    if ((rc = acquire_ws(st))) return rc;
+    if (g_ws.h_state.ensure(total * 8))
+      return fail(AFM_ECUDA, "cudaMalloc of the swarm staging buffer failed");
+    base = (double*)g_ws.h_state.p;
+    g_ws.last_stream = st;
+  }
+  double* dJ = base;
+  double* dx = dJ + PT;
+  double* dv = dx + nd;
+  double* dpb = dv + nd;
+  double* dpbJ = dpb + nd;
+  double* dg = dpbJ + PT;
+  double* dgJ = dg + nt * n_dims;
+  const struct { double* d; const double* h; size_t n; } in[] = {
+      {dJ, J, PT}, {dx, x, nd}, {dv, v, nd}, {dpb, pbest, nd},
+      {dpbJ, pbestJ, PT}, {dg, gbest, nt * n_dims}, {dgJ, gbestJ, nt}};
+  for (const auto& c : in)
+    CUDA_TRY(cudaMemcpyAsync(c.d, c.h, c.n * 8, cudaMemcpyHostToDevice, st));
+  rc = afm_pso_step(bounds, swarm, n_dims, n_traces, seed, iteration, do_move, dJ, dx, dv,
+                    dpb, dpbJ, dg, dgJ, cuda_stream);
+  if (rc) return rc;
+  const struct { double* h; const double* d; size_t n; } out[] = {
+      {x, dx, nd}, {v, dv, nd}, {pbest, dpb, nd}, {pbestJ, dpbJ, PT},
+      {gbest, dg, nt * n_dims}, {gbestJ, dgJ, nt}};
+  for (const auto& c : out)
+    CUDA_TRY(cudaMemcpyAsync(c.h, c.d, c.n * 8, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
-  double* base = (double*)g_ws.scratch.p;
-  const int n = launch_dispatch_probe(mode, warps_per_subpartition, g_n_sm, base,
-                                      base + 64, ns_per_dfma, st);
-  if (n < 0) return fail(AFM_ECUDA, "cudaEventCreate failed");
-  g_launches += n;
-  CUDA_TRY(cudaGetLastError());
-  return release_ws(st);
+  return AFM_OK;
 }
 
 int64_t afm_launch_count(void) { return g_launches; }
@@ -1323,6 +1389,12 @@ int afm_set_option(const char* name, int64_t value) {
   if (!strcmp(name, "pack")) {
     if (value < 0 || value > 2) return fail(AFM_EINVAL, "pack must be 0, 1 or 2");
     g_opt_pack = (int)value;
+    return AFM_OK;
+  }
+  if (!strcmp(name, "kernel_events")) {
+    if (value < 0 || value > 1) return fail(AFM_EINVAL, "kernel_events must be 0 or 1");
+    g_opt_kernel_events = (int)value;
+    g_kev_count = 0;
     return AFM_OK;
   }
   if (!strcmp(name, "queue")) {
@@ -1361,6 +1433,7 @@ void afm_shutdown(void) {
   g_ws.h_trace.release();
   g_ws.h_z0v0.release();
   g_ws.h_misfit.release();
+  g_ws.h_state.release();
   g_ws.scratch.release();
   g_ws.sort.release();
   g_ws.segq.release();

@@ -22,6 +22,8 @@
 
 namespace afm {
 
+constexpr int kPadRows = kPadBytes / 32;  // pad rows after each stage of the tile ring
+
 // ---- initialisation -------------------------------------------------------------
 // Eq. 7 with "+ exp(-2 beta L)" in the denominator (R22).
 __device__ __forceinline__ double beam_G(double bL) {
@@ -197,8 +199,8 @@ __global__ void beam_integrate_f64(BeamConsts bc, BeamModeConsts mo, IntegrateIO
                                    int blocks_per_tr) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double4* tile0 = reinterpret_cast<double4*>(smem_raw);
-  double4* tile1 = tile0 + bc.T;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(tile1 + bc.T);
+  double4* tile1 = tile0 + (bc.T + kPadRows);  // one pad row per stage for the row fetched ahead
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tile1 + (bc.T + kPadRows));
   __shared__ Cand red[32];
 
   const int tid = threadIdx.x;
@@ -209,6 +211,8 @@ __global__ void beam_integrate_f64(BeamConsts bc, BeamModeConsts mo, IntegrateIO
   const double* stream = io.stream + (int64_t)s * bc.N * 4;
 
   if (tid == 0) {
+    tile0[bc.T] = make_double4(0.0, 0.0, 0.0, 0.0);
+    tile1[bc.T] = make_double4(0.0, 0.0, 0.0, 0.0);
     mbar_init(&bars[0], 1);
     mbar_init(&bars[1], 1);
     fence_mbar_init();
@@ -343,7 +347,13 @@ static int launch_beam_t(const BeamConsts& bc, const BeamModeConsts& mo,
                          const IntegrateIO& io, int block, cudaStream_t st) {
   const int bpt = blocks_per_trace(io.per, block);
   const unsigned grid = (unsigned)(bpt * io.n_traces);
-  const size_t smem = (size_t)bc.T * 32 * 2 + 64;
+  const size_t smem = (size_t)(bc.T + kPadRows) * 32 * 2 + 64;
+  if (smem > 48 * 1024) {  // afm_set_option("tile") above 767 steps
+    cudaFuncSetAttribute(beam_integrate_f64<M, 1>,
+                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(beam_integrate_f64<M, 0>,
+                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  }
   if (io.mode == 1)
     beam_integrate_f64<M, 1><<<grid, block, smem, st>>>(bc, mo, io, bpt);
   else

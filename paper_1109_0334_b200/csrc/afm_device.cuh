@@ -124,10 +124,16 @@ __device__ __forceinline__ bool ge_pos(double d, long long a0_bits) {
 
 // Free-flight (d >= a0) side of the DMT laws, and the whole of law NONE when
 // c0 = 0 is skipped by the caller.
-template <bool LAT>
+// WFOLD (latency form only): the stage velocity is already known when the
+// reciprocal chain starts (stages 1 and 3: w, and w3 which comes from the short
+// k2 path), so -alpha w joins the constant term and the stage ends with the one
+// FMA after the correction polynomial; in stages 2 and 4 w is the last operand to
+// arrive and enters through a final FMA.
+template <bool LAT, bool WFOLD = false>
 __device__ __forceinline__ double accel_free(const Particle64& P, double s,
                                              double d, double w) {
   const double b0 = fma(P.nbeta, d, s);
+  if (LAT && WFOLD) return vdw_plus(P.c0, d * d, fma(P.nalpha, w, b0));
   if (LAT) return fma(P.nalpha, w, vdw_plus(P.c0, d * d, b0));
   return fma(P.nalpha, w, fma(P.c0, rcp_fast(d * d), b0));
 }
@@ -141,14 +147,15 @@ __device__ __forceinline__ double accel_free(const Particle64& P, double s,
 // (Measured and rejected: one shared rsqrt chain on a per-lane selected argument
 // with selected tail coefficients -- 14 instead of 19 FP64 instructions per
 // stage, but ten more 32-bit selects; 19.8 ms against 19.1 ms on configs[1].)
-template <int LAW, bool LAT>
+template <int LAW, bool LAT, bool WFOLD = false>
 __device__ __forceinline__ double accel_both(const Particle64& P, double s,
                                              double d, double w,
                                              long long a0_bits) {
   const double b0 = fma(P.nbeta, d, s);
   const double g_free =
-      LAT ? fma(P.nalpha, w, vdw_plus(P.c0, d * d, b0))
-          : fma(P.nalpha, w, fma(P.c0, rcp_fast(d * d), b0));
+      (LAT && WFOLD) ? vdw_plus(P.c0, d * d, fma(P.nalpha, w, b0))
+      : LAT          ? fma(P.nalpha, w, vdw_plus(P.c0, d * d, b0))
+                     : fma(P.nalpha, w, fma(P.c0, rcp_fast(d * d), b0));
   const double del = P.a0 - d;
   const double sq = sqrt_fast(del);
   const double part = fma(P.c1 * del, sq, P.c2 + b0);
@@ -233,34 +240,58 @@ __device__ __forceinline__ bool diverged_step(double d, const DivergeTest& T) {
   return false;
 }
 
-// One free-flight step taken speculatively, without the vote: new state in
-// (dn, wn); returns whether THIS lane's four stage gaps stayed above a0 and the
-// new gap is a positive number below the divergence filter (the conditions
-// under which rk4_step keeps a speculative step).  Same arithmetic as the
-// mode-0 branch of rk4_step.
+// Stage-3 position and the RK4 combination.  Throughput form: the textbook
+// association with the fewest operations.  Latency form: the same sums associated
+// so that the loop-carried chain d_n -> k1 -> d3 -> k3 -> d_{n+1} is as short as it
+// can be: d3 = d2 + k1/4 (= d + w2/2 without waiting for w2) and
+// d_{n+1} = [d + w + (k1 + k2)/6] + k3/6 (one FMA after k3); two more additions,
+// three fewer dependent operations per step (8.1 cycles each).
+template <bool LAT>
+__device__ __forceinline__ double stage3_gap(double d, double d2, double k1, double w2) {
+  return LAT ? fma(0.25, k1, d2) : fma(0.5, w2, d);
+}
+template <bool LAT>
+__device__ __forceinline__ void rk4_combine(double dw, double w, double k1, double k2,
+                                            double k3, double k4, double& dn,
+                                            double& wn) {
+  const double sixth = 1.0 / 6.0;
+  const double t23 = k2 + k3;
+  if (LAT) {
+    const double a12 = k1 + k2;
+    dn = fma(k3, sixth, fma(a12, sixth, dw));
+    wn = fma((a12 + t23) + (k3 + k4), sixth, w);
+  } else {
+    const double s3 = k1 + t23;
+    dn = fma(s3, sixth, dw);
+    wn = fma((s3 + t23) + k4, sixth, w);
+  }
+}
+
+// One speculative free-flight step of one particle, without the vote: new state
+// in (dn, wn); returns whether this lane's four stage gaps stayed above a0 and the
+// new gap is a positive number below the divergence filter -- the conditions
+// under which the step may be kept (see rk4_step).
 template <bool LAT>
 __device__ __forceinline__ bool free_step(const Particle64& P, double s0, double sh,
                                           double s1, long long a0_bits,
                                           const DivergeTest& T, double d, double w,
                                           double& dn, double& wn) {
-  const double sixth = 1.0 / 6.0;
   const double dw = d + w;
   const double d2 = fma(0.5, w, d);
-  const double k1 = accel_free<LAT>(P, s0, d, w);
+  const double k1 = accel_free<LAT, true>(P, s0, d, w);
   const double w2 = fma(0.5, k1, w);
-  const double k2 = accel_free<LAT>(P, sh, d2, w2);
+  const double k2 = accel_free<LAT, false>(P, sh, d2, w2);
   const double w3 = fma(0.5, k2, w);
-  const double d3 = fma(0.5, w2, d);
-  const double k3 = accel_free<LAT>(P, sh, d3, w3);
+  const double d3 = stage3_gap<LAT>(d, d2, k1, w2);
+  const double k3 = accel_free<LAT, true>(P, sh, d3, w3);
   const double d4 = d + w3;
-  const double k4 = accel_free<LAT>(P, s1, d4, w + k3);
+  const double k4 = accel_free<LAT, false>(P, s1, d4, w + k3);
   const int m = min(min(__double2hiint(d), __double2hiint(d2)),
                     min(__double2hiint(d3), __double2hiint(d4)));
-  const double t23 = k2 + k3;
-  const double s3 = k1 + t23;
-  dn = fma(s3, sixth, dw);
-  wn = fma((s3 + t23) + k4, sixth, w);
-  return (m > (int)(a0_bits >> 32)) & ((unsigned)__double2hiint(dn) < (unsigned)T.safe_hi);
+  rk4_combine<LAT>(dw, w, k1, k2, k3, k4, dn, wn);
+  // unsigned compare: a negative or NaN high word is huge
+  return (m > (int)(a0_bits >> 32)) &
+         ((unsigned)__double2hiint(dn) < (unsigned)T.safe_hi);
 }
 
 template <int LAW, int PPT, bool LAT>
@@ -270,7 +301,6 @@ __device__ __forceinline__ void rk4_step(const Particle64 (&P)[PPT], double s0,
                                          double (&w)[PPT], int& mode,
                                          bool (&bad)[PPT],
                                          const DivergeTest& T) {
-  const double sixth = 1.0 / 6.0;
   double dw[PPT], d2[PPT];
 #pragma unroll
   for (int q = 0; q < PPT; ++q) {
@@ -284,43 +314,23 @@ __device__ __forceinline__ void rk4_step(const Particle64 (&P)[PPT], double s0,
       const double w2 = fma(0.5, k1, w[q]);
       const double k2 = accel_smooth<LAW>(P[q], sh, d2[q], w2);
       const double w3 = fma(0.5, k2, w[q]);
-      const double k3 = accel_smooth<LAW>(P[q], sh, fma(0.5, w2, d[q]), w3);
+      const double k3 =
+          accel_smooth<LAW>(P[q], sh, stage3_gap<LAT>(d[q], d2[q], k1, w2), w3);
       const double k4 = accel_smooth<LAW>(P[q], s1, d[q] + w3, w[q] + k3);
-      const double t23 = k2 + k3;
-      const double s3 = k1 + t23;
-      d[q] = fma(s3, sixth, dw[q]);
-      w[q] = fma((s3 + t23) + k4, sixth, w[q]);
+      rk4_combine<LAT>(dw[q], w[q], k1, k2, k3, k4, d[q], w[q]);
       bad[q] |= diverged_step(d[q], T);
     }
     return;
   }
   if (mode == 0) {
     double dn[PPT], wn[PPT];
-    int m = 0x7fffffff;
-    unsigned hmax = 0u;
+    bool ok = true;
 #pragma unroll
-    for (int q = 0; q < PPT; ++q) {
-      const double k1 = accel_free<LAT>(P[q], s0, d[q], w[q]);
-      const double w2 = fma(0.5, k1, w[q]);
-      const double k2 = accel_free<LAT>(P[q], sh, d2[q], w2);
-      const double w3 = fma(0.5, k2, w[q]);
-      const double d3 = fma(0.5, w2, d[q]);
-      const double k3 = accel_free<LAT>(P[q], sh, d3, w3);
-      const double d4 = d[q] + w3;
-      const double k4 = accel_free<LAT>(P[q], s1, d4, w[q] + k3);
-      m = min(m, min(min(__double2hiint(d[q]), __double2hiint(d2[q])),
-                     min(__double2hiint(d3), __double2hiint(d4))));
-      const double t23 = k2 + k3;
-      const double s3 = k1 + t23;
-      dn[q] = fma(s3, sixth, dw[q]);
-      wn[q] = fma((s3 + t23) + k4, sixth, w[q]);
-      hmax = max(hmax, (unsigned)__double2hiint(dn[q]));
-    }
+    for (int q = 0; q < PPT; ++q)
+      ok &= free_step<LAT>(P[q], s0, sh, s1, a0_bits, T, d[q], w[q], dn[q], wn[q]);
     // kept only if no stage touched the sample and the new gap is a positive
-    // number below the divergence filter (unsigned compare: a negative or NaN
-    // high word is huge) -- so a kept step needs no divergence test
-    if (__all_sync(0xffffffffu, (m > (int)(a0_bits >> 32)) &
-                                    (hmax < (unsigned)T.safe_hi))) {
+    // number below the divergence filter -- so a kept step needs no divergence test
+    if (__all_sync(0xffffffffu, ok)) {
 #pragma unroll
       for (int q = 0; q < PPT; ++q) {
         d[q] = dn[q];
@@ -336,20 +346,17 @@ __device__ __forceinline__ void rk4_step(const Particle64 (&P)[PPT], double s0,
   int m = 0x7fffffff;
 #pragma unroll
   for (int q = 0; q < PPT; ++q) {
-    const double k1 = accel_both<LAW, LAT>(P[q], s0, d[q], w[q], a0_bits);
+    const double k1 = accel_both<LAW, LAT, true>(P[q], s0, d[q], w[q], a0_bits);
     const double w2 = fma(0.5, k1, w[q]);
-    const double k2 = accel_both<LAW, LAT>(P[q], sh, d2[q], w2, a0_bits);
+    const double k2 = accel_both<LAW, LAT, false>(P[q], sh, d2[q], w2, a0_bits);
     const double w3 = fma(0.5, k2, w[q]);
-    const double d3 = fma(0.5, w2, d[q]);
-    const double k3 = accel_both<LAW, LAT>(P[q], sh, d3, w3, a0_bits);
+    const double d3 = stage3_gap<LAT>(d[q], d2[q], k1, w2);
+    const double k3 = accel_both<LAW, LAT, true>(P[q], sh, d3, w3, a0_bits);
     const double d4 = d[q] + w3;
-    const double k4 = accel_both<LAW, LAT>(P[q], s1, d4, w[q] + k3, a0_bits);
+    const double k4 = accel_both<LAW, LAT, false>(P[q], s1, d4, w[q] + k3, a0_bits);
     m = min(m, min(min(__double2hiint(d[q]), __double2hiint(d2[q])),
                    min(__double2hiint(d3), __double2hiint(d4))));
-    const double t23 = k2 + k3;
-    const double s3 = k1 + t23;
-    d[q] = fma(s3, sixth, dw[q]);
-    w[q] = fma((s3 + t23) + k4, sixth, w[q]);
+    rk4_combine<LAT>(dw[q], w[q], k1, k2, k3, k4, d[q], w[q]);
     bad[q] |= diverged_step(d[q], T);
   }
   // back to speculation once a whole step stayed clear of the sample

@@ -11,6 +11,13 @@
 
 namespace afm {
 
+// Each stage of a time-tile ring is followed by pad rows: the kernels fetch the
+// next row one step ahead, so the row after a stage's last one is read (and
+// discarded); it must be neither a bulk-copy target nor a barrier word.  128
+// bytes keep the second stage aligned like the first; only the first pad row is
+// ever read (it is zeroed once).
+constexpr int kPadBytes = 128;
+
 // ---- mbarrier / bulk-copy PTX (sm_90+; SASS: SYNCS.*, UBLKCP) ---------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));

@@ -182,9 +182,6 @@ int launch_pso_shard_gbest(const BoxDev& box, int D, int n_traces, int n_ranks,
                            cudaStream_t st);
 int launch_fma_peak(int precision, int iters, int blocks, int threads,
                     void* sink, float* ms, cudaStream_t st);
-int launch_dispatch_probe(int mode, int warps_per_subpartition, int n_sm,
-                          const double* in, double* sink, double* ns_per_dfma,
-                          cudaStream_t st);
 int launch_beam_setup(const afm_beam_cfg& cfg, double h, BeamModeConsts* dev_out,
                       cudaStream_t st);
 int launch_beam_integrate(const BeamConsts& bc, const BeamModeConsts& mo,

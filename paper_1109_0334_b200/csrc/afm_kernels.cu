@@ -17,6 +17,8 @@
 
 namespace afm {
 
+constexpr int kPadRows = kPadBytes / 32;  // pad rows after each stage of the tile ring
+
 // ============================================================================
 // Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11): the counter-based
 // generator north_star names.  DESIGN.md reading R11 fixes key and counter.
@@ -122,46 +124,11 @@ __device__ __forceinline__ void run_steps(const double4* sp, int i0, int i1,
                                           double (&J)[PPT], bool (&bad)[PPT],
                                           int& mode) {
   if (i0 >= i1) return;
-#ifdef AFM_PAIR
-  if (IsDmt<LAW>::value && PPT == 1) {
-    // DMT laws: in free flight two steps are taken speculatively before the
-    // warp votes once on both; a failed pair redoes its first step in the
-    // general form (rk4_step with mode 1), which also finds the way back.
-    int i = i0;
-    while (i < i1) {
-      if (mode == 0 && i + 1 < i1) {
-        const double4 ra = sp[i], rb = sp[i + 1];
-        double d1, w1, d2, w2;
-        const bool ok1 = free_step<LAT>(P[0], ra.x, ra.y, ra.z, a0_bits, T, d[0], w[0], d1, w1);
-        const bool ok2 = free_step<LAT>(P[0], rb.x, rb.y, rb.z, a0_bits, T, d1, w1, d2, w2);
-        if (__all_sync(0xffffffffu, ok1 & ok2)) {
-          if (WIN) {
-            const double e1 = d1 - ra.w, e2 = d2 - rb.w;
-            J[0] = fma(e2, e2, fma(e1, e1, J[0]));
-          }
-          d[0] = d2;
-          w[0] = w2;
-          i += 2;
-          continue;
-        }
-        mode = 1;
-      }
-      const double4 r = sp[i];
-      rk4_step<LAW, PPT, LAT>(P, r.x, r.y, r.z, a0_bits, d, w, mode, bad, T);
-      if (WIN) {
-        const double res = d[0] - r.w;
-        J[0] = fma(res, res, J[0]);
-      }
-      ++i;
-    }
-    return;
-  }
-#endif
   double4 r = sp[i0];
 #pragma unroll 2
   for (int i = i0; i < i1; ++i) {
     // next row fetched one step ahead; the fetch past the last row of a tile
-    // lands in the other stage or the padding and is discarded
+    // reads the stage's own pad row (zeroed once, never a bulk-copy target)
     const double4 rn = sp[i + 1];
     rk4_step<LAW, PPT, LAT>(P, r.x, r.y, r.z, a0_bits, d, w, mode, bad, T);
     if (WIN) {
@@ -182,9 +149,10 @@ template <int LAW, int MODE, int PPT, bool LAT>
 __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
                                      int blocks_per_tr) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
+  // two stages of T rows, each followed by one pad row for the one-step-ahead fetch
   double4* tile0 = reinterpret_cast<double4*>(smem_raw);
-  double4* tile1 = tile0 + mc.T;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(tile1 + mc.T);
+  double4* tile1 = tile0 + (mc.T + kPadRows);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tile1 + (mc.T + kPadRows));
   __shared__ Cand red[32];
 
   const int tid = threadIdx.x;
@@ -210,6 +178,8 @@ __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
   const double* stream = io.stream + (int64_t)s * mc.N * 4;
 
   if (tid == 0) {
+    tile0[mc.T] = make_double4(0.0, 0.0, 0.0, 0.0);
+    tile1[mc.T] = make_double4(0.0, 0.0, 0.0, 0.0);
     mbar_init(&bars[0], 1);
     mbar_init(&bars[1], 1);
     fence_mbar_init();
@@ -354,12 +324,14 @@ __global__ void __launch_bounds__(32)
 integrate_misfit_f64_q(ModelConsts mc, IntegrateIO io, int blocks_per_tr, SegQueue q) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double4* tile0 = reinterpret_cast<double4*>(smem_raw);
-  double4* tile1 = tile0 + mc.T;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(tile1 + mc.T);
+  double4* tile1 = tile0 + (mc.T + kPadRows);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tile1 + (mc.T + kPadRows));
   __shared__ Cand red[32];
 
   const int tid = threadIdx.x;
   if (tid == 0) {
+    tile0[mc.T] = make_double4(0.0, 0.0, 0.0, 0.0);
+    tile1[mc.T] = make_double4(0.0, 0.0, 0.0, 0.0);
     mbar_init(&bars[0], 1);
     mbar_init(&bars[1], 1);
     fence_mbar_init();
@@ -812,7 +784,7 @@ static int launch_integrate_t(const ModelConsts& mc, const IntegrateIO& io,
                       : blocks_per_trace(io.per, block * PPT);
   if (LAT) block = 32;  // one warp per CTA
   const unsigned grid = (unsigned)(bpt * io.n_traces);
-  const size_t smem = (size_t)mc.T * 32 * 2 + 64;  // + barriers + over-read pad
+  const size_t smem = (size_t)(mc.T + kPadRows) * 32 * 2 + 64;  // two stages + pad rows + barriers
   auto kern = integrate_misfit_f64<LAW, MODE, PPT, LAT>;
   if (smem > 48 * 1024)
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -857,7 +829,7 @@ template <int LAW, int MODE>
 static int launch_integrate_q_t(const ModelConsts& mc, const IntegrateIO& io,
                                 const SegQueue& q, int workers, cudaStream_t st) {
   const int bpt = blocks_per_trace(io.per, 32);
-  const size_t smem = (size_t)mc.T * 32 * 2 + 64;
+  const size_t smem = (size_t)(mc.T + kPadRows) * 32 * 2 + 64;
   auto kern = integrate_misfit_f64_q<LAW, MODE>;
   if (smem > 48 * 1024)
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

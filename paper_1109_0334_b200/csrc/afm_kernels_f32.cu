@@ -16,6 +16,8 @@
 
 namespace afm {
 
+constexpr int kPadRows = kPadBytes / 16;  // pad rows after each stage of the tile ring
+
 // s6(t) = (beta/6) (F0/k) cos(w t) + (beta/6) z_c  [nm per step^2 / 6], FP64.
 __device__ __forceinline__ double s6_of(const ModelConstsF32& mf, double t) {
   return fma(mf.drive6, cos(__dmul_rn(mf.w_drive, t)), mf.b6_zc);
@@ -63,7 +65,7 @@ __device__ __forceinline__ void run_steps32(const float4* sp, int i0, int i1,
   float4 r = sp[i0];
 #pragma unroll 2
   for (int i = i0; i < i1; ++i) {
-    const float4 rn = sp[i + 1];  // one step ahead; past the tile: discarded
+    const float4 rn = sp[i + 1];  // one step ahead; past the tile: the pad row
     rk4_step32<LAW, PPT>(M, P, s_prev, r.x, r.y, r.w, S, mode, bad);
     if (WIN) {
 #pragma unroll
@@ -82,8 +84,8 @@ __global__ void integrate_misfit_f32(ModelConstsF32 mf, IntegrateIO io,
                                      int blocks_per_tr) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float4* tile0 = reinterpret_cast<float4*>(smem_raw);
-  float4* tile1 = tile0 + mf.T;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(tile1 + mf.T);
+  float4* tile1 = tile0 + (mf.T + kPadRows);  // one pad row per stage for the row fetched ahead
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tile1 + (mf.T + kPadRows));
   __shared__ Cand red[32];
 
   const int tid = threadIdx.x;
@@ -103,6 +105,8 @@ __global__ void integrate_misfit_f32(ModelConstsF32 mf, IntegrateIO io,
       reinterpret_cast<const float4*>(io.stream) + (int64_t)s * mf.N;
 
   if (tid == 0) {
+    tile0[mf.T] = make_float4(0.f, 0.f, 0.f, 0.f);
+    tile1[mf.T] = make_float4(0.f, 0.f, 0.f, 0.f);
     mbar_init(&bars[0], 1);
     mbar_init(&bars[1], 1);
     fence_mbar_init();
@@ -260,12 +264,14 @@ __global__ void __launch_bounds__(32)
 integrate_misfit_f32_q(ModelConstsF32 mf, IntegrateIO io, int blocks_per_tr, SegQueue q) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float4* tile0 = reinterpret_cast<float4*>(smem_raw);
-  float4* tile1 = tile0 + mf.T;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(tile1 + mf.T);
+  float4* tile1 = tile0 + (mf.T + kPadRows);  // one pad row per stage for the row fetched ahead
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tile1 + (mf.T + kPadRows));
   __shared__ Cand red[32];
 
   const int tid = threadIdx.x;
   if (tid == 0) {
+    tile0[mf.T] = make_float4(0.f, 0.f, 0.f, 0.f);
+    tile1[mf.T] = make_float4(0.f, 0.f, 0.f, 0.f);
     mbar_init(&bars[0], 1);
     mbar_init(&bars[1], 1);
     fence_mbar_init();
@@ -466,7 +472,7 @@ static int launch_integrate32_t(const ModelConstsF32& mf, const IntegrateIO& io,
                                 int block, cudaStream_t st) {
   const int bpt = blocks_per_trace(io.per, block * PPT);
   const unsigned grid = (unsigned)(bpt * io.n_traces);
-  const size_t smem = (size_t)mf.T * 16 * 2 + 64;
+  const size_t smem = (size_t)(mf.T + kPadRows) * 16 * 2 + 64;
   auto kern = integrate_misfit_f32<LAW, MODE, PPT>;
   if (smem > 48 * 1024)
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -501,7 +507,7 @@ template <int LAW, int MODE>
 static int launch_integrate32_q_t(const ModelConstsF32& mf, const IntegrateIO& io,
                                   const SegQueue& q, int workers, cudaStream_t st) {
   const int bpt = blocks_per_trace(io.per, 32);
-  const size_t smem = (size_t)mf.T * 16 * 2 + 64;
+  const size_t smem = (size_t)(mf.T + kPadRows) * 16 * 2 + 64;
   auto kern = integrate_misfit_f32_q<LAW, MODE>;
   if (smem > 48 * 1024)
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

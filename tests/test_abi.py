@@ -35,17 +35,25 @@ def test_header_functions_are_all_exported(lib):
     assert sorted(afm.SYMBOLS) == names
 
 
-def test_struct_layouts_match_the_header():
-    # sizes the C compiler gives the PODs of afm.h
-    code = ('#include <stdio.h>\n#include "afm.h"\nint main(){printf("%zu %zu %zu\\n",'
-            'sizeof(afm_cfg),sizeof(afm_bounds),sizeof(afm_swarm_cfg));return 0;}')
-    exe = os.path.join(ROOT, "_work", "abi_sizes")
-    os.makedirs(os.path.dirname(exe), exist_ok=True)
-    src = exe + ".c"
-    open(src, "w").write(code)
-    subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), src, "-o", exe])
-    sizes = [int(x) for x in subprocess.check_output([exe]).split()]
-    assert sizes == [C.sizeof(afm.Cfg), C.sizeof(afm.Bounds), C.sizeof(afm.SwarmCfg)]
+def test_struct_layouts_match_the_header(tmp_path):
+    """Size of every POD of afm.h and offset of every field, as the C compiler lays
+    them out, against the ctypes mirrors of the binding."""
+    pods = (("afm_cfg", afm.Cfg), ("afm_bounds", afm.Bounds), ("afm_swarm_cfg", afm.SwarmCfg),
+            ("afm_beam_cfg", afm.BeamCfg))
+    lines = ['#include <stdio.h>', '#include <stddef.h>', '#include "afm.h"', 'int main(){']
+    want = []
+    for cname, cls in pods:
+        lines.append('printf("%%zu\\n", sizeof(%s));' % cname)
+        want.append(C.sizeof(cls))
+        for fname, _ in cls._fields_:
+            lines.append('printf("%%zu\\n", offsetof(%s, %s));' % (cname, fname))
+            want.append(getattr(cls, fname).offset)
+    lines.append('return 0;}')
+    src, exe = tmp_path / "abi_layout.c", tmp_path / "abi_layout"
+    src.write_text("\n".join(lines))
+    subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)])
+    got = [int(x) for x in subprocess.check_output([str(exe)]).split()]
+    assert got == want
 
 
 def test_library_is_sm100a_and_uses_bulk_async_copy():
@@ -142,9 +150,18 @@ def test_new_entry_points_validate_before_touching_the_device(lib):
     out = C.c_double(0.0)
     assert lib.afm_fma_peak(7, 0.1, C.byref(out), None) == afm.EINVAL
     assert lib.afm_fma_peak(0, 100.0, C.byref(out), None) == afm.EINVAL
-    assert lib.afm_dispatch_probe(9, 1, C.byref(out), None) == afm.EINVAL
-    assert lib.afm_dispatch_probe(0, 0, C.byref(out), None) == afm.EINVAL
-    for name, bad in (("form", 3), ("lanes", 3), ("pack", 5), ("ppt", 4), ("tile", -1)):
+    ms, n = (C.c_double * 4)(), C.c_int32(0)
+    assert lib.afm_kernel_times(None, 4, C.byref(n)) == afm.EINVAL
+    assert lib.afm_kernel_times(ms, 4, C.byref(n)) == afm.OK and n.value == 0
+    z = np.zeros(8)
+    assert lib.afm_pso_step_host(C.byref(b), C.byref(sw), 9, 1, 0, 0, 1, z.ctypes.data,
+                                 z.ctypes.data, z.ctypes.data, z.ctypes.data, z.ctypes.data,
+                                 z.ctypes.data, z.ctypes.data, None) == afm.EINVAL
+    assert lib.afm_pso_step_host(C.byref(b), C.byref(sw), 2, 1, 0, 0, 1, None, z.ctypes.data,
+                                 z.ctypes.data, z.ctypes.data, z.ctypes.data, z.ctypes.data,
+                                 z.ctypes.data, None) == afm.EINVAL
+    for name, bad in (("form", 3), ("lanes", 3), ("pack", 5), ("ppt", 4), ("tile", -1),
+                      ("queue", 3), ("segs", 5000), ("workers", 9), ("kernel_events", 2)):
         with pytest.raises(afm.AfmError):
             afm.afm_set_option(name, bad)
         assert afm.afm_set_option(name, 0) is None
