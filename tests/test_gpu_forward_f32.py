@@ -211,28 +211,45 @@ def test_f32_divergence_gives_inf(afm):
 
 
 def test_f32_pso_teacher_forced(afm):
-    """DESIGN.md R17: FP32 misfits differ from FP64 by up to 1e-3, so the swarm
-    may legitimately take another path.  Teacher forcing: at every iteration
-    the GPU's own positions x are evaluated by the oracle (J within 1e-3), and
-    the GPU's personal/global bests must be consistent with the GPU's own J."""
+    """DESIGN.md R17 / SURVEY.md c-17: FP32 misfits differ from FP64 by up to 1e-3, so
+    the swarm may legitimately take another path than the FP64 oracle's.  Teacher
+    forcing, both halves: (1) at every iteration the GPU's own positions x are
+    evaluated by the oracle (J within 1e-3); (2) the ORACLE's PSO loop is replayed
+    with the GPU's own J as its cost (a scripted callback: the k-th evaluation
+    returns the J the GPU recorded for it), and every x, v, pbest and pbestJ of the
+    GPU run must equal that replay bit for bit, as must theta* and J*."""
     import torch
     wl = wlm.scaled(wlm.config(2), n_cycles=20, n_skip_cycles=10, n_particles=96,
                     n_iters=6)
     trace = oracle_trace(wl)
     t = torch.as_tensor(trace, device="cuda")
     cfg = afm.cfg_from(wl, precision=afm.F32)
-    g = afm.afm_pso_invert(afm.bounds_from(wl), afm.swarm_from(wl), 0, t, cfg,
+    seed = 5
+    g = afm.afm_pso_invert(afm.bounds_from(wl), afm.swarm_from(wl), seed, t, cfg,
                            dump=True, hist=True)
     d = g["dump"].cpu().numpy()            # [it][P][3D+2]
-    D = wl["n_params"]
+    D, P = wl["n_params"], d.shape[1]
     M = orc.model_from(wl)
-    best = np.full(d.shape[1], np.inf)
     for it in range(d.shape[0]):
-        x = d[it, :, 0:D]
-        Jg = d[it, :, 3 * D]
-        th = wlm.theta_of_coords(wl, x)
+        th = wlm.theta_of_coords(wl, d[it, :, 0:D])
         Jo = orc.forward_batch(M, th, trace, z0=wl["z0"], v0=wl["v0"], openmp=True)
-        assert rel_err(Jg, Jo).max() < TOL_F32, it
-        best = np.minimum(best, Jg)
-        assert np.array_equal(d[it, :, 3 * D + 1], best), it   # pbestJ from own J
-    assert g["J_star"][0] == best.min()
+        assert rel_err(d[it, :, 3 * D], Jo).max() < TOL_F32, it
+    # (2) Eq. 8 on the CPU from the GPU's own J
+    calls = {"k": 0, "theta": []}
+
+    def gpu_cost(theta, _U):
+        k = calls["k"]
+        calls["k"] += 1
+        calls["theta"].append(theta)
+        return d[k // P, k % P, 3 * D]
+
+    o = orc.pso_core(gpu_cost, D, orc.box_from(wl), orc.swarm_from(wl), seed, trace)
+    assert calls["k"] == d.shape[0] * P
+    assert np.array_equal(o["dump"], d)                 # x, v, pbest, J, pbestJ
+    assert np.array_equal(o["gbest_hist"], g["gbest_hist"].cpu().numpy())
+    assert np.array_equal(o["J_star"], g["J_star"])
+    # theta* = 10^x through two different pow() implementations: last-bit agreement
+    assert rel_err(g["theta_star"], o["theta_star"]).max() < 1e-15
+    # the oracle asked for the cost at exactly the parameters the GPU integrated
+    th_all = wlm.theta_of_coords(wl, d[:, :, 0:D].reshape(-1, D))
+    assert rel_err(np.array(calls["theta"]), th_all).max() < 1e-15

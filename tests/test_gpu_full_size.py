@@ -2,11 +2,13 @@
 times (default options), on sampled outputs the oracle can compute one by one
 plus properties that hold at any size.
 
-configs[1]: all 65 536 particles x 51 200 steps on the GPU, 160 sampled
-particles through the oracle (FP64 1e-9; FP32 1e-3 with the c-15 protocol).
-configs[2], [3], [4]: the full swarm for the first PSO batches; sampled
-particles' misfits against the oracle at the positions the GPU evaluated, and
-personal/global-best consistency over ALL particles.
+configs[1]: all 65 536 particles x 51 200 steps on the GPU, 2 048 sampled
+particles through the oracle (FP64 1e-9; FP32 1e-3), every particle above the
+tolerance verified one by one by the R15 protocol and their number capped at 0.2 %.
+configs[2]: the WHOLE inversion (1 024 x 200 x 25 600) replayed against the oracle,
+and the run to the cost cutoff.  configs[3], [4]: the full swarm for the first PSO
+batches; sampled particles' misfits against the oracle at the positions the GPU
+evaluated, and personal/global-best consistency over ALL particles.
 """
 import numpy as np
 import pytest
@@ -36,7 +38,7 @@ def cfg1_inputs():
     trace = oracle_trace(wl)
     params = wlm.draw_params(wl, P, seed=1)
     z0v0 = wlm.draw_initial_states(wl, P, seed=2)
-    pick = np.random.default_rng(7).choice(P, size=160, replace=False)
+    pick = np.random.default_rng(7).choice(P, size=2048, replace=False)
     pick[:4] = [0, 31, P - 32, P - 1]          # first/last warp edges
     Jo = orc.forward_batch(orc.model_from(wl), params[pick], trace, z0v0=z0v0[pick],
                            openmp=True)
@@ -53,19 +55,57 @@ def _forward(afm, wl, params, trace, z0v0, precision):
     return J.cpu().numpy()
 
 
+EXCUSED_CAP = 0.002      # DESIGN.md R15: at most 0.2 % of a batch may be excused
+
+
+def _excused_f64(wl, M, trace, theta, state, Jo_i):
+    """R15, FP64: the particle is one the oracle itself cannot resolve to 1e-9: a
+    1e-13 relative change of its initial state (or, with the common start, of theta)
+    moves the ORACLE's J by more than the tolerance."""
+    if state is not None:
+        J2 = orc.forward_batch(M, theta[None], trace, z0v0=state[None] * (1 + 1e-13))[0]
+    else:
+        J2 = orc.forward_batch(M, theta[None] * (1 + 1e-13), trace, z0=wl["z0"],
+                               v0=wl["v0"])[0]
+    return abs(J2 - Jo_i) / Jo_i > 1e-9
+
+
+def _excused_f32(wl, M, trace, theta, state, Jo_i):
+    """R15, FP32: a ONE-ulp FP32 perturbation (2^-23) of the inputs alone already moves
+    the oracle's J by TOL/4: measured with a 1e-10 perturbation and scaled."""
+    ill = 0.25 * 1e-3 / 2.0 ** -23 * 1e-10
+    moved = 0.0
+    for eps in (1e-10, -1e-10):
+        if state is not None:
+            J1 = orc.forward_batch(M, theta[None], trace, z0v0=state[None] * (1 + eps))[0]
+        else:
+            J1 = orc.forward_batch(M, theta[None], trace, z0=wl["z0"] + eps * 1e-9,
+                                   v0=wl["v0"] * (1 + eps))[0]
+        kw = dict(z0v0=state[None]) if state is not None else dict(z0=wl["z0"], v0=wl["v0"])
+        J2 = orc.forward_batch(M, theta[None] * (1 + eps), trace, **kw)[0]
+        moved = max(moved, abs(J1 - Jo_i) / Jo_i, abs(J2 - Jo_i) / Jo_i)
+    return moved > ill
+
+
+def _check_with_r15(e, tol, excused, label):
+    """Every sampled particle meets `tol` unless excused(i) verifies it as
+    ill-conditioned; at most 0.2 % of the sample may be excused."""
+    out = np.flatnonzero(~(e < tol))
+    print("%s: n %d median %.2e p99 %.2e max %.2e, above tolerance %d"
+          % (label, e.size, np.median(e), np.percentile(e, 99), e.max(), out.size))
+    assert out.size <= max(1, int(np.ceil(EXCUSED_CAP * e.size))), (out.size, e[out][:8])
+    for i in out:
+        assert excused(int(i)), (label, int(i), e[i])
+
+
 def test_cfg1_full_size_f64(afm, cfg1_inputs):
     wl, trace, params, z0v0, pick, Jo = cfg1_inputs
     Jg = _forward(afm, wl, params, trace, z0v0, afm.F64)
     assert Jg.shape == (65536,) and not np.isnan(Jg).any()
-    e = rel_err(Jg[pick], Jo)
-    # c-15: a chaotic particle is excused only if the oracle itself moves by more
-    # than the tolerance under a 1e-13 relative change of its initial state
     M = orc.model_from(wl)
-    for i in np.flatnonzero(e >= 1e-9):
-        p, z = params[pick[i]][None], z0v0[pick[i]][None]
-        J2 = orc.forward_batch(M, p, trace, z0v0=z * (1 + 1e-13))[0]
-        assert abs(J2 - Jo[i]) / Jo[i] > 1e-9, (int(pick[i]), e[i])
-    assert np.percentile(e, 95) < 1e-9
+    _check_with_r15(rel_err(Jg[pick], Jo), 1e-9,
+                    lambda i: _excused_f64(wl, M, trace, params[pick[i]], z0v0[pick[i]], Jo[i]),
+                    "cfg1 f64")
     # whole-batch properties: every misfit positive; J >= the noise floor scale
     assert (Jg[np.isfinite(Jg)] > 0).all()
 
@@ -74,21 +114,17 @@ def test_cfg1_full_size_f32(afm, cfg1_inputs):
     wl, trace, params, z0v0, pick, Jo = cfg1_inputs
     Jg = _forward(afm, wl, params, trace, z0v0, afm.F32)
     J64 = _forward(afm, wl, params, trace, z0v0, afm.F64)
-    e = rel_err(Jg[pick], Jo)
     M = orc.model_from(wl)
-    ill = 0.25 * 1e-3 / 2.0 ** -23 * 1e-10
-    for i in np.flatnonzero(e >= 1e-3):
-        p, z = params[pick[i]][None], z0v0[pick[i]][None]
-        J2 = orc.forward_batch(M, p, trace, z0v0=z * (1 + 1e-10))[0]
-        assert abs(J2 - Jo[i]) / Jo[i] > ill, (int(pick[i]), e[i])
-    assert np.percentile(e, 95) < 1e-3
+    _check_with_r15(rel_err(Jg[pick], Jo), 1e-3,
+                    lambda i: _excused_f32(wl, M, trace, params[pick[i]], z0v0[pick[i]], Jo[i]),
+                    "cfg1 f32")
     # over ALL 65 536 particles, against the FP64 kernel (itself checked above)
     ea = rel_err(Jg, J64)
     print("cfg1 f32 vs f64 kernel, all particles: median %.2e p99 %.2e p99.9 %.2e, "
           "%d above 1e-3" % (np.median(ea), np.percentile(ea, 99),
                               np.percentile(ea, 99.9), int((ea >= 1e-3).sum())))
     assert np.percentile(ea, 99) < 1e-4
-    assert (ea >= 1e-3).mean() < 5e-3
+    assert (ea >= 1e-3).mean() < EXCUSED_CAP
 
 
 def _full_swarm_batches(afm, ci, n_iters, n_sample, precision=0, n_traces=None):
@@ -120,32 +156,104 @@ def _full_swarm_batches(afm, ci, n_iters, n_sample, precision=0, n_traces=None):
     rng = np.random.default_rng(11 + ci)
     pick = rng.choice(T * per, size=n_sample, replace=False)
     M = orc.model_from(wl)
-    worst = 0.0
+    tol = 1e-3 if precision == 1 else 1e-9
+    excuse = _excused_f32 if precision == 1 else _excused_f64
     for it in range(n_iters):
         xs = d[it, pick, 0:D].cpu().numpy()
         Jg = d[it, pick, 3 * D].cpu().numpy()
         th = wlm.theta_of_coords(wl, xs)
+        Jo = np.empty(n_sample)
         for s in np.unique(pick // per):
             m = (pick // per) == s
-            Jo = orc.forward_batch(M, th[m], trace[s], z0=wl["z0"], v0=wl["v0"],
-                                   openmp=True)
-            worst = max(worst, rel_err(Jg[m], Jo).max())
-    return worst
+            Jo[m] = orc.forward_batch(M, th[m], trace[s], z0=wl["z0"], v0=wl["v0"],
+                                      openmp=True)
+        assert np.array_equal(np.isfinite(Jg), np.isfinite(Jo))
+        _check_with_r15(rel_err(Jg, Jo), tol,
+                        lambda i: excuse(wl, M, trace[pick[i] // per], th[i], None, Jo[i]),
+                        "cfg%d %s batch %d" % (ci, "f32" if precision else "f64", it))
 
 
 def test_cfg2_full_swarm_first_batches(afm):
-    assert _full_swarm_batches(afm, 2, n_iters=3, n_sample=96) < 1e-9
+    _full_swarm_batches(afm, 2, n_iters=3, n_sample=256)
 
 
 def test_cfg3_full_swarm_first_batches_f64(afm):
-    assert _full_swarm_batches(afm, 3, n_iters=2, n_sample=64) < 1e-9
+    _full_swarm_batches(afm, 3, n_iters=2, n_sample=256)
 
 
 def test_cfg3_full_swarm_first_batches_f32(afm):
-    # 64 samples x 2 batches: the bulk bound (p99.9 of the FP32 error is 8e-4)
-    assert _full_swarm_batches(afm, 3, n_iters=2, n_sample=64, precision=1) < 2e-3
+    """north_star's 1e-3 with the R15 protocol (no widened tolerance): 2 048 of the
+    8 192 particles per batch through the oracle."""
+    _full_swarm_batches(afm, 3, n_iters=2, n_sample=2048, precision=1)
 
 
 def test_cfg4_full_line_scan_first_batches(afm):
     """All 256 pixels x 4 096 particles = 1 048 576 concurrent particles."""
-    assert _full_swarm_batches(afm, 4, n_iters=2, n_sample=96) < 1e-9
+    _full_swarm_batches(afm, 4, n_iters=2, n_sample=256)
+
+
+def test_cfg2_full_inversion_replays_the_oracle(afm):
+    """configs[2] exactly as BASELINE.json states it -- 1 024 particles x 200 batches
+    x 25 600 steps, 5.2e9 particle-steps -- against the OpenMP build of the oracle
+    (about half a minute on 16 cores): the whole best-cost history, theta* and J*
+    (north_star: "the final theta* must agree with the oracle's")."""
+    import torch
+    wl = wlm.config(2)
+    trace = oracle_trace(wl)
+    g = afm.afm_pso_invert(afm.bounds_from(wl), afm.swarm_from(wl), wl["pso_seed"],
+                           torch.as_tensor(trace, device="cuda"), afm.cfg_from(wl),
+                           hist=True)
+    o = orc.pso_invert(orc.model_from(wl), orc.box_from(wl), orc.swarm_from(wl),
+                       wl["pso_seed"], trace, wl["z0"], wl["v0"], openmp=True)
+    gh, oh = g["gbest_hist"].cpu().numpy(), o["gbest_hist"]
+    assert g["n_iters_done"] == o["n_iters_done"] == 200
+    # the best cost of every one of the 200 batches
+    assert rel_err(gh[:, 0, 3], oh[:, 0, 3]).max() < 1e-9
+    assert rel_err(g["J_star"], o["J_star"]).max() < 1e-9
+    # the best position: identical until the swarm has converged onto the flat bottom
+    # of the cost, where candidates whose costs differ by less than the 1e-11 rounding
+    # difference between the two solvers may swap places (several results are then
+    # correct).  What is unique is checked: the cost history above; what is not is
+    # checked for validity: the position the GPU reports really has the cost it
+    # reports (oracle evaluation), and theta* agrees far inside north_star's 1e-3.
+    pe = rel_err(gh[:, 0, :3], oh[:, 0, :3]).max(axis=1)
+    first = int(np.argmax(pe >= 1e-9)) if (pe >= 1e-9).any() else 200
+    print("cfg2 full replay: best position identical (1e-9) for %d of 200 batches, "
+          "max later difference %.1e" % (first, pe.max()))
+    assert first >= 100 and pe.max() < 1e-6
+    M = orc.model_from(wl)
+    for it in sorted(set([first - 1, min(first, 199), 199])):
+        th = wlm.theta_of_coords(wl, gh[it:it + 1, 0, :3])[0]
+        Jchk = orc.misfit(M, th, wl["z0"], wl["v0"], trace[0])
+        assert abs(Jchk - gh[it, 0, 3]) / Jchk < 1e-9, it
+        assert abs(gh[it, 0, 3] - oh[it, 0, 3]) / oh[it, 0, 3] < 1e-9
+    assert rel_err(g["theta_star"], o["theta_star"]).max() < 1e-6
+    # and the answer is the noisy trace's minimiser: J* below J(truth), theta* within
+    # a fraction of a percent of the truth (noise-limited, DESIGN.md R16)
+    Jt = orc.misfit(orc.model_from(wl), wl["truth"], wl["z0"], wl["v0"], trace[0])
+    assert g["J_star"][0] <= Jt
+    assert rel_err(g["theta_star"][0], wl["truth"]).max() < 5e-3
+
+
+def test_cfg2_run_to_the_cost_cutoff_matches_the_oracle(afm):
+    """The cutoff run bench.py reports (cfg2_time_to_cutoff_ms, cfg2_batches_to_cutoff:
+    noise energy of the trace, W sigma^2 + 3 sd, R24): the oracle stops
+    after the same number of batches with the same theta*."""
+    import torch
+    wl = wlm.config(2)
+    trace = oracle_trace(wl)
+    W, sg = wl["n_window"], wl["sigma"]
+    jt = W * sg * sg * (1.0 + 3.0 * (2.0 / W) ** 0.5)
+    g = afm.afm_pso_invert(afm.bounds_from(wl), afm.swarm_from(wl, j_target=jt),
+                           wl["pso_seed"], torch.as_tensor(trace, device="cuda"),
+                           afm.cfg_from(wl), hist=True)
+    o = orc.pso_invert(orc.model_from(wl), orc.box_from(wl),
+                       orc.swarm_from(wl, j_target=jt), wl["pso_seed"], trace, wl["z0"],
+                       wl["v0"], openmp=True)
+    n = o["n_iters_done"]
+    print("configs[2] to the cutoff %.3e: %d batches" % (jt, n))
+    assert 1 < n < 200 and g["n_iters_done"] == n
+    assert abs(o["gbest_hist"][n - 1, 0, 3] / jt - 1.0) > 1e-6     # not a near tie
+    assert rel_err(g["gbest_hist"].cpu().numpy()[:n, 0, 3], o["gbest_hist"][:n, 0, 3]).max() < 1e-9
+    assert rel_err(g["theta_star"], o["theta_star"]).max() < 1e-9
+    assert g["J_star"][0] <= jt
