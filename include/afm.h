@@ -118,9 +118,10 @@ typedef struct {
 /* Swarm: n_particles PER TRACE; n_iters forward batches (iteration 0
  * evaluates the initial positions; the result is the global best after the
  * last batch).  w, c1, c2 are the weights of Eq. 8.
- * j_target > 0 enables the paper's cutoff rule: the run
- * ends after the first batch at which every trace's global best J is
- * <= j_target; <= 0 disables it. */
+ * j_target > 0 enables the paper's cutoff rule (
+ * DESIGN.md R24): the run ends after the first batch at which every trace's
+ * global best J is <= j_target, that batch is not followed by a move, and
+ * n_iters_done reports the batches run; <= 0 disables it. */
 typedef struct {
   int32_t n_particles;
   int32_t n_iters;
@@ -131,8 +132,14 @@ typedef struct {
                          of particle p is the best personal best among p-1, p,
                          p+1, wrapping inside the swarm, lowest index among
                          equal minima.  theta*, J* are the swarm's best either
-                         way.  Not available for a sharded swarm. */
-  int32_t reserved_;  /* must be 0 */
+                         way. */
+  int32_t async_chunk; /* 0 (or >= n_particles): the synchronous, generation by
+                         generation swarm of the paper.  B in 1..n_particles-1:
+                         asynchronous swarm (R25): every swarm is
+                         processed in chunks of B particles in index order; a
+                         chunk is evaluated, the bests are updated from it and
+                         it moves at once with the best known at that moment
+                         (same random streams).  afm_pso_invert[_host] only. */
 } afm_swarm_cfg;
 
 /* ---- forward problem + cost (Eq. 5) -------------
@@ -220,10 +227,13 @@ int afm_pso_init(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
  * afm_pso_invert).  Philox counters and the lowest-index tie-break use the
  * global index, so a sharded run replays the unsharded one bit for bit.  The
  * only data exchanged per iteration is the candidate row of every rank
- * (D + 2 doubles per trace), which the CALLER all-gathers (torch.distributed /
- * NCCL) between afm_pso_shard_eval and afm_pso_shard_move; sharding whole
- * traces needs no exchange (n_ranks = 1, gathered = own cand_out).
- * swarm->n_particles is the LOCAL particle count per local trace. */
+ * (per trace D + 2 doubles, or 3 D + 4 with the ring topology, whose rows also
+ * carry the personal bests of the shard's first and last particle: the ring
+ * neighbours of the adjacent shards), which the CALLER all-gathers
+ * (torch.distributed / NCCL) between afm_pso_shard_eval and afm_pso_shard_move;
+ * sharding whole traces needs no exchange (n_ranks = 1, gathered = own
+ * cand_out).  swarm->n_particles is the LOCAL particle count per local trace.
+ * The asynchronous swarm (async_chunk) is not available here. */
 
 /* afm_pso_init for a shard.  Note: gbest is set to the first LOCAL particle;
  * when one trace is sharded over ranks, copy rank 0's gbest to the others. */
@@ -236,7 +246,9 @@ int afm_pso_shard_init(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
 /* Rows a1-a5 + the local part of a6 for this shard: theta = map(x), forward
  * solve + misfit, personal bests, and the shard's best candidate per trace.
  * All device, FP64:  trace [cfg->n_traces][W]; x, pbest [PT][D]; J, pbestJ
- * [PT]; cand_out [cfg->n_traces][D+2] = { pbestJ, global index, pbest x[D] }.
+ * [PT]; cand_out [cfg->n_traces][R], R = D + 2 = { pbestJ, global index, pbest
+ * x[D] }, or with swarm->topology == 1 R = 3 D + 4 = that + { pbestJ, pbest
+ * x[D] } of the first and of the last local particle of the trace.
  * Asynchronous. */
 int afm_pso_shard_eval(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
                        const double* trace, const afm_cfg* cfg,
@@ -245,16 +257,23 @@ int afm_pso_shard_eval(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
                        void* cuda_stream);
 
 /* Rest of a6 + a7: global best per trace from the gathered candidates
- * (device [n_ranks][n_traces][D+2]; lowest global index among equal minima,
+ * (device [n_ranks][n_traces][R]; lowest global index among equal minima,
  * replaced only on a strict improvement), then Eq. 8 + move + bound rule when
- * do_move != 0.  theta_star [n_traces][D], J_star [n_traces]: device or NULL.
+ * do_move != 0.  rank: which of the n_ranks row blocks is this process's own;
+ * swarm_particles: particles per trace of the WHOLE swarm (= swarm->n_particles
+ * when whole traces are sharded).  With the ring topology and a swarm split
+ * over ranks (one trace, consecutive slices in rank order) the neighbours of
+ * the shard's edge particles are read from the rows of rank - 1 and rank + 1
+ * (wrapping), and pbestJ [PT] (device) is required; otherwise pbestJ may be
+ * NULL.  theta_star [n_traces][D], J_star [n_traces]: device or NULL.
  * Asynchronous. */
 int afm_pso_shard_move(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
                        int32_t n_dims, int32_t n_traces, uint64_t seed,
                        int32_t iteration, int32_t do_move,
                        int64_t first_particle, const double* gathered,
-                       int32_t n_ranks, double* x, double* v,
-                       const double* pbest, double* gbest, double* gbestJ,
+                       int32_t n_ranks, int32_t rank, int64_t swarm_particles,
+                       double* x, double* v, const double* pbest,
+                       const double* pbestJ, double* gbest, double* gbestJ,
                        double* theta_star, double* J_star, void* cuda_stream);
 
 /* ---- Multi-mode Euler-Bernoulli cantilever (the paper's own forward model) ----
@@ -298,8 +317,8 @@ int afm_beam_forward_batch(const double* params, int64_t n_particles,
                            const afm_bounds* bounds, double* misfit,
                            void* cuda_stream);
 
-/* afm_pso_invert around the beam forward batch: same swarm rules, same Philox
- * streams, same outputs. */
+/* afm_pso_invert around the beam forward batch: same swarm rules (cutoff, ring),
+ * same Philox streams, same outputs; the asynchronous swarm is not available. */
 int afm_beam_pso_invert(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
                         uint64_t seed, const double* trace,
                         const afm_beam_cfg* cfg, double* theta_star,

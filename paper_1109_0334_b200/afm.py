@@ -87,7 +87,7 @@ class SwarmCfg(C.Structure):
     _fields_ = [("n_particles", C.c_int32), ("n_iters", C.c_int32),
                 ("w", C.c_double), ("c1", C.c_double), ("c2", C.c_double),
                 ("j_target", C.c_double), ("topology", C.c_int32),
-                ("reserved_", C.c_int32)]
+                ("async_chunk", C.c_int32)]
 
 
 _lib = None
@@ -124,8 +124,8 @@ def lib():
         L.afm_pso_shard_eval.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), dp,
                                          C.POINTER(Cfg), i64, dp, dp, dp, dp, dp, vp]
         L.afm_pso_shard_move.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), i32,
-                                         i32, u64, i32, i32, i64, dp, i32, dp, dp, dp,
-                                         dp, dp, dp, dp, vp]
+                                         i32, u64, i32, i32, i64, dp, i32, i32, i64, dp,
+                                         dp, dp, dp, dp, dp, dp, dp, vp]
         L.afm_beam_modes.argtypes = [C.POINTER(BeamCfg), dp, dp, dp, dp, dp, vp]
         L.afm_beam_forward_batch.argtypes = [dp, i64, dp, C.POINTER(BeamCfg),
                                              C.POINTER(Bounds), dp, vp]
@@ -193,7 +193,7 @@ def swarm_from(wl, j_target=0.0, **over):
     s = wl["swarm"]
     sc = SwarmCfg(n_particles=s["n_particles"], n_iters=s["n_iters"], w=s["w"],
                   c1=s["c1"], c2=s["c2"], j_target=j_target,
-                  topology=s.get("topology", 0), reserved_=0)
+                  topology=s.get("topology", 0), async_chunk=s.get("async_chunk", 0))
     for k, v in over.items():
         setattr(sc, k, v)
     return sc
@@ -376,6 +376,12 @@ def afm_kernel_times(max_n=64):
     return [buf[i] for i in range(n.value)]
 
 
+def shard_row_doubles(n_dims, topology):
+    """Doubles per trace in a shard's candidate row (include/afm.h): D + 2, or 3 D + 4
+    with the ring topology (edge particles' personal bests ride along)."""
+    return 3 * n_dims + 4 if topology == 1 else n_dims + 2
+
+
 def afm_pso_shard_init(bounds, swarm, n_dims, n_traces, seed, first_particle,
                        stream=None):
     """Swarm state of a shard: swarm.n_particles local particles
@@ -387,7 +393,7 @@ def afm_pso_shard_init(bounds, swarm, n_dims, n_traces, seed, first_particle,
               pbest=torch.empty((PT, n_dims), **kw), pbestJ=torch.empty(PT, **kw),
               gbest=torch.empty((n_traces, n_dims), **kw),
               gbestJ=torch.empty(n_traces, **kw), J=torch.empty(PT, **kw),
-              cand=torch.empty((n_traces, n_dims + 2), **kw),
+              cand=torch.empty((n_traces, shard_row_doubles(n_dims, swarm.topology)), **kw),
               theta_star=torch.empty((n_traces, n_dims), **kw),
               J_star=torch.empty(n_traces, **kw))
     _check(lib().afm_pso_shard_init(C.byref(bounds), C.byref(swarm), n_dims, n_traces,
@@ -400,7 +406,8 @@ def afm_pso_shard_init(bounds, swarm, n_dims, n_traces, seed, first_particle,
 
 def afm_pso_shard_eval(bounds, swarm, trace, cfg, first_particle, st, stream=None):
     """Forward batch + personal bests of the shard; returns st["cand"]
-    [n_traces][D+2] = (pbestJ, global index, pbest x[D]) for the exchange."""
+    [n_traces][R] = (pbestJ, global index, pbest x[D][, edge particles' bests]) for the
+    exchange."""
     trace = _dev_f64(trace, "trace")
     if trace.numel() != cfg.n_traces * cfg.n_window:
         raise ValueError("trace must hold n_traces * W samples")
@@ -413,17 +420,23 @@ def afm_pso_shard_eval(bounds, swarm, trace, cfg, first_particle, st, stream=Non
 
 
 def afm_pso_shard_move(bounds, swarm, n_dims, n_traces, seed, iteration, do_move,
-                       first_particle, gathered, st, stream=None):
-    """Global best from the gathered candidates [n_ranks][n_traces][D+2], then the
-    Eq. 8 move of the shard."""
+                       first_particle, gathered, st, rank=0, swarm_particles=None,
+                       stream=None):
+    """Global best from the gathered candidates [n_ranks][n_traces][R], then the
+    Eq. 8 move of the shard.  rank: this process's block in `gathered`;
+    swarm_particles: particles per trace of the whole swarm (default: the shard's)."""
     gathered = _dev_f64(gathered, "gathered")
-    n_ranks = gathered.numel() // (n_traces * (n_dims + 2))
-    if n_ranks * n_traces * (n_dims + 2) != gathered.numel():
-        raise ValueError("gathered must be [n_ranks][n_traces][D+2]")
+    R = shard_row_doubles(n_dims, swarm.topology)
+    n_ranks = gathered.numel() // (n_traces * R)
+    if n_ranks * n_traces * R != gathered.numel():
+        raise ValueError("gathered must be [n_ranks][n_traces][%d]" % R)
+    total = swarm.n_particles if swarm_particles is None else int(swarm_particles)
     _check(lib().afm_pso_shard_move(C.byref(bounds), C.byref(swarm), n_dims, n_traces,
                                     int(seed), int(iteration), int(bool(do_move)),
                                     int(first_particle), _ptr(gathered), n_ranks,
+                                    int(rank), total,
                                     _ptr(st["x"]), _ptr(st["v"]), _ptr(st["pbest"]),
+                                    _ptr(st["pbestJ"]),
                                     _ptr(st["gbest"]), _ptr(st["gbestJ"]),
                                     _ptr(st["theta_star"]), _ptr(st["J_star"]),
                                     _stream_ptr(stream)))

@@ -118,19 +118,30 @@ struct Workspace {
   Buffer scratch;                      // theta for afm_trajectory
   Buffer sort;                         // warp-packing keys, order, radix-sort temp
   Buffer segq;                         // segment queue: control words, slots, checkpoints
+  Buffer chunk;                        // asynchronous swarm: theta and J of one chunk
   cudaEvent_t last_use = nullptr;      // orders reuse across streams
   cudaStream_t last_stream = nullptr;
   bool checked_device = false;
+  int device = -1;                     // owner of every buffer above
   void* pinned = nullptr;              // small pinned host block
   size_t pinned_cap = 0;
 } g_ws;
 
+// The workspace (and the SM count the launch decisions use) belongs to the device
+// that was current at the first compute call; a caller that switches devices must
+// call afm_shutdown() in between.
 int check_device() {
-  if (g_ws.checked_device) return AFM_OK;
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess)
     return fail(AFM_ECUDA, "no CUDA device: %s", cudaGetErrorString(e));
+  if (g_ws.checked_device) {
+    if (dev != g_ws.device)
+      return fail(AFM_EUNSUPPORTED,
+                  "the library workspace lives on device %d but device %d is current: "
+                  "call afm_shutdown() before switching devices", g_ws.device, dev);
+    return AFM_OK;
+  }
   cudaDeviceProp prop;
   CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
   if (prop.major != 10)
@@ -138,6 +149,7 @@ int check_device() {
                 "device %s is sm_%d%d; this library is built for sm_100a only",
                 prop.name, prop.major, prop.minor);
   g_n_sm = prop.multiProcessorCount;
+  g_ws.device = dev;
   g_ws.checked_device = true;
   return AFM_OK;
 }
@@ -294,24 +306,11 @@ void make_consts_f32(const afm_cfg* c, ModelConstsF32* mf) {
   mf->n_tiles = (mf->N + T - 1) / T;
 }
 
-int pick_block(int64_t per, int n_traces) {
-  if (g_opt_block > 0) return g_opt_block;
-  (void)per;
-  (void)n_traces;
-  return 32;
-}
-
-// Particles per thread: two interleaved chains once the batch would put at
-// least two one-particle warps on every SM sub-partition (148 x 4 of them).
-int pick_ppt(int64_t per, int n_traces) {
-  if (g_opt_ppt > 0) return g_opt_ppt;
-  // measured on B200: with >= 3 warps per SM
-  // sub-partition the issue port is already the limit and a second chain per
-  // thread only lowers the free-flight hit rate, so one particle per thread
-  (void)per;
-  (void)n_traces;
-  return 1;
-}
+// Launch shape of the integrate kernels: one warp per CTA and one particle per
+// thread unless afm_set_option says otherwise (measured on B200, DESIGN.md 6:
+// 64- and 128-thread CTAs change nothing, two particles per thread cost 28 %).
+int block_threads() { return g_opt_block > 0 ? g_opt_block : 32; }
+int particles_per_thread() { return g_opt_ppt > 0 ? g_opt_ppt : 1; }
 
 // Kernel form of the FP64 integrate kernel (afm_device.cuh, vdw_plus): the
 // latency form below two warps per SM sub-partition, where nothing hides the
@@ -501,7 +500,16 @@ int validate_swarm(const afm_swarm_cfg* s) {
     return fail(AFM_EINVAL, "w, c1, c2 must be finite");
   if (s->topology != 0 && s->topology != 1)
     return fail(AFM_EINVAL, "topology must be 0 (global best) or 1 (ring of three)");
-  if (s->reserved_ != 0) return fail(AFM_EINVAL, "swarm reserved_ must be 0");
+  if (s->async_chunk < 0) return fail(AFM_EINVAL, "async_chunk must be >= 0");
+  return AFM_OK;
+}
+
+// Entry points that step a swarm batch by batch from outside have no place for the
+// chunked, asynchronous swarm.
+int reject_async(const afm_swarm_cfg* s, const char* who) {
+  if (s->async_chunk > 0 && s->async_chunk < s->n_particles)
+    return fail(AFM_EUNSUPPORTED, "%s: the asynchronous swarm (async_chunk) runs inside "
+                                  "afm_pso_invert only", who);
   return AFM_OK;
 }
 
@@ -511,8 +519,8 @@ int forward_locked(const double* params, int64_t P, const double* trace,
                    cudaStream_t st) {
   const bool f32 = (cfg->precision == AFM_F32);
   const int64_t per = P / cfg->n_traces;
-  const int block = pick_block(per, cfg->n_traces);
-  const int ppt = pick_ppt(per, cfg->n_traces);
+  const int block = block_threads();
+  const int ppt = particles_per_thread();
   ModelConsts mc;
   ModelConstsF32 mf;
   make_consts(cfg, block, &mc);
@@ -661,6 +669,7 @@ int afm_pso_step(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   int rc = validate_bounds(bounds, n_dims);
   if (rc) return rc;
   if ((rc = validate_swarm(swarm))) return rc;
+  if ((rc = reject_async(swarm, "afm_pso_step"))) return rc;
   if (!J || !x || !v || !pbest || !pbestJ || !gbest || !gbestJ)
     return fail(AFM_EINVAL, "NULL swarm array");
   if ((rc = check_device())) return rc;
@@ -674,14 +683,14 @@ int afm_pso_step(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
     return fail(AFM_ECUDA, "cudaMalloc of candidates failed");
   BoxDev box = make_box(bounds, n_dims);
   SwarmDev sw = {swarm->w, swarm->c1, swarm->c2, swarm->topology, 0};
-  LAUNCHED(launch_pso_best(n_dims, per, n_traces, J, x, pbest, pbestJ,
-                           (Cand*)g_ws.cand.p, block, st));
+  LAUNCHED(launch_pso_best(n_dims, per, 0, per, n_traces, const_cast<double*>(J), nullptr,
+                           x, pbest, pbestJ, (Cand*)g_ws.cand.p, block, st));
   LAUNCHED(launch_pso_gbest(box, n_dims, n_traces, bpt, (Cand*)g_ws.cand.p,
                             pbest, gbest, gbestJ, nullptr, nullptr, nullptr, st));
   if (do_move)
-    LAUNCHED(launch_pso_move(box, sw, n_dims, per, n_traces, seed, 0,
-                             (uint32_t)iteration, 1, J, x, v, pbest, pbestJ,
-                             gbest, nullptr, st));
+    LAUNCHED(launch_pso_move(box, sw, n_dims, per, 0, per, n_traces, seed, 0,
+                             (uint32_t)iteration, 1, RingEdges{0, 0, nullptr, nullptr, 0}, J, x, v, pbest,
+                             pbestJ, gbest, nullptr, st));
   return release_ws(st);
 }
 
@@ -696,8 +705,8 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
   const int T = cfg->n_traces;
   const int64_t per = swarm->n_particles;
   const int64_t PT = per * T;
-  const int block = pick_block(per, T);
-  const int ppt = pick_ppt(per, T);
+  const int block = block_threads();
+  const int ppt = particles_per_thread();
   const int lanes = pick_lanes(cfg, per, T);
   const int bpt = f32 ? blocks_per_trace(per, block * ppt)
                       : integrate_bpt(per, block, ppt, pick_variant(per, T, ppt), lanes);
@@ -750,41 +759,91 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
   io.mode = 1;
   io.lanes = lanes;
 
+  // Asynchronous swarm (R25): chunks of `chunk` particles of every swarm,
+  // in index order; a chunk is integrated on its own (theta = map(x) gathered into a
+  // compact batch for the forward-only kernel), its personal bests and the swarm's
+  // best are updated from it, and it moves at once.
+  const int64_t chunk =
+      (swarm->async_chunk > 0 && swarm->async_chunk < per) ? swarm->async_chunk : per;
+  const bool asynchronous = chunk < per;
+  double* th_c = nullptr;  // [T][chunk][D]
+  double* J_c = nullptr;   // [T][chunk]
+  if (asynchronous) {
+    const size_t a256 = 255;
+    const size_t th_bytes = ((size_t)T * chunk * D * 8 + a256) & ~a256;
+    if (g_ws.chunk.ensure(th_bytes + (size_t)T * chunk * 8))
+      return fail(AFM_ECUDA, "cudaMalloc of the chunk workspace failed");
+    th_c = (double*)g_ws.chunk.p;
+    J_c = (double*)((char*)g_ws.chunk.p + th_bytes);
+  }
+  const RingEdges no_edges = {0, 0, nullptr, nullptr, 0};
+
   int done = 0;
   for (int it = 0; it < swarm->n_iters; ++it) {
     const bool last = (it == swarm->n_iters - 1);
-    // throughput regime, DMT laws: warp packing (afm_sort.cu).  The swarm state
-    // stays in particle order; theta = map(x) is gathered in packed order, the
-    // forward-only kernel runs on it, the misfits are scattered back and the
-    // stand-alone personal-best kernel takes the place of the fused epilogue.
-    Packed pk;
-    if ((rc = pack_inputs(cfg, x, nullptr, per, T, &box, &pk, st))) return rc;
-    int n_cand = bpt;
-    if (pk.order) {
-      IntegrateIO iof = io;
-      iof.params = pk.params;
-      iof.J = pk.J;
-      iof.mode = 0;
-      if (f32)
-        rc = run_integrate_f32(mf, iof, block, ppt, st);
-      else
-        rc = run_integrate_f64(mc, iof, block, pick_variant(iof.per, iof.n_traces, ppt), st);
-      if (rc) return rc;
-      LAUNCHED(launch_pack_scatter(pk.order, pk.J, PT, J, st));
-      n_cand = blocks_per_trace(per, 128);
-      LAUNCHED(launch_pso_best(D, per, T, J, x, pbest, pbestJ, (Cand*)g_ws.cand.p, 128,
-                               st));
+    double* hist_row = gbest_hist ? gbest_hist + (size_t)it * T * (D + 1) : nullptr;
+    double* dump_row =
+        swarm_dump ? swarm_dump + (size_t)it * PT * (3 * D + 2) : nullptr;
+    if (asynchronous) {
+      for (int64_t c0 = 0; c0 < per; c0 += chunk) {
+        const int64_t cn = (c0 + chunk < per) ? chunk : per - c0;
+        const bool last_chunk = (c0 + cn == per);
+        LAUNCHED(launch_chunk_gather(box, D, per, c0, cn, T, x, th_c, st));
+        IntegrateIO ioc = io;
+        ioc.params = th_c;
+        ioc.J = J_c;
+        ioc.per = cn;
+        ioc.mode = 0;
+        ioc.lanes = pick_lanes(cfg, cn, T);
+        if (f32)
+          rc = run_integrate_f32(mf, ioc, block, ppt, st);
+        else
+          rc = run_integrate_f64(mc, ioc, block, pick_variant(cn, T, ppt), st);
+        if (rc) return rc;
+        LAUNCHED(launch_pso_best(D, per, c0, cn, T, J, J_c, x, pbest, pbestJ,
+                                 (Cand*)g_ws.cand.p, 128, st));
+        LAUNCHED(launch_pso_gbest(box, D, T, blocks_per_trace(cn, 128), (Cand*)g_ws.cand.p,
+                                  pbest, gbest, gbestJ, last_chunk ? hist_row : nullptr,
+                                  th_dev, Js_dev, st));
+        if (!last || dump_row)
+          LAUNCHED(launch_pso_move(box, sw, D, per, c0, cn, T, seed, 0, (uint32_t)it,
+                                   last ? 0 : 1, no_edges, J, x, v, pbest, pbestJ, gbest,
+                                   dump_row, st));
+      }
     } else {
-      if (f32)
-        rc = run_integrate_f32(mf, io, block, ppt, st);
-      else
-        rc = run_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st);
-      if (rc) return rc;
+      // throughput regime, DMT laws: warp packing (afm_sort.cu).  The swarm state
+      // stays in particle order; theta = map(x) is gathered in packed order, the
+      // forward-only kernel runs on it, the misfits are scattered back and the
+      // stand-alone personal-best kernel takes the place of the fused epilogue.
+      Packed pk;
+      if ((rc = pack_inputs(cfg, x, nullptr, per, T, &box, &pk, st))) return rc;
+      int n_cand = bpt;
+      if (pk.order) {
+        IntegrateIO iof = io;
+        iof.params = pk.params;
+        iof.J = pk.J;
+        iof.mode = 0;
+        if (f32)
+          rc = run_integrate_f32(mf, iof, block, ppt, st);
+        else
+          rc = run_integrate_f64(mc, iof, block, pick_variant(iof.per, iof.n_traces, ppt),
+                                 st);
+        if (rc) return rc;
+        LAUNCHED(launch_pack_scatter(pk.order, pk.J, PT, J, st));
+        n_cand = blocks_per_trace(per, 128);
+        LAUNCHED(launch_pso_best(D, per, 0, per, T, J, nullptr, x, pbest, pbestJ,
+                                 (Cand*)g_ws.cand.p, 128, st));
+      } else {
+        if (f32)
+          rc = run_integrate_f32(mf, io, block, ppt, st);
+        else
+          rc = run_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st);
+        if (rc) return rc;
+      }
+      LAUNCHED(launch_pso_gbest(box, D, T, n_cand, (Cand*)g_ws.cand.p, pbest, gbest, gbestJ,
+                                hist_row, th_dev, Js_dev, st));
     }
-    LAUNCHED(launch_pso_gbest(
-        box, D, T, n_cand, (Cand*)g_ws.cand.p, pbest, gbest, gbestJ,
-        gbest_hist ? gbest_hist + (size_t)it * T * (D + 1) : nullptr, th_dev,
-        Js_dev, st));
+    // cost cutoff (R24): once per batch, after the best updates
     bool stop = last;
     if (!stop && swarm->j_target > 0) {
       double* hJ = (double*)g_ws.pinned;
@@ -794,11 +853,9 @@ static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swar
       for (int s = 0; s < T; ++s)
         if (!(hJ[s] <= swarm->j_target)) stop = false;
     }
-    double* dump_row =
-        swarm_dump ? swarm_dump + (size_t)it * PT * (3 * D + 2) : nullptr;
-    if (!stop || dump_row)
-      LAUNCHED(launch_pso_move(box, sw, D, per, T, seed, 0, (uint32_t)it,
-                               stop ? 0 : 1, J, x, v, pbest, pbestJ, gbest,
+    if (!asynchronous && (!stop || dump_row))
+      LAUNCHED(launch_pso_move(box, sw, D, per, 0, per, T, seed, 0, (uint32_t)it,
+                               stop ? 0 : 1, no_edges, J, x, v, pbest, pbestJ, gbest,
                                dump_row, st));
     done = it + 1;
     if (stop) break;
@@ -872,6 +929,7 @@ int afm_pso_shard_eval(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   if (cfg->n_params < 1) return fail(AFM_EINVAL, "n_params = 0");
   if ((rc = validate_bounds(bounds, cfg->n_params))) return rc;
   if ((rc = validate_swarm(swarm))) return rc;
+  if ((rc = reject_async(swarm, "afm_pso_shard_eval"))) return rc;
   if (first_particle < 0) return fail(AFM_EINVAL, "first_particle must be >= 0");
   if (!trace || !x || !J || !pbest || !pbestJ || !cand_out)
     return fail(AFM_EINVAL, "NULL array");
@@ -881,8 +939,8 @@ int afm_pso_shard_eval(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   const bool f32 = (cfg->precision == AFM_F32);
   const int D = cfg->n_params, T = cfg->n_traces;
   const int64_t per = swarm->n_particles;
-  const int block = pick_block(per, T);
-  const int ppt = pick_ppt(per, T);
+  const int block = block_threads();
+  const int ppt = particles_per_thread();
   const int lanes = pick_lanes(cfg, per, T);
   const int bpt = f32 ? blocks_per_trace(per, block * ppt)
                       : integrate_bpt(per, block, ppt, pick_variant(per, T, ppt), lanes);
@@ -916,8 +974,8 @@ int afm_pso_shard_eval(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   else
     rc = run_integrate_f64(mc, io, block, pick_variant(io.per, io.n_traces, ppt), st);
   if (rc) return rc;
-  LAUNCHED(launch_pso_shard_cand(D, T, bpt, first_particle, (Cand*)g_ws.cand.p,
-                                 pbest, cand_out, st));
+  LAUNCHED(launch_pso_shard_cand(D, T, bpt, first_particle, per, swarm->topology == 1,
+                                 (Cand*)g_ws.cand.p, pbest, pbestJ, cand_out, st));
   return release_ws(st);
 }
 
@@ -925,33 +983,52 @@ int afm_pso_shard_move(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
                        int32_t n_dims, int32_t n_traces, uint64_t seed,
                        int32_t iteration, int32_t do_move,
                        int64_t first_particle, const double* gathered,
-                       int32_t n_ranks, double* x, double* v,
-                       const double* pbest, double* gbest, double* gbestJ,
+                       int32_t n_ranks, int32_t rank, int64_t swarm_particles,
+                       double* x, double* v, const double* pbest,
+                       const double* pbestJ, double* gbest, double* gbestJ,
                        double* theta_star, double* J_star, void* cuda_stream) {
   if (n_dims < 1 || n_dims > 4) return fail(AFM_EINVAL, "n_dims must be 1..4");
   if (n_traces < 1) return fail(AFM_EINVAL, "n_traces must be >= 1");
   if (n_ranks < 1) return fail(AFM_EINVAL, "n_ranks must be >= 1");
+  if (rank < 0 || rank >= n_ranks) return fail(AFM_EINVAL, "rank must be in [0, n_ranks)");
   if (iteration < 0) return fail(AFM_EINVAL, "iteration must be >= 0");
   if (first_particle < 0) return fail(AFM_EINVAL, "first_particle must be >= 0");
   int rc = validate_bounds(bounds, n_dims);
   if (rc) return rc;
   if ((rc = validate_swarm(swarm))) return rc;
-  if (swarm->topology != 0)
-    return fail(AFM_EUNSUPPORTED,
-                "the ring topology needs its neighbours' personal bests: not "
-                "available for a sharded swarm");
+  if ((rc = reject_async(swarm, "afm_pso_shard_move"))) return rc;
+  if (swarm_particles < swarm->n_particles)
+    return fail(AFM_EINVAL, "swarm_particles %lld is smaller than the shard's %d",
+                (long long)swarm_particles, swarm->n_particles);
   if (!gathered || !x || !v || !pbest || !gbest || !gbestJ)
     return fail(AFM_EINVAL, "NULL swarm array");
+  const bool ring = (swarm->topology == 1);
+  if (ring && !pbestJ) return fail(AFM_EINVAL, "the ring topology needs pbestJ");
+  if (ring && swarm_particles > swarm->n_particles && n_traces != 1)
+    return fail(AFM_EINVAL, "a swarm split over ranks is one trace per call");
   if ((rc = check_device())) return rc;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   BoxDev box = make_box(bounds, n_dims);
   SwarmDev sw = {swarm->w, swarm->c1, swarm->c2, swarm->topology, 0};
-  LAUNCHED(launch_pso_shard_gbest(box, n_dims, n_traces, n_ranks, gathered, gbest,
+  const int width = ring ? 3 * n_dims + 4 : n_dims + 2;
+  LAUNCHED(launch_pso_shard_gbest(box, n_dims, n_traces, n_ranks, width, gathered, gbest,
                                   gbestJ, theta_star, J_star, st));
-  if (do_move)
-    LAUNCHED(launch_pso_move(box, sw, n_dims, swarm->n_particles, n_traces, seed,
-                             first_particle, (uint32_t)iteration, 1, nullptr, x,
-                             v, pbest, nullptr, gbest, nullptr, st));
+  if (do_move) {
+    RingEdges re = {0, 0, nullptr, nullptr, 0};
+    if (ring && swarm_particles > swarm->n_particles) {
+      // the neighbours of the shard's edge particles: last particle of the rank
+      // before, first particle of the rank after (ranks hold consecutive slices)
+      const int before = (rank + n_ranks - 1) % n_ranks, after = (rank + 1) % n_ranks;
+      re.total = swarm_particles;
+      re.off = first_particle % swarm_particles;
+      re.stride = width;
+      re.left = gathered + (size_t)before * n_traces * width + (n_dims + 2) + (n_dims + 1);
+      re.right = gathered + (size_t)after * n_traces * width + (n_dims + 2);
+    }
+    LAUNCHED(launch_pso_move(box, sw, n_dims, swarm->n_particles, 0, swarm->n_particles,
+                             n_traces, seed, first_particle, (uint32_t)iteration, 1, re,
+                             nullptr, x, v, pbest, pbestJ, gbest, nullptr, st));
+  }
   return AFM_OK;
 }
 
@@ -1098,7 +1175,7 @@ int afm_beam_forward_batch(const double* params, int64_t n_particles,
     io.box = make_box(bounds, cfg->n_params);
     io.mode = 2;
   }
-  LAUNCHED(launch_beam_integrate(bc, mo, io, pick_block(io.per, io.n_traces), st));
+  LAUNCHED(launch_beam_integrate(bc, mo, io, block_threads(), st));
   return release_ws(st);
 }
 
@@ -1112,6 +1189,7 @@ int afm_beam_pso_invert(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   if (cfg->n_params < 1) return fail(AFM_EINVAL, "nothing to invert: n_params = 0");
   if ((rc = validate_bounds(bounds, cfg->n_params))) return rc;
   if ((rc = validate_swarm(swarm))) return rc;
+  if ((rc = reject_async(swarm, "afm_beam_pso_invert"))) return rc;
   if (!trace || !theta_star || !J_star)
     return fail(AFM_EINVAL, "trace/theta_star/J_star is NULL");
   if ((rc = check_device())) return rc;
@@ -1124,7 +1202,7 @@ int afm_beam_pso_invert(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   if ((rc = beam_stream(bc, trace, cfg->n_traces, st))) return rc;
   const int D = cfg->n_params, T = cfg->n_traces;
   const int64_t per = swarm->n_particles, PT = per * T;
-  const int block = pick_block(per, T);
+  const int block = block_threads();
   const int bpt = blocks_per_trace(per, block);
   const size_t n_dbl = (size_t)PT * (3 * D + 2) + (size_t)T * (2 * D + 2);
   if (g_ws.swarm.ensure(n_dbl * 8) || g_ws.cand.ensure((size_t)bpt * T * sizeof(Cand)))
@@ -1175,9 +1253,9 @@ int afm_beam_pso_invert(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
     double* dump_row =
         swarm_dump ? swarm_dump + (size_t)it * PT * (3 * D + 2) : nullptr;
     if (!stop || dump_row)
-      LAUNCHED(launch_pso_move(box, sw, D, per, T, seed, 0, (uint32_t)it,
-                               stop ? 0 : 1, J, x, v, pbest, pbestJ, gbest,
-                               dump_row, st));
+      LAUNCHED(launch_pso_move(box, sw, D, per, 0, per, T, seed, 0, (uint32_t)it,
+                               stop ? 0 : 1, RingEdges{0, 0, nullptr, nullptr, 0}, J, x, v,
+                               pbest, pbestJ, gbest, dump_row, st));
     done = it + 1;
     if (stop) break;
   }
@@ -1437,12 +1515,21 @@ void afm_shutdown(void) {
   g_ws.scratch.release();
   g_ws.sort.release();
   g_ws.segq.release();
+  g_ws.chunk.release();
   if (g_ws.pinned) cudaFreeHost(g_ws.pinned);
   g_ws.pinned = nullptr;
   g_ws.pinned_cap = 0;
   if (g_ws.last_use) cudaEventDestroy(g_ws.last_use);
   g_ws.last_use = nullptr;
   g_ws.last_stream = nullptr;
+  if (g_kev_made) {
+    for (int i = 0; i < kMaxKernelEvents; ++i)
+      for (int j = 0; j < 2; ++j) cudaEventDestroy(g_kev[i][j]);
+    g_kev_made = false;
+  }
+  g_kev_count = 0;
+  g_ws.checked_device = false;
+  g_ws.device = -1;
 }
 
 }  // extern "C"

@@ -161,23 +161,38 @@ int launch_pso_init(const BoxDev& box, int D, int64_t per, int n_traces,
                     uint64_t seed, int64_t first, double* x, double* v,
                     double* pbest, double* pbestJ, double* gbest, double* gbestJ,
                     cudaStream_t st);
-int launch_pso_best(int D, int64_t per, int n_traces, const double* J,
-                    const double* x, double* pbest, double* pbestJ, Cand* cand,
-                    int block, cudaStream_t st);
+// Ring of three in a sharded swarm: where the neighbours outside the shard live.
+// total = 0: the shard holds whole swarms (plain wrap inside the local swarm).
+struct RingEdges {
+  int64_t total;        // particles of the whole swarm over all shards, or 0
+  int64_t off;          // in-swarm index of local particle 0
+  const double* left;   // { pbestJ, pbest x[D] } of the particle before the shard,
+  const double* right;  //   after the shard; trace 0's row, `stride` doubles per trace
+  int64_t stride;
+};
+
+int launch_pso_best(int D, int64_t per, int64_t off, int64_t cnt, int n_traces,
+                    double* J, const double* Jc, const double* x, double* pbest,
+                    double* pbestJ, Cand* cand, int block, cudaStream_t st);
+int launch_chunk_gather(const BoxDev& box, int D, int64_t per, int64_t off,
+                        int64_t cnt, int n_traces, const double* x, double* theta_c,
+                        cudaStream_t st);
 int launch_pso_gbest(const BoxDev& box, int D, int n_traces, int n_cand,
                      const Cand* cand, const double* pbest, double* gbest,
                      double* gbestJ, double* hist_row, double* theta_star,
                      double* J_star, cudaStream_t st);
 int launch_pso_move(const BoxDev& box, const SwarmDev& sw, int D, int64_t per,
-                    int n_traces, uint64_t seed, int64_t first, uint32_t it,
-                    int do_move, const double* J, double* x, double* v,
-                    const double* pbest, const double* pbestJ,
-                    const double* gbest, double* dump_row, cudaStream_t st);
+                    int64_t off, int64_t cnt, int n_traces, uint64_t seed,
+                    int64_t first, uint32_t it, int do_move, const RingEdges& re,
+                    const double* J, double* x, double* v, const double* pbest,
+                    const double* pbestJ, const double* gbest, double* dump_row,
+                    cudaStream_t st);
 int launch_pso_shard_cand(int D, int n_traces, int n_cand, int64_t first,
-                          const Cand* cand, const double* pbest,
+                          int64_t per, int ring, const Cand* cand,
+                          const double* pbest, const double* pbestJ,
                           double* cand_out, cudaStream_t st);
 int launch_pso_shard_gbest(const BoxDev& box, int D, int n_traces, int n_ranks,
-                           const double* gathered, double* gbest,
+                           int width, const double* gathered, double* gbest,
                            double* gbestJ, double* theta_star, double* J_star,
                            cudaStream_t st);
 int launch_fma_peak(int precision, int iters, int blocks, int threads,

@@ -544,9 +544,13 @@ __global__ void pso_init_kernel(BoxDev box, int D, int64_t per, int n_traces,
 }
 
 // Personal best from caller-supplied J + block candidates (the stand-alone
-// form of the epilogue fused into integrate_misfit_f64<., 1>).
-__global__ void pso_best_kernel(int D, int64_t per, int blocks_per_tr,
-                                const double* __restrict__ J,
+// form of the epilogue fused into integrate_misfit_f64<., 1>), for the particles
+// [off, off + cnt) of every swarm.  Jc != nullptr: the misfits arrive compact,
+// [n_traces][cnt] (asynchronous swarm: a chunk was integrated on its own), and
+// are also stored at the particles' own places in J.
+__global__ void pso_best_kernel(int D, int64_t per, int64_t off, int64_t cnt,
+                                int blocks_per_tr, double* __restrict__ J,
+                                const double* __restrict__ Jc,
                                 const double* __restrict__ x,
                                 double* __restrict__ pbest,
                                 double* __restrict__ pbestJ,
@@ -555,12 +559,18 @@ __global__ void pso_best_kernel(int D, int64_t per, int blocks_per_tr,
   const int s = blockIdx.x / blocks_per_tr;
   const int64_t li =
       (int64_t)(blockIdx.x - s * blocks_per_tr) * blockDim.x + threadIdx.x;
-  const bool active = li < per;
-  const int64_t gp = (int64_t)s * per + li;
+  const bool active = li < cnt;
+  const int64_t gp = (int64_t)s * per + off + li;
   double pb = CUDART_INF;
   long long idx = 0x7fffffffffffffffLL;
   if (active) {
-    const double Jp = J[gp];
+    double Jp;
+    if (Jc != nullptr) {
+      Jp = Jc[(int64_t)s * cnt + li];
+      J[gp] = Jp;
+    } else {
+      Jp = J[gp];
+    }
     pb = pbestJ[gp];
     if (Jp < pb) {
       pb = Jp;
@@ -573,6 +583,22 @@ __global__ void pso_best_kernel(int D, int64_t per, int blocks_per_tr,
   if (threadIdx.x == 0) {
     cand[blockIdx.x].J = pb;
     cand[blockIdx.x].idx = idx;
+  }
+}
+
+// theta = map(x) of the particles [off, off + cnt) of every swarm, compact
+// [n_traces][cnt][D]: the forward batch of one chunk of an asynchronous swarm.
+__global__ void chunk_gather_kernel(BoxDev box, int D, int64_t per, int64_t off,
+                                    int64_t cnt, int n_traces,
+                                    const double* __restrict__ x,
+                                    double* __restrict__ theta_c) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= cnt * n_traces) return;
+  const int64_t s = i / cnt;
+  const int64_t gp = s * per + off + (i - s * cnt);
+  for (int j = 0; j < D; ++j) {
+    const double xv = x[gp * D + j];
+    theta_c[i * D + j] = box.lg[j] ? pow(10.0, xv) : xv;
   }
 }
 
@@ -617,10 +643,14 @@ __global__ void pso_gbest_kernel(BoxDev box, int D, int n_cand,
 
 // Sharded swarm: this process's best candidate of every local
 // trace, in a form that can be exchanged: row s = { pbestJ, global particle
-// index (exact in a double below 2^53), pbest x[D] }.
-__global__ void pso_shard_cand_kernel(int D, int n_cand, int64_t first,
-                                      const Cand* __restrict__ cand,
+// index (exact in a double below 2^53), pbest x[D] }.  With the ring topology the
+// row also carries the personal bests of the shard's first and last particle,
+// { pbestJ, pbest x[D] } each, which are the ring neighbours of the adjacent
+// shards: 3 D + 4 doubles.
+__global__ void pso_shard_cand_kernel(int D, int n_cand, int64_t first, int64_t per,
+                                      int ring, const Cand* __restrict__ cand,
                                       const double* __restrict__ pbest,
+                                      const double* __restrict__ pbestJ,
                                       double* __restrict__ cand_out) {
   __shared__ Cand red[32];
   const int s = blockIdx.x;
@@ -635,10 +665,20 @@ __global__ void pso_shard_cand_kernel(int D, int n_cand, int64_t first,
   }
   block_argmin(Jm, im, red);
   if (threadIdx.x == 0) {
-    double* r = cand_out + (int64_t)s * (D + 2);
+    const int width = ring ? 3 * D + 4 : D + 2;
+    double* r = cand_out + (int64_t)s * width;
     r[0] = Jm;
     r[1] = (double)(first + im);
     for (int j = 0; j < D; ++j) r[2 + j] = pbest[im * D + j];
+    if (ring) {
+      const int64_t p0 = (int64_t)s * per, p1 = p0 + per - 1;
+      double* e = r + D + 2;
+      e[0] = pbestJ[p0];
+      for (int j = 0; j < D; ++j) e[1 + j] = pbest[p0 * D + j];
+      e += D + 1;
+      e[0] = pbestJ[p1];
+      for (int j = 0; j < D; ++j) e[1 + j] = pbest[p1 * D + j];
+    }
   }
 }
 
@@ -646,7 +686,7 @@ __global__ void pso_shard_cand_kernel(int D, int n_cand, int64_t first,
 // (gathered [n_ranks][n_traces][D+2]): lowest global index among the minima,
 // taken only on a strict improvement -- the rule of pso_gbest_kernel.
 __global__ void pso_shard_gbest_kernel(BoxDev box, int D, int n_traces,
-                                       int n_ranks,
+                                       int n_ranks, int width,
                                        const double* __restrict__ gathered,
                                        double* __restrict__ gbest,
                                        double* __restrict__ gbestJ,
@@ -658,7 +698,7 @@ __global__ void pso_shard_gbest_kernel(BoxDev box, int D, int n_traces,
   long long im = 0x7fffffffffffffffLL;
   int rm = -1;
   for (int r = 0; r < n_ranks; ++r) {
-    const double* row = gathered + ((int64_t)r * n_traces + s) * (D + 2);
+    const double* row = gathered + ((int64_t)r * n_traces + s) * width;
     const long long idx = (long long)row[1];
     if (cand_less(row[0], idx, Jm, im)) {
       Jm = row[0];
@@ -670,7 +710,7 @@ __global__ void pso_shard_gbest_kernel(BoxDev box, int D, int n_traces,
   if (rm >= 0 && Jm < gJ) {
     gJ = Jm;
     gbestJ[s] = Jm;
-    const double* row = gathered + ((int64_t)rm * n_traces + s) * (D + 2);
+    const double* row = gathered + ((int64_t)rm * n_traces + s) * width;
     for (int j = 0; j < D; ++j) gbest[s * D + j] = row[2 + j];
   }
   for (int j = 0; j < D; ++j) {
@@ -680,20 +720,36 @@ __global__ void pso_shard_gbest_kernel(BoxDev box, int D, int n_traces,
   if (J_star) J_star[s] = gJ;
 }
 
-// Optional dump, then Eq. 8, x <- x + v, clamp + zero velocity.
+// Optional dump, then Eq. 8, x <- x + v, clamp + zero velocity, for
+// the particles [off, off + cnt) of every (local) swarm.
+// Ring of three (R23): the social attractor is the best personal best among the
+// in-swarm indices g - 1, g, g + 1 (mod the swarm size rg.total), g = rg.off +
+// local index; a neighbour outside this shard is the last particle of the shard
+// before (row rg.left) or the first particle of the shard after (row rg.right),
+// { pbestJ, pbest x[D] } per trace, rg.stride doubles apart.
+struct RingShard {
+  int64_t total;        // particles of the whole swarm (all shards)
+  int64_t off;          // in-swarm index of this shard's local particle 0
+  const double* left;   // neighbour rows of trace 0, or nullptr (whole swarm here)
+  const double* right;
+  int64_t stride;
+};
+
 __global__ void pso_move_kernel(BoxDev box, SwarmDev sw, int D, int64_t per,
-                                int n_traces, uint64_t seed, int64_t first,
-                                uint32_t it, int do_move,
+                                int64_t off, int64_t cnt, int n_traces,
+                                uint64_t seed, int64_t first, uint32_t it,
+                                int do_move, RingShard rg,
                                 const double* __restrict__ J,
                                 double* __restrict__ x, double* __restrict__ v,
                                 const double* __restrict__ pbest,
                                 const double* __restrict__ pbestJ,
                                 const double* __restrict__ gbest,
                                 double* __restrict__ dump_row) {
-  const int64_t gp = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const int64_t PT = per * n_traces;
-  if (gp >= PT) return;
-  const int64_t s = gp / per;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= cnt * n_traces) return;
+  const int64_t s = i / cnt;
+  const int64_t p = off + (i - s * cnt);  // local index inside the (local) swarm
+  const int64_t gp = s * per + p;
   double xi[4], vi[4], pb[4];
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
@@ -719,21 +775,33 @@ __global__ void pso_move_kernel(BoxDev box, SwarmDev sw, int D, int64_t per,
   if (!do_move) return;
   double r1[4], r2[4];
   pso_uniforms(seed, (uint64_t)(first + gp), it, 1u, D, r1, r2);
-  // social attractor: the swarm's best, or (ring of three, R23) the best
-  // personal best among p-1, p, p+1 inside the swarm of trace s
   const double* social = gbest + s * D;
   if (sw.topology == 1) {
-    const int64_t p = gp - s * per;
-    const int64_t c0 = (p + per - 1) % per, c2 = (p + 1) % per;
-    int64_t best = c0;
-    double Jb = pbestJ[s * per + c0];
-    const double J1 = pbestJ[gp], J2 = pbestJ[s * per + c2];
-    if (J1 < Jb || (J1 == Jb && p < best)) {
-      best = p;
+    const int64_t g = rg.off + p;
+    const int64_t gl = (g + rg.total - 1) % rg.total, gr = (g + 1) % rg.total;
+    // personal best (J, position) of in-swarm index c
+    auto best_of = [&](int64_t c, double& Jc) -> const double* {
+      const int64_t lc = c - rg.off;
+      if (lc >= 0 && lc < per) {
+        Jc = pbestJ[s * per + lc];
+        return pbest + (s * per + lc) * D;
+      }
+      const double* row = (c == gl ? rg.left : rg.right) + s * rg.stride;
+      Jc = row[0];
+      return row + 1;
+    };
+    double Jb, J1, J2;
+    const double* xb = best_of(gl, Jb);
+    int64_t best = gl;
+    const double* x1 = best_of(g, J1);
+    if (J1 < Jb || (J1 == Jb && g < best)) {
+      best = g;
       Jb = J1;
+      xb = x1;
     }
-    if (J2 < Jb || (J2 == Jb && c2 < best)) best = c2;
-    social = pbest + (s * per + best) * D;
+    const double* x2 = best_of(gr, J2);
+    if (J2 < Jb || (J2 == Jb && gr < best)) xb = x2;
+    social = xb;
   }
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
@@ -905,12 +973,22 @@ int launch_pso_init(const BoxDev& box, int D, int64_t per, int n_traces,
   return 1;
 }
 
-int launch_pso_best(int D, int64_t per, int n_traces, const double* J,
-                    const double* x, double* pbest, double* pbestJ, Cand* cand,
-                    int block, cudaStream_t st) {
-  const int bpt = blocks_per_trace(per, block);
+int launch_pso_best(int D, int64_t per, int64_t off, int64_t cnt, int n_traces,
+                    double* J, const double* Jc, const double* x, double* pbest,
+                    double* pbestJ, Cand* cand, int block, cudaStream_t st) {
+  const int bpt = blocks_per_trace(cnt, block);
   pso_best_kernel<<<(unsigned)(bpt * n_traces), block, 0, st>>>(
-      D, per, bpt, J, x, pbest, pbestJ, cand);
+      D, per, off, cnt, bpt, J, Jc, x, pbest, pbestJ, cand);
+  return 1;
+}
+
+int launch_chunk_gather(const BoxDev& box, int D, int64_t per, int64_t off,
+                        int64_t cnt, int n_traces, const double* x, double* theta_c,
+                        cudaStream_t st) {
+  const int threads = 128;
+  const int64_t n = cnt * n_traces;
+  chunk_gather_kernel<<<(unsigned)((n + threads - 1) / threads), threads, 0, st>>>(
+      box, D, per, off, cnt, n_traces, x, theta_c);
   return 1;
 }
 
@@ -925,36 +1003,44 @@ int launch_pso_gbest(const BoxDev& box, int D, int n_traces, int n_cand,
 }
 
 int launch_pso_move(const BoxDev& box, const SwarmDev& sw, int D, int64_t per,
-                    int n_traces, uint64_t seed, int64_t first, uint32_t it,
-                    int do_move, const double* J, double* x, double* v,
-                    const double* pbest,
+                    int64_t off, int64_t cnt, int n_traces, uint64_t seed,
+                    int64_t first, uint32_t it, int do_move, const RingEdges& re,
+                    const double* J, double* x, double* v, const double* pbest,
                     const double* pbestJ, const double* gbest, double* dump_row,
                     cudaStream_t st) {
-  const int64_t PT = per * n_traces;
+  const int64_t n = cnt * n_traces;
   const int threads = 128;
-  pso_move_kernel<<<(unsigned)((PT + threads - 1) / threads), threads, 0, st>>>(
-      box, sw, D, per, n_traces, seed, first, it, do_move, J, x, v, pbest,
-      pbestJ, gbest, dump_row);
+  RingShard rg;
+  rg.total = re.total > 0 ? re.total : per;
+  rg.off = re.total > 0 ? re.off : 0;
+  rg.left = re.left;
+  rg.right = re.right;
+  rg.stride = re.stride;
+  pso_move_kernel<<<(unsigned)((n + threads - 1) / threads), threads, 0, st>>>(
+      box, sw, D, per, off, cnt, n_traces, seed, first, it, do_move, rg, J, x, v,
+      pbest, pbestJ, gbest, dump_row);
   return 1;
 }
 
 int launch_pso_shard_cand(int D, int n_traces, int n_cand, int64_t first,
-                          const Cand* cand, const double* pbest,
+                          int64_t per, int ring, const Cand* cand,
+                          const double* pbest, const double* pbestJ,
                           double* cand_out, cudaStream_t st) {
   int threads = n_cand <= 32 ? 32 : (n_cand <= 64 ? 64 : 128);
   pso_shard_cand_kernel<<<(unsigned)n_traces, threads, 0, st>>>(
-      D, n_cand, first, cand, pbest, cand_out);
+      D, n_cand, first, per, ring, cand, pbest, pbestJ, cand_out);
   return 1;
 }
 
 int launch_pso_shard_gbest(const BoxDev& box, int D, int n_traces, int n_ranks,
-                           const double* gathered, double* gbest,
+                           int width, const double* gathered, double* gbest,
                            double* gbestJ, double* theta_star, double* J_star,
                            cudaStream_t st) {
   const int threads = 64;
   pso_shard_gbest_kernel<<<(unsigned)((n_traces + threads - 1) / threads),
-                           threads, 0, st>>>(box, D, n_traces, n_ranks, gathered,
-                                             gbest, gbestJ, theta_star, J_star);
+                           threads, 0, st>>>(box, D, n_traces, n_ranks, width,
+                                             gathered, gbest, gbestJ, theta_star,
+                                             J_star);
   return 1;
 }
 

@@ -5,9 +5,11 @@ Two ways to shard, both with every arithmetic step inside the CUDA library:
 
 * ``shard="particles"`` -- one trace, the particles split into contiguous
   slices.  Per iteration each rank evaluates its slice (afm_pso_shard_eval),
-  the ranks all-gather ONE candidate row of D + 2 doubles each (the only data
-  exchange; NCCL over NVLink on GPUs, gloo in the CPU tests), and every rank
-  picks the same global best and moves its slice (afm_pso_shard_move).
+  the ranks all-gather ONE candidate row each (D + 2 doubles; 3 D + 4 with the
+  ring topology, whose rows also carry the personal bests of the slice's first
+  and last particle, the ring neighbours of the adjacent slices) -- the only
+  data exchange; NCCL over NVLink on GPUs, gloo in the CPU tests -- and every
+  rank picks the same global best and moves its slice (afm_pso_shard_move).
 * ``shard="traces"`` -- configs[4]: whole pixels per rank, no collective in the
   loop at all; the per-pixel results are gathered once at the end.
 
@@ -50,9 +52,10 @@ class CudaBackend:
         return self.afm.afm_pso_shard_eval(bounds, swarm, trace, cfg, first, st)
 
     def move(self, bounds, swarm, n_dims, n_traces, seed, it, do_move, first,
-             gathered, st):
+             gathered, st, rank=0, swarm_particles=None):
         return self.afm.afm_pso_shard_move(bounds, swarm, n_dims, n_traces, seed, it,
-                                           do_move, first, gathered, st)
+                                           do_move, first, gathered, st, rank=rank,
+                                           swarm_particles=swarm_particles)
 
 
 class ShardedSwarm:
@@ -135,7 +138,9 @@ class ShardedSwarm:
         else:
             gathered = cand.reshape((1,) + tuple(cand.shape))
         self.backend.move(self.bounds, self.swarm, self.D, self.n_traces, self.seed,
-                          self.iteration, do_move, self.first, gathered, st)
+                          self.iteration, do_move, self.first, gathered, st,
+                          rank=self.rank if self.exchange else 0,
+                          swarm_particles=self.global_per)
         self.iteration += 1
         return st
 

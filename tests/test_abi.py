@@ -145,8 +145,24 @@ def test_new_entry_points_validate_before_touching_the_device(lib):
                                   p16, p16, None) == afm.EINVAL
     assert lib.afm_pso_shard_eval(C.byref(b), C.byref(sw), p16, C.byref(c0), -5, p16, p16,
                                   p16, p16, p16, None) == afm.EINVAL
-    assert lib.afm_pso_shard_move(C.byref(b), C.byref(sw), 2, 1, 0, 0, 1, 0, p16, 0, p16, p16,
-                                  p16, p16, p16, None, None, None) == afm.EINVAL
+    def shard_move(n_ranks=1, rank=0, total=64, swarm=sw, pbestJ=p16):
+        return lib.afm_pso_shard_move(C.byref(b), C.byref(swarm), 2, 1, 0, 0, 1, 0, p16,
+                                      n_ranks, rank, total, p16, p16, p16, pbestJ, p16, p16,
+                                      None, None, None)
+    assert shard_move(n_ranks=0) == afm.EINVAL
+    assert shard_move(n_ranks=2, rank=2) == afm.EINVAL
+    assert shard_move(total=10) == afm.EINVAL          # smaller than the shard itself
+    ring = afm.swarm_from(w0, topology=1)
+    assert shard_move(swarm=ring, pbestJ=None) == afm.EINVAL
+    chunked = afm.swarm_from(w0, async_chunk=8)
+    assert shard_move(swarm=chunked) == afm.EUNSUPPORTED
+    assert lib.afm_pso_shard_eval(C.byref(b), C.byref(chunked), p16, C.byref(c0), 0, p16, p16,
+                                  p16, p16, p16, None) == afm.EUNSUPPORTED
+    assert lib.afm_pso_step(C.byref(b), C.byref(chunked), 2, 1, 0, 0, 1, p16, p16, p16, p16,
+                            p16, p16, p16, None) == afm.EUNSUPPORTED
+    bad = afm.swarm_from(w0, async_chunk=-1)
+    assert lib.afm_pso_step(C.byref(b), C.byref(bad), 2, 1, 0, 0, 1, p16, p16, p16, p16,
+                            p16, p16, p16, None) == afm.EINVAL
     out = C.c_double(0.0)
     assert lib.afm_fma_peak(7, 0.1, C.byref(out), None) == afm.EINVAL
     assert lib.afm_fma_peak(0, 100.0, C.byref(out), None) == afm.EINVAL

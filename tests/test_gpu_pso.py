@@ -29,14 +29,16 @@ def afm():
     return m
 
 
-def _both(afm, wl, trace, seed=None, dump=True):
+def _both(afm, wl, trace, seed=None, dump=True, j_target=0.0, async_chunk=0):
     import torch
     seed = wl["pso_seed"] if seed is None else seed
     cfg = afm.cfg_from(wl)
-    g = afm.afm_pso_invert(afm.bounds_from(wl), afm.swarm_from(wl), seed,
-                           torch.as_tensor(np.ascontiguousarray(trace), device="cuda"),
+    g = afm.afm_pso_invert(afm.bounds_from(wl),
+                           afm.swarm_from(wl, j_target=j_target, async_chunk=async_chunk),
+                           seed, torch.as_tensor(np.ascontiguousarray(trace), device="cuda"),
                            cfg, dump=dump, hist=True)
-    o = orc.pso_invert(orc.model_from(wl), orc.box_from(wl), orc.swarm_from(wl), seed,
+    o = orc.pso_invert(orc.model_from(wl), orc.box_from(wl),
+                       orc.swarm_from(wl, j_target=j_target, async_chunk=async_chunk), seed,
                        trace, wl["z0"], wl["v0"], n_traces=wl["n_traces"], dump=dump,
                        openmp=True)
     return g, o
@@ -276,3 +278,76 @@ def test_ring_topology_replays_the_oracle(afm, cfg_i, T):
     wl0["swarm"]["topology"] = 0
     g0, _ = _both(afm, wl0, trace)
     assert not np.array_equal(g0["dump"].cpu().numpy()[3], g["dump"].cpu().numpy()[3])
+
+
+@pytest.mark.parametrize("cfg_i,T,per,chunk,topology",
+                         [(2, 1, 45, 16, 0), (4, 3, 40, 7, 0), (2, 1, 45, 1, 0),
+                          (4, 2, 33, 16, 1), (0, 1, 64, 32, 1)])
+def test_async_swarm_replays_the_oracle(afm, cfg_i, T, per, chunk, topology):
+    """async_chunk (R25): the swarm is processed in chunks of `chunk`
+    particles that move as soon as they are evaluated.  Same dump as the oracle's
+    chunked swarm -- ragged last chunk, several traces, one particle per chunk, the
+    ring of three reading neighbours' bests as they stand when the chunk moves -- and
+    a different swarm from the synchronous one."""
+    over = dict(n_cycles=8, n_skip_cycles=4, n_particles=per, n_iters=6)
+    if cfg_i == 4:
+        over["n_traces"] = T
+    wl = wlm.scaled(wlm.config(cfg_i), **over)
+    wl["swarm"]["topology"] = topology
+    truths = None if wl["truth"] is not None else wlm.pixel_truths(wl)
+    trace = oracle_trace(wl, truths=truths)
+    g, o = _both(afm, wl, trace, async_chunk=chunk)
+    _compare_runs(g, o, wl["n_params"])
+    assert g["n_iters_done"] == o["n_iters_done"] == 6
+    gs, _ = _both(afm, wl, trace)
+    if topology == 0:    # (in the ring only the particles at a chunk edge can tell)
+        assert not np.array_equal(gs["dump"].cpu().numpy()[2], g["dump"].cpu().numpy()[2])
+    # a chunk that covers the swarm is the synchronous swarm, bit for bit
+    gw, _ = _both(afm, wl, trace, async_chunk=per)
+    assert np.array_equal(gw["dump"].cpu().numpy(), gs["dump"].cpu().numpy())
+
+
+def test_async_swarm_with_cost_cutoff_and_fp32_kernel(afm):
+    """The cutoff is tested once per batch, after the last chunk (R24 + R25); and the
+    chunked loop runs the FP32 kernel too (checked by replaying the oracle's PSO loop
+    on the GPU's own J, as in test_gpu_forward_f32.py)."""
+    import torch
+    wl = wlm.scaled(wlm.config(0), n_iters=40)
+    trace = oracle_trace(wl)
+    full = orc.pso_invert(orc.model_from(wl), orc.box_from(wl),
+                          orc.swarm_from(wl, async_chunk=24), 0, trace, wl["z0"], wl["v0"],
+                          openmp=True)
+    target, k = _cut_target(full["gbest_hist"][:, 0, 2], 10)
+    g, o = _both(afm, wl, trace, seed=0, j_target=target, async_chunk=24)
+    assert o["n_iters_done"] == k + 1 < 40
+    _compare_cut_runs(g, o, 2)
+    w32 = wlm.scaled(wlm.config(2), n_cycles=12, n_skip_cycles=6, n_particles=50, n_iters=5)
+    tr = oracle_trace(w32)
+    sw = afm.swarm_from(w32, async_chunk=16)
+    g = afm.afm_pso_invert(afm.bounds_from(w32), sw, 4, torch.as_tensor(tr, device="cuda"),
+                           afm.cfg_from(w32, precision=afm.F32), dump=True, hist=True)
+    d = g["dump"].cpu().numpy()
+    calls = {"k": 0}
+    # evaluation order of the chunked swarm: batch, chunk, particle
+    order = [(it, p) for it in range(5) for c0 in range(0, 50, 16)
+             for p in range(c0, min(c0 + 16, 50))]
+
+    def gpu_cost(theta, _U):
+        it, p = order[calls["k"]]
+        calls["k"] += 1
+        return d[it, p, 9]
+
+    o = orc.pso_core(gpu_cost, 3, orc.box_from(w32), orc.swarm_from(w32, async_chunk=16), 4, tr)
+    assert calls["k"] == 250 and np.array_equal(o["dump"], d)
+    assert np.array_equal(o["gbest_hist"], g["gbest_hist"].cpu().numpy())
+
+
+def test_async_is_refused_where_it_has_no_meaning(afm):
+    wl = wlm.scaled(wlm.config(0), n_particles=32, n_iters=2)
+    sw = afm.swarm_from(wl, async_chunk=8)
+    st = afm.afm_pso_init(afm.bounds_from(wl), afm.swarm_from(wl), 2, 1, 0)
+    import torch
+    J = torch.zeros(32, dtype=torch.float64, device="cuda")
+    with pytest.raises(afm.AfmError) as e:
+        afm.afm_pso_step(afm.bounds_from(wl), sw, 2, 1, 0, 0, True, J, st)
+    assert e.value.code == afm.EUNSUPPORTED

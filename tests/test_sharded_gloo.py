@@ -34,6 +34,7 @@ class _Swarm:
         s = wl["swarm"]
         self.n_particles, self.n_iters = s["n_particles"], s["n_iters"]
         self.w, self.c1, self.c2 = s["w"], s["c1"], s["c2"]
+        self.topology = s.get("topology", 0)
 
 
 class OracleDouble:
@@ -58,7 +59,8 @@ class OracleDouble:
         t = lambda a: torch.from_numpy(np.ascontiguousarray(a))
         return dict(x=t(x), v=t(v), pbest=t(x.copy()), pbestJ=t(np.full(PT, np.inf)),
                     gbest=t(x[::swarm.n_particles].copy()), gbestJ=t(np.full(T, np.inf)),
-                    J=t(np.empty(PT)), cand=t(np.empty((T, D + 2))),
+                    J=t(np.empty(PT)),
+                    cand=t(np.empty((T, 3 * D + 4 if swarm.topology == 1 else D + 2))),
                     theta_star=t(np.empty((T, D))), J_star=t(np.empty(T)))
 
     def eval(self, bounds, swarm, trace, cfg, first, st):
@@ -78,32 +80,61 @@ class OracleDouble:
             i = int(np.argmin(seg)) if np.isfinite(seg).any() else 0   # first minimum
             if not np.isfinite(seg).any():
                 cand[s, 0], cand[s, 1] = np.inf, float(2 ** 62)
-                cand[s, 2:] = pb[s * per]
+                cand[s, 2:D + 2] = pb[s * per]
             else:
                 cand[s, 0], cand[s, 1] = seg[i], float(first + s * per + i)
-                cand[s, 2:] = pb[s * per + i]
+                cand[s, 2:D + 2] = pb[s * per + i]
+            if swarm.topology == 1:            # edge particles' personal bests ride along
+                for k, q in enumerate((s * per, s * per + per - 1)):
+                    e = D + 2 + k * (D + 1)
+                    cand[s, e] = pbJ[q]
+                    cand[s, e + 1:e + 1 + D] = pb[q]
         return st["cand"]
 
-    def move(self, bounds, swarm, D, T, seed, it, do_move, first, gathered, st):
-        g = gathered.numpy().reshape(-1, T, D + 2)
+    def move(self, bounds, swarm, D, T, seed, it, do_move, first, gathered, st, rank=0,
+             swarm_particles=None):
+        R = 3 * D + 4 if swarm.topology == 1 else D + 2
+        g = gathered.numpy().reshape(-1, T, R)
         gb, gbJ = st["gbest"].numpy(), st["gbestJ"].numpy()
         for s in range(T):
             order = sorted(range(g.shape[0]), key=lambda r: (g[r, s, 0], g[r, s, 1]))
             r = order[0]
             if g[r, s, 0] < gbJ[s]:
                 gbJ[s] = g[r, s, 0]
-                gb[s] = g[r, s, 2:]
+                gb[s] = g[r, s, 2:D + 2]
             st["theta_star"].numpy()[s] = orc.theta_of_x(self.B, D, gb[s])
             st["J_star"].numpy()[s] = gbJ[s]
         if not do_move:
             return st
         x, v, pb = st["x"].numpy(), st["v"].numpy(), st["pbest"].numpy()
+        pbJ = st["pbestJ"].numpy()
         per = swarm.n_particles
+        total = per if swarm_particles is None else swarm_particles
+        off = first % total
+        n_ranks = g.shape[0]
         for i in range(x.shape[0]):
             r1, r2 = orc.pso_uniforms(seed, first + i, it, 1, D)
             s = i // per
+            social = gb[s]
+            if swarm.topology == 1:
+                # ring of three over in-swarm indices; a neighbour outside this shard
+                # is the last particle of the rank before / the first of the rank after
+                gi = off + (i - s * per)
+
+                def best_of(c):
+                    lc = c - off
+                    if 0 <= lc < per:
+                        return pbJ[s * per + lc], pb[s * per + lc]
+                    if c == (gi - 1) % total:
+                        row = g[(rank - 1) % n_ranks, s, D + 2 + (D + 1):]
+                    else:
+                        row = g[(rank + 1) % n_ranks, s, D + 2:D + 2 + (D + 1)]
+                    return row[0], row[1:1 + D]
+                cands = [(gi - 1) % total, gi, (gi + 1) % total]
+                best = min(cands, key=lambda c: (best_of(c)[0], c))
+                social = best_of(best)[1]
             vn = (swarm.w * v[i] + (swarm.c1 * r1) * (pb[i] - x[i])) + \
-                 (swarm.c2 * r2) * (gb[s] - x[i])
+                 (swarm.c2 * r2) * (social - x[i])
             xn = x[i] + vn
             low, high = xn < self.lo, xn > self.hi
             xn = np.where(low, self.lo, np.where(high, self.hi, xn))
@@ -160,6 +191,34 @@ def test_particle_sharding_world2_replays_the_single_process_oracle():
     for th, Js, *_ in res:                       # identical on both ranks
         assert np.array_equal(th, o["theta_star"])
         assert np.array_equal(Js, o["J_star"])
+
+
+def test_ring_topology_sharded_over_2_ranks_replays_the_oracle():
+    """topology = 1 on a swarm of 23 particles split 12 + 11: the edge particles'
+    personal bests travel in the all-gathered rows (3 D + 4 doubles per rank), the
+    ring wraps from the last rank to the first; and with whole traces per rank."""
+    wl = wlm.scaled(wlm.config(0), n_cycles=6, n_skip_cycles=3, n_particles=23,
+                    n_iters=6)
+    wl["swarm"]["topology"] = 1
+    trace = oracle_trace(wl)
+    o = orc.pso_invert(orc.model_from(wl), orc.box_from(wl), orc.swarm_from(wl),
+                       wl["pso_seed"], trace, wl["z0"], wl["v0"])
+    ref = orc.pso_invert(orc.model_from(wl), orc.box_from(wl),
+                         orc.swarm_from(wl, topology=0), wl["pso_seed"], trace, wl["z0"],
+                         wl["v0"])
+    assert not np.array_equal(o["theta_star"], ref["theta_star"])
+    for th, Js, *_ in _run(2, wl, trace, "particles"):
+        assert np.array_equal(th, o["theta_star"])
+        assert np.array_equal(Js, o["J_star"])
+    w4 = wlm.scaled(wlm.config(4), n_cycles=4, n_skip_cycles=2, n_traces=3,
+                    n_particles=9, n_iters=4, steps_per_cycle=64)
+    w4["swarm"]["topology"] = 1
+    tr4 = oracle_trace(w4, truths=wlm.pixel_truths(w4))
+    o4 = orc.pso_invert(orc.model_from(w4), orc.box_from(w4), orc.swarm_from(w4),
+                        w4["pso_seed"], tr4, w4["z0"], w4["v0"], n_traces=3)
+    for th, Js, *_ in _run(2, w4, tr4, "traces"):
+        assert np.array_equal(th, o4["theta_star"])
+        assert np.array_equal(Js, o4["J_star"])
 
 
 def test_trace_sharding_world2_needs_no_exchange_and_matches():
