@@ -21,6 +21,11 @@ weak; value = all ranks' particle-steps / max-over-ranks time.
 
 --impl reference times the CPU oracle (oracle/, single thread) on a bounded
 sample of the same workload.
+
+--sharded particles|traces (with torchrun for N > 1) runs ONE inversion sharded over
+the ranks with paper_1109_0334_b200.sharded.ShardedSwarm: configs[3] cut by particles
+(one NCCL all-gather of a candidate row per rank and batch) or configs[4] dealt by
+pixels (no collective in the loop); strong scaling; see run_sharded.
 """
 import argparse
 import json
@@ -553,6 +558,146 @@ def extras(afm, torch, dev, main_prec):
     return ex
 
 
+class _PlanBackend:
+    """--plan-only: records what ShardedSwarm asks for, computes nothing."""
+
+    def init(self, bounds, swarm, n_dims, n_traces, seed, first):
+        import torch
+        return {"gbest": torch.zeros((n_traces, n_dims), dtype=torch.float64)}
+
+
+def run_sharded(args):
+    """--sharded particles|traces: ONE inversion sharded over the ranks
+    (paper_1109_0334_b200.sharded.ShardedSwarm: CUDA library + NCCL; DESIGN.md
+    section 9).  particles: configs[3], one swarm of 8 192 particles cut into
+    contiguous slices, one all-gather of a candidate row per rank and batch.  traces:
+    configs[4], 256 pixels dealt to the ranks, no collective in the loop.  Total work
+    is fixed as N grows: strong scaling.  --plan-only prints the partition of every
+    rank and exits (no GPU needed: gloo)."""
+    import torch
+    import torch.distributed as dist
+    from paper_1109_0334_b200.sharded import ShardedSwarm
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    ci = 3 if args.sharded == "particles" else 4
+    wl = wlm.config(ci)
+    if args.sharded_iters:
+        wl = wlm.scaled(wl, n_iters=args.sharded_iters)
+    T, per, D = wl["n_traces"], wl["swarm"]["n_particles"], wl["n_params"]
+
+    if args.plan_only:
+        from paper_1109_0334_b200 import afm as _afm
+        if world > 1:
+            dist.init_process_group("gloo")
+        cfg, sw = _afm.cfg_from(wl), _afm.swarm_from(wl)
+        s = ShardedSwarm(_afm.bounds_from(wl), sw, wl["pso_seed"],
+                         torch.zeros((T, wl["n_window"]), dtype=torch.float64), cfg,
+                         shard=args.sharded, backend=_PlanBackend())
+        mine = {"rank": s.rank, "first_particle": int(s.first),
+                "particles_per_trace": int(s.swarm.n_particles), "n_traces": int(s.n_traces),
+                "collective_per_batch": bool(s.exchange),
+                "row_doubles": _afm.shard_row_doubles(D, sw.topology) if s.exchange else 0}
+        plans = [mine]
+        if world > 1:
+            plans = [None] * world
+            dist.all_gather_object(plans, mine)
+            dist.destroy_process_group()
+        if rank == 0:
+            print(json.dumps({"sharded": args.sharded, "workload": "configs[%d]" % ci,
+                              "n_ranks": world, "plan": plans}))
+        return 0
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --sharded needs CUDA devices: there is no CPU fallback")
+    # NCCL's own communicator log (ranks, devices, transports) goes to stderr
+    os.environ.setdefault("NCCL_DEBUG", "INFO")
+    os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    from paper_1109_0334_b200 import afm
+    afm.lib()
+    prec = afm.F32 if args.precision == "f32" else afm.F64
+    cfg = afm.cfg_from(wl, precision=prec)
+    b, sw = afm.bounds_from(wl), afm.swarm_from(wl)
+    truths = [wl["truth"]] if wl["truth"] is not None else wlm.pixel_truths(wl)
+    c64 = afm.cfg_from(wl)
+    rows = [afm.afm_trajectory(truths[s], c64, wl["z0"], wl["v0"])[0][-wl["n_window"]:]
+            for s in range(T)]
+    h_trace = torch.as_tensor(np.stack(rows) + wlm.trace_noise(wl)).pin_memory()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def one_run(timed):
+        trace = h_trace.to(dev, non_blocking=True)            # H2D inside the run
+        s = ShardedSwarm(b, sw, wl["pso_seed"], trace, cfg, shard=args.sharded,
+                         time_exchange=timed)
+        th, Js = s.run()                                      # D2H of theta*, J* inside
+        return s, th, Js
+
+    one_run(False)                                            # warm-up
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+    afm.afm_reset_launch_count()
+    t0 = time.perf_counter()
+    s, th, Js = one_run(True)
+    barrier()
+    wall_ms = (time.perf_counter() - t0) * 1e3
+    launches = afm.afm_launch_count()
+    clocks = sampler.stop() if sampler else None
+    ex = s.exchange_ms()
+    t = torch.tensor([wall_ms, float(np.mean(ex)) if ex else 0.0], dtype=torch.float64,
+                     device=dev)
+    ids = [(rank, torch.cuda.get_device_properties(local).uuid.__str__())]
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        got = [None] * world
+        dist.all_gather_object(got, ids[0])
+        ids = got
+    wall_ms, ex_ms = [float(v) for v in t.cpu()]
+    if rank == 0:
+        units = float(T) * per * wl["n_steps"] * sw.n_iters
+        value = units / (wall_ms * 1e-3)
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": 1,
+            "warmup": 1, "ms_per_step": wall_ms, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None,
+            "dtype": args.precision, "data": "synthetic",
+            "config": {"workload": "configs[%d] inversion sharded by %s over %d rank(s): "
+                                   "%d trace(s) x %d particles x %d batches x %d RK4 steps"
+                                   % (ci, args.sharded, world, T, per, sw.n_iters,
+                                      wl["n_steps"]),
+                       "step": "one whole inversion (ShardedSwarm.run)",
+                       "collective": ("all_gather of %d doubles per rank and batch (NCCL)"
+                                      % afm.shard_row_doubles(D, sw.topology))
+                                     if s.exchange else "none in the loop"},
+            "inversion_ms": wall_ms,
+            "exchange_ms_per_batch": ex_ms if s.exchange else None,
+            "theta_star_first": [float(x) for x in th[0]], "J_star_first": float(Js[0]),
+            "e2e": {"value": value, "unit": UNIT,
+                    "h2d_bytes_per_step": int(h_trace.numel() * 8),
+                    "d2h_bytes_per_step": int(th.numel() * 8 + Js.numel() * 8),
+                    "api": "ShardedSwarm.run (trace H2D and theta*, J* D2H inside the "
+                           "timed region)"},
+            "gpu_launches": int(launches), "clocks": clocks,
+            "ranks": [{"rank": r, "device_uuid": u} for r, u in ids],
+            "nccl_version": ".".join(str(v) for v in torch.cuda.nccl.version())
+                            if world > 1 else None}))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
 def _one_batch_beam(args, afm, torch, dev):
     """--one-batch 7: the paper's 8-mode Euler-Bernoulli forward model
     (workloads.beam_workload): one forward batch of --beam-particles particles, or
@@ -647,7 +792,16 @@ def main():
     ap.add_argument("--beam-particles", type=int, default=65536)
     ap.add_argument("--invert", action="store_true",
                     help="with --one-batch: time the full PSO inversion instead")
+    ap.add_argument("--sharded", default=None, choices=["particles", "traces"],
+                    help="ONE inversion sharded over the ranks: configs[3] by particles "
+                         "(all-gather per batch) or configs[4] by traces (no collective)")
+    ap.add_argument("--sharded-iters", type=int, default=0,
+                    help="with --sharded: run this many batches instead of the config's")
+    ap.add_argument("--plan-only", action="store_true",
+                    help="with --sharded: print every rank's partition and exit")
     args = ap.parse_args()
+    if args.sharded is not None:
+        return run_sharded(args)
     if args.one_batch is not None:
         return run_one_batch(args)
     if args.warmup < 3 and args.impl == "ours":

@@ -68,8 +68,9 @@ class ShardedSwarm:
     """
 
     def __init__(self, bounds, swarm, seed, trace, cfg, shard="particles",
-                 group=None, backend=None):
+                 group=None, backend=None, time_exchange=False):
         import torch.distributed as dist
+        self.exchange_events = [] if time_exchange else None   # CUDA event pairs
         self.dist = dist
         self.group = group
         on = dist.is_available() and dist.is_initialized()
@@ -133,8 +134,16 @@ class ShardedSwarm:
             # rows of rank r land at [r * n_traces, (r + 1) * n_traces)
             gathered = torch.empty((self.world * cand.shape[0], cand.shape[1]),
                                    dtype=cand.dtype, device=cand.device)
+            timed = self.exchange_events is not None and cand.is_cuda
+            if timed:
+                e0 = torch.cuda.Event(enable_timing=True)
+                e1 = torch.cuda.Event(enable_timing=True)
+                e0.record()
             self.dist.all_gather_into_tensor(gathered, cand.contiguous(),
                                              group=self.group)
+            if timed:
+                e1.record()
+                self.exchange_events.append((e0, e1))
         else:
             gathered = cand.reshape((1,) + tuple(cand.shape))
         self.backend.move(self.bounds, self.swarm, self.D, self.n_traces, self.seed,
@@ -143,6 +152,12 @@ class ShardedSwarm:
                           swarm_particles=self.global_per)
         self.iteration += 1
         return st
+
+    def exchange_ms(self):
+        """Durations of the recorded all-gathers (time_exchange=True), device time."""
+        import torch
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in (self.exchange_events or [])]
 
     def run(self):
         """All swarm.n_iters iterations (the last one without a move, as

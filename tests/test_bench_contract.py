@@ -31,6 +31,58 @@ def test_reference_arm_times_the_oracle_on_cpu():
     assert d["value"] > 1e6          # > 1e6 particle-steps/s on one core
 
 
+def _free_port():
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+@pytest.mark.parametrize("mode", ["particles", "traces"])
+def test_sharded_flag_partitions_as_design_says_world2(mode):
+    """bench.py --sharded ... --plan-only under a 2-rank gloo group (no GPU): the
+    flag parses and the partition is DESIGN.md section 9's: configs[3]'s 8 192
+    particles cut into two contiguous slices with one collective of D + 2 doubles
+    per rank and batch; configs[4]'s 256 pixels dealt 128 + 128 with none."""
+    port = _free_port()
+    procs = []
+    for r in range(2):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE="2",
+                   MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), CUDA_VISIBLE_DEVICES="")
+        procs.append(subprocess.Popen(
+            [sys.executable, os.path.join(ROOT, "bench.py"), "--sharded", mode, "--plan-only",
+             "--gpus", "2"], env=env, cwd=ROOT, stdout=subprocess.PIPE,
+            stderr=subprocess.PIPE, text=True))
+    outs = [p.communicate(timeout=300) for p in procs]
+    assert all(p.returncode == 0 for p in procs), outs
+    assert outs[1][0].strip() == ""                      # only rank 0 prints
+    d = json.loads(outs[0][0].strip())
+    assert d["n_ranks"] == 2 and d["sharded"] == mode
+    a, b = d["plan"]
+    if mode == "particles":
+        assert d["workload"] == "configs[3]"
+        assert (a["first_particle"], a["particles_per_trace"]) == (0, 4096)
+        assert (b["first_particle"], b["particles_per_trace"]) == (4096, 4096)
+        assert a["n_traces"] == b["n_traces"] == 1
+        assert a["collective_per_batch"] and a["row_doubles"] == 4 + 2
+    else:
+        assert d["workload"] == "configs[4]"
+        assert (a["n_traces"], b["n_traces"]) == (128, 128)
+        assert (a["first_particle"], b["first_particle"]) == (0, 128 * 4096)
+        assert a["particles_per_trace"] == b["particles_per_trace"] == 4096
+        assert not a["collective_per_batch"] and a["row_doubles"] == 0
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("mode", ["particles", "traces"])
+def test_sharded_arm_runs_on_one_gpu(mode):
+    """The sharded arm itself (world size 1: no process group), a few batches."""
+    d = _run("--sharded", mode, "--sharded-iters", "3")
+    assert BASE_KEYS <= set(d) and d["scaling"] == "strong" and d["n_gpus"] == 1
+    assert d["inversion_ms"] > 0 and d["gpu_launches"] > 0
+    assert d["config"]["workload"].startswith("configs[%d]" % (3 if mode == "particles" else 4))
+
+
 @pytest.mark.gpu
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 def test_gpu_arm_json_line(prec):
