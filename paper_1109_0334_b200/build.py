@@ -1,6 +1,7 @@
 """Build libafm_b200.so (the C-ABI library of include/afm.h) in-tree.
 
-    python -m paper_1109_0334_b200.build [--force] [--verbose]
+    python -m paper_1109_0334_b200.build [--force] [--verbose] [--ptxas-v]
+                                         [--bounds-check]
 
 nvcc cross-compiles for sm_100a only (no GPU needed to build).  The output
 sits next to this file so that it travels with the source tree; it is
@@ -58,6 +59,8 @@ def build(force=False, verbose=False, extra_flags=()):
 
 if __name__ == "__main__":
     extra = ["-Xptxas", "-v"] if "--ptxas-v" in sys.argv else []
+    if "--bounds-check" in sys.argv:    # checked build for debugging, see AFM_CHECK
+        extra.append("-DAFM_BOUNDS_CHECK")
     print("built", build(force="--force" in sys.argv,
                          verbose="--verbose" in sys.argv or bool(extra),
                          extra_flags=extra))

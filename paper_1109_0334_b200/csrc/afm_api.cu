@@ -1500,7 +1500,7 @@ int afm_set_option(const char* name, int64_t value) {
 }
 
 const char* afm_last_error(void) { return g_err; }
-const char* afm_version(void) { return "afm-b200 0.1 (sm_100a)"; }
+const char* afm_version(void) { return "afm-b200 0.2 (sm_100a)"; }
 
 void afm_shutdown(void) {
   std::lock_guard<std::mutex> lock(g_ws.mu);

@@ -257,6 +257,7 @@ __global__ void beam_integrate_f64(BeamConsts bc, BeamModeConsts mo, IntegrateIO
     mbar_wait(&bars[st], (uint32_t)((tile >> 1) & 1));
     const int n_begin = tile * bc.T;
     const int n_steps = min(bc.T, bc.N - n_begin);
+    AFM_CHECK(n_steps >= 1 && n_steps <= bc.T && n_begin + n_steps <= bc.N);
     double4 r = sp[0];
     for (int i = 0; i < n_steps; ++i) {
       const double4 rn = sp[i + 1];

@@ -195,26 +195,6 @@ struct IsDmt {
   static constexpr bool value = (LAW == AFM_LAW_DMT || LAW == AFM_LAW_DMT_VISC);
 };
 
-// One classical RK4 step (PAPER.md:139; tableau c = (0, 1/2, 1/2, 1),
-// b = (1/6, 1/3, 1/3, 1/6)) of unit length in per-step variables, for the PPT
-// particles of one thread.  With k_jd = stage velocity, k_j = stage acceleration:
-//   k_1d = w, k_2d = w + k1/2, k_3d = w + k2/2, k_4d = w + k3
-//   d' = d + (k_1d + 2 k_2d + 2 k_3d + k_4d)/6 = d + w + (k1 + k2 + k3)/6
-//   w' = w + (k1 + 2 k2 + 2 k3 + k4)/6
-// s0, sh, s1: Dp at t_n, t_n + h/2, t_n + h.
-//
-// DMT laws: the tip is in free flight for most of every cycle, and there the
-// four stages are straight-line code whose reciprocal chains overlap (stage 2's
-// position does not depend on stage 1's force, stage 4's not on stage 3's).
-// `mode` is a warp-uniform state: in mode 0 the step is first taken
-// speculatively on the free-flight side and kept only if every stage position
-// of every particle of the warp really was >= a0 (tested on the high words:
-// conservative by < 2^-20 relative; the exact test lives in the general path);
-// a failed speculation redoes the step in the general form and switches to
-// mode 1, which skips the speculation until a whole step passes without
-// contact.  The general form evaluates both sides of the law in every stage
-// and selects per lane.  A given particle and stage sees the same arithmetic
-// whichever path ran, so the path never changes a result.
 // Monotone integer key of a double (total order equal to the numeric order
 // for non-NaN; +NaN above +Inf, -NaN below -Inf), for the divergence test on
 // the ALU pipe instead of two FP64 compares.
@@ -294,6 +274,26 @@ __device__ __forceinline__ bool free_step(const Particle64& P, double s0, double
          ((unsigned)__double2hiint(dn) < (unsigned)T.safe_hi);
 }
 
+// One classical RK4 step (PAPER.md:139; tableau c = (0, 1/2, 1/2, 1),
+// b = (1/6, 1/3, 1/3, 1/6)) of unit length in per-step variables, for the PPT
+// particles of one thread.  With k_jd = stage velocity, k_j = stage acceleration:
+//   k_1d = w, k_2d = w + k1/2, k_3d = w + k2/2, k_4d = w + k3
+//   d' = d + (k_1d + 2 k_2d + 2 k_3d + k_4d)/6 = d + w + (k1 + k2 + k3)/6
+//   w' = w + (k1 + 2 k2 + 2 k3 + k4)/6
+// s0, sh, s1: Dp at t_n, t_n + h/2, t_n + h.
+//
+// DMT laws: the tip is in free flight for most of every cycle, and there the
+// four stages are straight-line code whose reciprocal chains overlap (stage 2's
+// position does not depend on stage 1's force, stage 4's not on stage 3's).
+// `mode` is a warp-uniform state: in mode 0 the step is first taken
+// speculatively on the free-flight side and kept only if every stage position
+// of every particle of the warp really was >= a0 (tested on the high words:
+// conservative by < 2^-20 relative; the exact test lives in the general path);
+// a failed speculation redoes the step in the general form and switches to
+// mode 1, which skips the speculation until a whole step passes without
+// contact.  The general form evaluates both sides of the law in every stage
+// and selects per lane.  A given particle and stage sees the same arithmetic
+// whichever path ran, so the path never changes a result.
 template <int LAW, int PPT, bool LAT>
 __device__ __forceinline__ void rk4_step(const Particle64 (&P)[PPT], double s0,
                                          double sh, double s1,

@@ -9,6 +9,26 @@
 
 #include "afm_internal.h"
 
+// Bounds checks of our own (compute-sanitizer is not available on the B200 pool):
+// python -m paper_1109_0334_b200.build --force --bounds-check compiles every index
+// computation below into a checked one that prints and traps; the GPU test suite
+// is then run once against that build (profiles/r2_bounds_check.md).
+#ifdef AFM_BOUNDS_CHECK
+#include <stdio.h>
+#define AFM_CHECK(cond)                                                          \
+  do {                                                                           \
+    if (!(cond)) {                                                               \
+      printf("AFM_CHECK failed: %s (%s:%d) block %d thread %d\n", #cond, __FILE__, \
+             __LINE__, (int)blockIdx.x, (int)threadIdx.x);                       \
+      __trap();                                                                  \
+    }                                                                            \
+  } while (0)
+#else
+#define AFM_CHECK(cond) \
+  do {                  \
+  } while (0)
+#endif
+
 namespace afm {
 
 // Each stage of a time-tile ring is followed by pad rows: the kernels fetch the
@@ -44,6 +64,8 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar,
 // dst, src 16-byte aligned, bytes a multiple of 16.
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src,
                                          uint32_t bytes, uint64_t* bar) {
+  AFM_CHECK(bytes > 0 && (bytes & 15u) == 0 && (smem_u32(dst) & 15u) == 0 &&
+            ((uintptr_t)src & 15u) == 0);
   asm volatile(
       "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes "
       "[%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
@@ -80,6 +102,7 @@ __device__ __forceinline__ void st_release_s32(int* p, int v) {
 __device__ __forceinline__ int segq_pop(const SegQueue& q) {
   const unsigned t = atomicAdd(&q.ctrl[0], 1u);
   if (t >= (unsigned)q.n_tasks) return -1;
+  AFM_CHECK(q.n_tasks == q.n_chains * q.n_segs);
   const long long t_start = clock64();
   int v;
   unsigned ns = 250;  // poll with back-off: a waiting worker shares its issue port
@@ -92,6 +115,7 @@ __device__ __forceinline__ int segq_pop(const SegQueue& q) {
     }
   }
   __threadfence();  // acquire: the chain's checkpoint was written before the slot
+  AFM_CHECK((v & 0xfffff) < q.n_chains && (v >> 20) < q.n_segs);
   return v;
 }
 
@@ -100,6 +124,7 @@ __device__ __forceinline__ int segq_pop(const SegQueue& q) {
 // stored the chain's checkpoint, fenced and synchronised its warp.  One lane.
 __device__ __forceinline__ void segq_push(const SegQueue& q, int chain, int seg) {
   const unsigned slot = atomicAdd(&q.ctrl[1], 1u);
+  AFM_CHECK(slot < (unsigned)q.n_tasks && chain < q.n_chains && seg < q.n_segs);
   st_release_s32(&q.slots[slot], (seg << 20) | chain);
 }
 

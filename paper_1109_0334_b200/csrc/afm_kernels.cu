@@ -124,6 +124,7 @@ __device__ __forceinline__ void run_steps(const double4* sp, int i0, int i1,
                                           double (&J)[PPT], bool (&bad)[PPT],
                                           int& mode) {
   if (i0 >= i1) return;
+  AFM_CHECK(i0 >= 0);
   double4 r = sp[i0];
 #pragma unroll 2
   for (int i = i0; i < i1; ++i) {
@@ -173,6 +174,7 @@ __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
     // an inactive slot of a ragged last CTA integrates a copy of the segment's
     // last particle (keeps every vote and barrier uniform) and writes nothing
     gp[q] = (int64_t)s * io.per + (active[q] ? li : io.per - 1);
+    AFM_CHECK(s < io.n_traces && gp[q] >= 0 && gp[q] < io.per * io.n_traces);
   }
 
   const double* stream = io.stream + (int64_t)s * mc.N * 4;
@@ -241,6 +243,7 @@ __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
     mbar_wait(&bars[st], (uint32_t)((tile >> 1) & 1));
     const int n_begin = tile * mc.T;
     const int n_steps = min(mc.T, mc.N - n_begin);
+    AFM_CHECK(n_steps >= 1 && n_steps <= mc.T && n_begin + n_steps <= mc.N);
     // steps [0, k0) of this tile precede the misfit window
     const int k0 = max(0, min(n_steps, mc.n0 - n_begin));
     run_steps<LAW, PPT, LAT, false>(sp, 0, k0, P, a0_bits, T, d, w, J, bad, mode);
@@ -355,6 +358,7 @@ integrate_misfit_f64_q(ModelConsts mc, IntegrateIO io, int blocks_per_tr, SegQue
     const int64_t li = (int64_t)(chain - s * blocks_per_tr) * 32 + tid;
     const bool active = li < io.per;
     const int64_t gp = (int64_t)s * io.per + (active ? li : io.per - 1);
+    AFM_CHECK(s < io.n_traces && gp >= 0 && gp < io.per * io.n_traces);
     const double* stream = io.stream + (int64_t)s * mc.N * 4;
     const int tile_begin = seg * q.tiles_per_seg;
     const int tile_end = min(tile_begin + q.tiles_per_seg, mc.n_tiles);
@@ -419,6 +423,8 @@ integrate_misfit_f64_q(ModelConsts mc, IntegrateIO io, int blocks_per_tr, SegQue
       if (st) ++n_wait1; else ++n_wait0;
       const int n_begin = tile * mc.T;
       const int n_steps = min(mc.T, mc.N - n_begin);
+      AFM_CHECK(n_steps >= 1 && n_steps <= mc.T && n_begin + n_steps <= mc.N);
+      AFM_CHECK(tile >= 0 && tile < mc.n_tiles && tile_end <= mc.n_tiles);
       const int k0 = max(0, min(n_steps, mc.n0 - n_begin));
       run_steps<LAW, 1, false, false>(sp, 0, k0, P, a0_bits, T, d, w, J, bad, mode);
       run_steps<LAW, 1, false, true>(sp, k0, n_steps, P, a0_bits, T, d, w, J, bad, mode);
@@ -561,6 +567,7 @@ __global__ void pso_best_kernel(int D, int64_t per, int64_t off, int64_t cnt,
       (int64_t)(blockIdx.x - s * blocks_per_tr) * blockDim.x + threadIdx.x;
   const bool active = li < cnt;
   const int64_t gp = (int64_t)s * per + off + li;
+  AFM_CHECK(!active || (off + li < per));
   double pb = CUDART_INF;
   long long idx = 0x7fffffffffffffffLL;
   if (active) {
@@ -750,6 +757,7 @@ __global__ void pso_move_kernel(BoxDev box, SwarmDev sw, int D, int64_t per,
   const int64_t s = i / cnt;
   const int64_t p = off + (i - s * cnt);  // local index inside the (local) swarm
   const int64_t gp = s * per + p;
+  AFM_CHECK(p < per && s < n_traces);
   double xi[4], vi[4], pb[4];
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
@@ -786,6 +794,7 @@ __global__ void pso_move_kernel(BoxDev box, SwarmDev sw, int D, int64_t per,
         Jc = pbestJ[s * per + lc];
         return pbest + (s * per + lc) * D;
       }
+      AFM_CHECK(rg.left != nullptr && rg.right != nullptr);
       const double* row = (c == gl ? rg.left : rg.right) + s * rg.stride;
       Jc = row[0];
       return row + 1;

@@ -62,6 +62,7 @@ __device__ __forceinline__ void run_steps32(const float4* sp, int i0, int i1,
                                             bool (&bad)[PPT], int& mode,
                                             float& s_prev) {
   if (i0 >= i1) return;
+  AFM_CHECK(i0 >= 0);
   float4 r = sp[i0];
 #pragma unroll 2
   for (int i = i0; i < i1; ++i) {
@@ -99,6 +100,7 @@ __global__ void integrate_misfit_f32(ModelConstsF32 mf, IntegrateIO io,
     const int64_t li = base + (int64_t)q * blockDim.x;
     active[q] = li < io.per;
     gp[q] = (int64_t)s * io.per + (active[q] ? li : io.per - 1);
+    AFM_CHECK(s < io.n_traces && gp[q] >= 0 && gp[q] < io.per * io.n_traces);
   }
 
   const float4* stream =
@@ -197,6 +199,7 @@ __global__ void integrate_misfit_f32(ModelConstsF32 mf, IntegrateIO io,
     mbar_wait(&bars[st], (uint32_t)((tile >> 1) & 1));
     const int n_begin = tile * mf.T;
     const int n_steps = min(mf.T, mf.N - n_begin);
+    AFM_CHECK(n_steps >= 1 && n_steps <= mf.T && n_begin + n_steps <= mf.N);
     const int k0 = max(0, min(n_steps, mf.n0 - n_begin));
     run_steps32<LAW, PPT, false>(sp, 0, k0, M, P, S, Jt, bad, mode, s_prev);
     run_steps32<LAW, PPT, true>(sp, k0, n_steps, M, P, S, Jt, bad, mode, s_prev);
@@ -382,6 +385,7 @@ integrate_misfit_f32_q(ModelConstsF32 mf, IntegrateIO io, int blocks_per_tr, Seg
       Jh = __ldcg(ck + 128);
       Jl = __ldcg(ck + 160);
       bad[0] = __ldcg(ck + 192) != 0.0f;
+      AFM_CHECK(tile_begin >= 1);
       s_prev = stream[tile_begin * mf.T - 1].y;  // s1 of the step before this segment
     }
     Jt[0] = 0.0f;
@@ -394,6 +398,8 @@ integrate_misfit_f32_q(ModelConstsF32 mf, IntegrateIO io, int blocks_per_tr, Seg
       if (st) ++n_wait1; else ++n_wait0;
       const int n_begin = tile * mf.T;
       const int n_steps = min(mf.T, mf.N - n_begin);
+      AFM_CHECK(n_steps >= 1 && n_steps <= mf.T && n_begin + n_steps <= mf.N);
+      AFM_CHECK(tile >= 0 && tile < mf.n_tiles && tile_end <= mf.n_tiles);
       const int k0 = max(0, min(n_steps, mf.n0 - n_begin));
       run_steps32<LAW, 1, false>(sp, 0, k0, M, P, S, Jt, bad, mode, s_prev);
       run_steps32<LAW, 1, true>(sp, k0, n_steps, M, P, S, Jt, bad, mode, s_prev);

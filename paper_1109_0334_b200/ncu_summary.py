@@ -129,6 +129,7 @@ def main():
     ap.add_argument("--kernel-index", type=int, default=0)
     ap.add_argument("--command", default="")
     ap.add_argument("--title", default="")
+    ap.add_argument("--no-sass", action="store_true", help="skip NAME_hot_sass.txt")
     a = ap.parse_args()
     kname, vals = read_raw(a.report, a.kernel_index)
     total, ops, hot = hot_sass(a.report)
@@ -153,8 +154,12 @@ def main():
     md += ["", "Executed warp-instructions by opcode (%d in total):" % total, "",
            "| opcode | warp-instructions | share |", "|---|---|---|"]
     md += ["| %s | %d | %.3f |" % (k, v, v / total) for k, v in ops[:16]]
-    md += ["", "Hot-loop SASS: `%s_hot_sass.txt`." % a.name, ""]
+    md += ["", "Hot-loop SASS: `%s_hot_sass.txt`." % a.name, ""] if not a.no_sass else [""]
     open(base + "_ncu.md", "w").write("\n".join(md))
+    if a.no_sass:
+        print("wrote %s_ncu.csv, _ncu.md (kernel %s, %.3f ms)"
+              % (base, kname.split("(")[0], to_ms(*vals["gpu__time_duration.sum"])))
+        return 0
     with open(base + "_hot_sass.txt", "w") as f:
         f.write("# %s: SASS rows with >= 5%% of the maximum execution count "
                 "(ncu --page source)\n# columns: row, warp-level executions, stall samples, "
