@@ -59,6 +59,8 @@ int g_opt_pack = 0;   // 0 = auto, 1 = never, 2 = always (DMT laws only)
 int g_opt_queue = 0;  // 0 = auto, 1 = never, 2 = always: segment-queue scheduling
 int g_opt_segs = 0;   // 0 = auto (~450 steps each): time segments per chain of the queue kernel
 int g_opt_workers = 0;  // 0 = auto: queue workers per SM sub-partition
+int g_opt_boost = 0;    // 0 = auto (2), 1 = off, k >= 2: parking beside the chains that are behind
+                        // more than 1/k of the chains by a whole segment
 int g_n_sm = 148;
 
 // afm_set_option("kernel_events", 1): every launch of an integrate kernel is
@@ -387,44 +389,67 @@ int integrate_bpt(int64_t per, int block, int ppt, int variant, int lanes) {
   return variant == 1 ? blocks_per_trace(per, lanes) : blocks_per_trace(per, block * ppt);
 }
 
-// Segment-queue scheduling (integrate_misfit_f64_q / _f32_q) serves a batch of a
-// few warps of particles ("chains") per SM sub-partition: floor(r) + 1 persistent
-// one-warp workers per sub-partition for r chains per sub-partition, so that the
-// spare worker slots rotate over the whole device.  *use is false when the plain
-// kernel should run.  Lock held.
+// Segment-queue scheduling (integrate_misfit_f64_q / _f32_q): the time loop of every
+// warp of particles (a "chain") is cut into segments that persistent one-warp
+// workers take from a priority queue keyed by the segment index.  Fewer workers
+// than chains -- chains per sub-partition / 1.15, rounded down, between 2 and 5
+// per sub-partition -- so that the chains that are ahead wait while the ones that
+// are behind run, and all finish together.  Measured (configs[1]-like batches of
+// r chains per sub-partition, best workers per sub-partition): r = 2.5: 2,
+// r = 3.5 and 4: 3, r = 5.5: 4, r = 8 and 12: 5 (6 to 8 are slower), configs[4]
+// (r = 55): 5 or 6.  *use is false when the plain kernel should run.  Lock held.
 int make_queue(int64_t per, int n_traces, int n_tiles, int T, bool eligible,
                SegQueue* q, int* workers, bool* use, cudaStream_t st) {
   const int64_t chains = (int64_t)blocks_per_trace(per, 32) * n_traces;
   const int64_t subparts = (int64_t)4 * g_n_sm;
   *use = eligible && g_opt_queue != 1 && chains < (1 << 20);
-  if (*use && g_opt_queue == 0)
-    *use = (2 * chains >= 3 * subparts && chains <= 6 * subparts && n_tiles >= 64);
+  if (*use && g_opt_queue == 0) *use = (2 * chains >= 3 * subparts && n_tiles >= 32);
   if (!*use) return AFM_OK;
-  int per_sub = g_opt_workers > 0 ? g_opt_workers : (int)(chains / subparts) + 1;
+  int per_sub = g_opt_workers > 0 ? g_opt_workers : (int)((chains * 100) / (subparts * 115));
+  if (g_opt_workers == 0 && per_sub < 2) per_sub = 2;
+  if (g_opt_workers == 0 && per_sub > 5) per_sub = 5;
   if (per_sub > 8) per_sub = 8;
   *workers = (int)(per_sub * subparts);
   if (*workers > chains) *workers = (int)chains;
-  // segments of about 450 steps (130 us at 3-4 FP64 warps per sub-partition: long
-  // against the 2-3 us a hand-over costs, short against the whole solve;
-  // measured on configs[1]: 8 segments 16.4 ms, 32: 15.7, 115: 14.9, 400: 15.3)
-  int segs = g_opt_segs > 0 ? g_opt_segs : (n_tiles * T + 447) / 448;
+  // segments of about 1 000 steps (250 us at 3 FP64 warps per sub-partition: long
+  // against the 2-3 us a hand-over costs, short against the whole solve; measured
+  // on configs[1], 51 200 steps: 29 to 58 segments 12.86 ms, 80: 12.91, 115: 13.06)
+  int segs = g_opt_segs > 0 ? g_opt_segs : (n_tiles * T + 1023) / 1024;
   if (segs > n_tiles) segs = n_tiles;
   if (segs > 2047) segs = 2047;
   if (segs < 1) segs = 1;
   q->tiles_per_seg = (n_tiles + segs - 1) / segs;
   q->n_segs = (n_tiles + q->tiles_per_seg - 1) / q->tiles_per_seg;
   q->n_chains = (int32_t)chains;
-  q->n_tasks = q->n_chains * q->n_segs;
+  const int64_t tasks = chains * q->n_segs;
+  if (tasks >= ((int64_t)1 << 30)) {
+    if (g_opt_queue == 2)
+      return fail(AFM_EINVAL, "segment queue: %lld chains x %d segments are too many",
+                  (long long)chains, (int)q->n_segs);
+    *use = false;
+    return AFM_OK;
+  }
+  q->n_tasks = (int32_t)tasks;
   q->timeout_cycles = 40000000000LL;  // ~20 s: only a corrupted queue gets there
   const size_t slot_bytes = ((size_t)q->n_tasks * 4 + 255) & ~(size_t)255;
-  const size_t need = 256 + slot_bytes + (size_t)chains * 128 * 8;
+  const size_t lvl_bytes = 3 * 2048 * 4;  // head[], tail[]: segs <= 2047; park[]
+  const size_t need = 256 + lvl_bytes + slot_bytes + (size_t)chains * 128 * 8;
+  if (need > ((size_t)2 << 30) && g_opt_queue == 0) {  // too many chains x segments
+    *use = false;
+    return AFM_OK;
+  }
   const bool fresh = need > g_ws.segq.cap;
   if (g_ws.segq.ensure(need))
     return fail(AFM_ECUDA, "cudaMalloc of the segment queue failed");
   if (fresh) CUDA_TRY(cudaMemsetAsync(g_ws.segq.p, 0, 256, st));
   q->ctrl = (unsigned*)g_ws.segq.p;
-  q->slots = (int*)((char*)g_ws.segq.p + 256);
-  q->ckpt = (double*)((char*)g_ws.segq.p + 256 + slot_bytes);
+  q->head = (unsigned*)((char*)g_ws.segq.p + 256);
+  q->tail = q->head + 2048;
+  q->park = q->tail + 2048;
+  q->n_park = (g_opt_boost != 1 && subparts <= 2048) ? (int32_t)subparts : 0;
+  q->boost_div = g_opt_boost >= 2 ? g_opt_boost : 2;
+  q->slots = (int*)((char*)g_ws.segq.p + 256 + lvl_bytes);
+  q->ckpt = (double*)((char*)g_ws.segq.p + 256 + lvl_bytes + slot_bytes);
   return AFM_OK;
 }
 
@@ -1483,6 +1508,11 @@ int afm_set_option(const char* name, int64_t value) {
   if (!strcmp(name, "workers")) {
     if (value < 0 || value > 8) return fail(AFM_EINVAL, "workers must be in 0..8");
     g_opt_workers = (int)value;
+    return AFM_OK;
+  }
+  if (!strcmp(name, "boost")) {
+    if (value < 0 || value > 64) return fail(AFM_EINVAL, "boost must be in 0..64");
+    g_opt_boost = (int)value;
     return AFM_OK;
   }
   if (!strcmp(name, "segs")) {

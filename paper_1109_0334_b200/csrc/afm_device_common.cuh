@@ -87,26 +87,69 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 }
 
 // ---- segment queue of the *_q integrate kernels (see afm_kernels.cu) ----------
+// A priority queue keyed by the segment index ("level"): level l holds one slot
+// per chain, filled in the order the chains finish segment l - 1 and consumed in
+// that order; a worker always takes the oldest published task of the LOWEST level
+// that has one, so a chain that has fallen behind (more general-form steps, a
+// higher cost per segment) is picked up the moment it is published while the
+// chains that are ahead wait.  With fewer workers than chains the chains thus
+// advance within about one segment of one another and finish together.
 __device__ __forceinline__ int ld_relaxed_s32(const int* p) {
   int v;
   asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ unsigned ld_relaxed_u32(const unsigned* p) {
+  unsigned v;
+  asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
 __device__ __forceinline__ void st_release_s32(int* p, int v) {
   asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-// Next task of this worker: -1 when every task has been handed out, -2 after a
-// time-out (cannot happen unless the queue is corrupted; keeps a bug from
-// hanging the device).  Called by one lane.
-__device__ __forceinline__ int segq_pop(const SegQueue& q) {
-  const unsigned t = atomicAdd(&q.ctrl[0], 1u);
-  if (t >= (unsigned)q.n_tasks) return -1;
+// Next task of this worker, (segment << 20) | chain: -1 when every task has been
+// handed out, -2 after a time-out (cannot happen unless the queue is corrupted;
+// keeps a bug from hanging the device).  Called by one lane.
+__device__ __forceinline__ int segq_take(const SegQueue& q) {
   AFM_CHECK(q.n_tasks == q.n_chains * q.n_segs);
-  const long long t_start = clock64();
-  int v;
+  const unsigned nc = (unsigned)q.n_chains;
+  long long t_start = 0;
   unsigned ns = 250;  // poll with back-off: a waiting worker shares its issue port
-  while ((v = ld_relaxed_s32(&q.slots[t])) < 0) {
+  for (;;) {
+    int l = (int)ld_relaxed_u32(&q.ctrl[0]);  // lowest level not yet handed out in full
+    if (l >= q.n_segs) return -1;
+    bool lowest = true;
+    for (; l < q.n_segs; ++l) {
+      const unsigned h = ld_relaxed_u32(&q.head[l]);
+      if (h >= nc) {  // level handed out in full
+        if (lowest) atomicMax(&q.ctrl[0], (unsigned)(l + 1));
+        continue;
+      }
+      lowest = false;
+      const unsigned t = ld_relaxed_u32(&q.tail[l]);
+      if (t == 0u) break;    // nothing was ever published here, so nothing above either
+      if (h >= t) continue;  // nothing ready at this level right now
+      const unsigned ticket = atomicAdd(&q.head[l], 1u);
+      if (ticket >= nc) continue;  // lost the race for the level's last tasks
+      // the ticket's slot is published already unless other workers raced for the
+      // same tasks; then it is the next chain to finish segment l - 1
+      const int* slot = &q.slots[(size_t)l * nc + ticket];
+      int v;
+      while ((v = ld_relaxed_s32(slot)) < 0) {
+        if (t_start == 0) t_start = clock64();
+        __nanosleep(ns);
+        if (ns < 4000) ns *= 2;
+        if (clock64() - t_start > q.timeout_cycles) {
+          atomicExch(&q.ctrl[2], 1u);
+          return -2;
+        }
+      }
+      __threadfence();  // acquire: the chain's checkpoint was written before the slot
+      AFM_CHECK(v < q.n_chains);
+      return (l << 20) | v;
+    }
+    if (t_start == 0) t_start = clock64();
     __nanosleep(ns);
     if (ns < 4000) ns *= 2;
     if (clock64() - t_start > q.timeout_cycles) {
@@ -114,18 +157,63 @@ __device__ __forceinline__ int segq_pop(const SegQueue& q) {
       return -2;
     }
   }
-  __threadfence();  // acquire: the chain's checkpoint was written before the slot
-  AFM_CHECK((v & 0xfffff) < q.n_chains && (v >> 20) < q.n_segs);
-  return v;
 }
 
+// SM sub-partition of the calling warp: warp slots w, w + 4, w + 8, ... of an SM share
+// a scheduler and its FP64 pipe (measured: two DFMA-bound warps slow each other down
+// exactly when their %warpid agree modulo 4).
+__device__ __forceinline__ unsigned smsp_id() {
+  unsigned smid, wid;
+  asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+  asm volatile("mov.u32 %0, %%warpid;" : "=r"(wid));
+  return smid * 4u + (wid & 3u);
+}
 
-// Publish segment `seg` of `chain` at the tail of the queue.  The caller has
-// stored the chain's checkpoint, fenced and synchronised its warp.  One lane.
+// segq_take plus the boost of the chains on the critical path.  Chains advance
+// within about a segment of one another, except the few whose cost per step is
+// far above the rest (a warp with a particle stuck to the sample runs every step
+// in the general form): always picked up at once, always running, they still
+// fall behind and set the time of the batch.  A worker that takes a task of a
+// level most chains have already finished marks its sub-partition: one of the
+// other workers there, when it next comes for a task, parks until the marked
+// segment is over, and the chain that is behind runs with one warp fewer beside
+// it (a third faster at three warps per sub-partition).  q.park[smsp]: 0 = free,
+// 1 = a parking place is offered, 2 = taken.  Called by one lane.
+struct SegqWorker {
+  unsigned offered;  // this worker's offer of a parking place is standing
+};
+__device__ __forceinline__ int segq_pop(const SegQueue& q, SegqWorker* wk) {
+  unsigned& offered = wk->offered;
+  const unsigned sp = smsp_id();
+  if (sp >= (unsigned)q.n_park) return segq_take(q);
+  unsigned* pk = &q.park[sp];
+  if (offered == 1u) {
+    offered = 0u;
+    atomicExch(pk, 0u);  // the marked segment is over: release the parked worker
+  } else if (ld_relaxed_u32(pk) == 1u && atomicCAS(pk, 1u, 2u) == 1u) {
+    unsigned waited = 0;
+    while (ld_relaxed_u32(pk) == 2u && (int)ld_relaxed_u32(&q.ctrl[0]) < q.n_segs &&
+           ++waited < 200000u)
+      __nanosleep(2000);
+  }
+  const int task = segq_take(q);
+  if (task >= 0) {
+    const int l = task >> 20;
+    if (l + 1 < q.n_segs &&
+        (unsigned)q.boost_div * ld_relaxed_u32(&q.tail[l + 1]) > (unsigned)q.n_chains &&
+        atomicCAS(pk, 0u, 1u) == 0u)
+      offered = 1u;
+  }
+  return task;
+}
+
+// Publish segment `seg` of `chain` at its level.  The caller has stored the
+// chain's checkpoint, fenced and synchronised its warp.  One lane.
 __device__ __forceinline__ void segq_push(const SegQueue& q, int chain, int seg) {
-  const unsigned slot = atomicAdd(&q.ctrl[1], 1u);
-  AFM_CHECK(slot < (unsigned)q.n_tasks && chain < q.n_chains && seg < q.n_segs);
-  st_release_s32(&q.slots[slot], (seg << 20) | chain);
+  AFM_CHECK(chain < q.n_chains && seg >= 1 && seg < q.n_segs);
+  const unsigned slot = atomicAdd(&q.tail[seg], 1u);
+  AFM_CHECK(slot < (unsigned)q.n_chains);
+  st_release_s32(&q.slots[(size_t)seg * q.n_chains + slot], chain);
 }
 
 __device__ __forceinline__ bool cand_less(double Ja, long long ia, double Jb,

@@ -127,8 +127,14 @@ struct IntegrateIO {
 // Segment queue of integrate_misfit_f64_q (afm_kernels.cu): tasks are
 // (chain, segment) = (warp of 32 particles, run of tiles_per_seg time tiles).
 struct SegQueue {
-  int* slots;            // [n_tasks]  (segment << 20) | chain, or -1 = not yet published
-  unsigned* ctrl;        // [0] consume ticket, [1] publish index, [2] time-out flag
+  int* slots;            // [n_segs][n_chains]  chain, or -1 = not yet published
+  unsigned* ctrl;        // [0] lowest level not handed out in full, [2] time-out flag
+  unsigned* head;        // [n_segs] tasks handed out per level
+  unsigned* tail;        // [n_segs] tasks published (slots reserved) per level
+  unsigned* park;        // [n_park] parking place per SM sub-partition (segq_pop)
+  int32_t n_park;        // 4 * SMs, or 0: no boost of the chains that are behind
+  int32_t boost_div;     // a task is behind when more than n_chains / boost_div chains
+                         // have finished its level
   double* ckpt;          // [n_chains][4][32] doubles: d, w, J, diverged flag of a chain at
                          // rest (FP32 kernel: [n_chains][8][32] floats, same size)
   long long timeout_cycles;

@@ -315,11 +315,13 @@ __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
 // ============================================================================
 __global__ void segq_init_kernel(SegQueue q) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < q.n_tasks) q.slots[i] = (i < q.n_chains) ? i : -1;  // segment 0 of chain i
-  if (i == 0) {
-    q.ctrl[0] = 0u;                    // head: next consume ticket
-    q.ctrl[1] = (unsigned)q.n_chains;  // tail: next publish slot
+  if (i < q.n_tasks) q.slots[i] = (i < q.n_chains) ? i : -1;  // level 0: every chain
+  if (i < q.n_segs) {
+    q.head[i] = 0u;
+    q.tail[i] = (i == 0) ? (unsigned)q.n_chains : 0u;
   }
+  if (i < q.n_park) q.park[i] = 0u;
+  if (i == 0) q.ctrl[0] = 0u;
 }
 
 template <int LAW, int MODE>
@@ -330,9 +332,11 @@ integrate_misfit_f64_q(ModelConsts mc, IntegrateIO io, int blocks_per_tr, SegQue
   double4* tile1 = tile0 + (mc.T + kPadRows);
   uint64_t* bars = reinterpret_cast<uint64_t*>(tile1 + (mc.T + kPadRows));
   __shared__ Cand red[32];
+  __shared__ SegqWorker qworker;  // lane 0's queue state (one warp per CTA)
 
   const int tid = threadIdx.x;
   if (tid == 0) {
+    qworker.offered = 0u;
     tile0[mc.T] = make_double4(0.0, 0.0, 0.0, 0.0);
     tile1[mc.T] = make_double4(0.0, 0.0, 0.0, 0.0);
     mbar_init(&bars[0], 1);
@@ -349,7 +353,7 @@ integrate_misfit_f64_q(ModelConsts mc, IntegrateIO io, int blocks_per_tr, SegQue
 
   for (;;) {
     int task = 0;
-    if (tid == 0) task = segq_pop(q);
+    if (tid == 0) task = segq_pop(q, &qworker);
     task = __shfl_sync(0xffffffffu, task, 0);
     if (task < 0) break;
     const int chain = task & 0xfffff;
@@ -898,7 +902,8 @@ int launch_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block
 }
 
 int launch_segq_init(const SegQueue& q, cudaStream_t st) {
-  segq_init_kernel<<<(unsigned)((q.n_tasks + 255) / 256), 256, 0, st>>>(q);
+  const int n_init = q.n_tasks > q.n_park ? q.n_tasks : q.n_park;
+  segq_init_kernel<<<(unsigned)((n_init + 255) / 256), 256, 0, st>>>(q);
   return 1;
 }
 

@@ -270,9 +270,11 @@ integrate_misfit_f32_q(ModelConstsF32 mf, IntegrateIO io, int blocks_per_tr, Seg
   float4* tile1 = tile0 + (mf.T + kPadRows);  // one pad row per stage for the row fetched ahead
   uint64_t* bars = reinterpret_cast<uint64_t*>(tile1 + (mf.T + kPadRows));
   __shared__ Cand red[32];
+  __shared__ SegqWorker qworker;  // lane 0's queue state (one warp per CTA)
 
   const int tid = threadIdx.x;
   if (tid == 0) {
+    qworker.offered = 0u;
     tile0[mf.T] = make_float4(0.f, 0.f, 0.f, 0.f);
     tile1[mf.T] = make_float4(0.f, 0.f, 0.f, 0.f);
     mbar_init(&bars[0], 1);
@@ -297,7 +299,7 @@ integrate_misfit_f32_q(ModelConstsF32 mf, IntegrateIO io, int blocks_per_tr, Seg
 
   for (;;) {
     int task = 0;
-    if (tid == 0) task = segq_pop(q);
+    if (tid == 0) task = segq_pop(q, &qworker);
     task = __shfl_sync(0xffffffffu, task, 0);
     if (task < 0) break;
     const int chain = task & 0xfffff;
