@@ -220,15 +220,18 @@ __device__ __forceinline__ bool diverged_step(double d, const DivergeTest& T) {
   return false;
 }
 
-// Stage-3 position and the RK4 combination.  Throughput form: the textbook
-// association with the fewest operations.  Latency form: the same sums associated
-// so that the loop-carried chain d_n -> k1 -> d3 -> k3 -> d_{n+1} is as short as it
-// can be: d3 = d2 + k1/4 (= d + w2/2 without waiting for w2) and
+// Stage-3 position and the RK4 combination.  d3 = d2 + k1/4 (= d + w2/2 without
+// waiting for w2: one dependent operation fewer, same instruction count) in both
+// forms (configs[1]: 12.89 -> 12.68 ms in the throughput form).  The combination in
+// the throughput form is the textbook association with the fewest operations; in
+// the latency form the same sums are associated so that the loop-carried chain
+// d_n -> k1 -> d3 -> k3 -> d_{n+1} is as short as it can be:
 // d_{n+1} = [d + w + (k1 + k2)/6] + k3/6 (one FMA after k3); two more additions,
-// three fewer dependent operations per step (8.1 cycles each).
-template <bool LAT>
-__device__ __forceinline__ double stage3_gap(double d, double d2, double k1, double w2) {
-  return LAT ? fma(0.25, k1, d2) : fma(0.5, w2, d);
+// two fewer dependent operations per step (8.1 cycles each).  (In the
+// throughput form that association, the folded van der Waals term and the folded
+// -alpha w each cost more than they save: 12.99, 13.69 and 13.27 ms.)
+__device__ __forceinline__ double stage3_gap(double d2, double k1) {
+  return fma(0.25, k1, d2);
 }
 template <bool LAT>
 __device__ __forceinline__ void rk4_combine(double dw, double w, double k1, double k2,
@@ -262,7 +265,7 @@ __device__ __forceinline__ bool free_step(const Particle64& P, double s0, double
   const double w2 = fma(0.5, k1, w);
   const double k2 = accel_free<LAT, false>(P, sh, d2, w2);
   const double w3 = fma(0.5, k2, w);
-  const double d3 = stage3_gap<LAT>(d, d2, k1, w2);
+  const double d3 = stage3_gap(d2, k1);
   const double k3 = accel_free<LAT, true>(P, sh, d3, w3);
   const double d4 = d + w3;
   const double k4 = accel_free<LAT, false>(P, s1, d4, w + k3);
@@ -315,7 +318,7 @@ __device__ __forceinline__ void rk4_step(const Particle64 (&P)[PPT], double s0,
       const double k2 = accel_smooth<LAW>(P[q], sh, d2[q], w2);
       const double w3 = fma(0.5, k2, w[q]);
       const double k3 =
-          accel_smooth<LAW>(P[q], sh, stage3_gap<LAT>(d[q], d2[q], k1, w2), w3);
+          accel_smooth<LAW>(P[q], sh, stage3_gap(d2[q], k1), w3);
       const double k4 = accel_smooth<LAW>(P[q], s1, d[q] + w3, w[q] + k3);
       rk4_combine<LAT>(dw[q], w[q], k1, k2, k3, k4, d[q], w[q]);
       bad[q] |= diverged_step(d[q], T);
@@ -350,7 +353,7 @@ __device__ __forceinline__ void rk4_step(const Particle64 (&P)[PPT], double s0,
     const double w2 = fma(0.5, k1, w[q]);
     const double k2 = accel_both<LAW, LAT, false>(P[q], sh, d2[q], w2, a0_bits);
     const double w3 = fma(0.5, k2, w[q]);
-    const double d3 = stage3_gap<LAT>(d[q], d2[q], k1, w2);
+    const double d3 = stage3_gap(d2[q], k1);
     const double k3 = accel_both<LAW, LAT, true>(P[q], sh, d3, w3, a0_bits);
     const double d4 = d[q] + w3;
     const double k4 = accel_both<LAW, LAT, false>(P[q], s1, d4, w[q] + k3, a0_bits);

@@ -154,6 +154,13 @@ def main():
     md += ["", "Executed warp-instructions by opcode (%d in total):" % total, "",
            "| opcode | warp-instructions | share |", "|---|---|---|"]
     md += ["| %s | %d | %.3f |" % (k, v, v / total) for k, v in ops[:16]]
+    if "_q<" in kname:
+        md += ["", "(The opcode counts come from ncu's instrumented pass.  A queue worker that "
+               "waits sleeps for a time in nanoseconds between two polls, and that pass runs "
+               "many times slower than a timed launch: its polling instructions -- "
+               "LDG.E.STRONG.GPU, NANOSLEEP, YIELD, CS2R and the BRA / ISETP around them -- "
+               "are over-counted here by that factor.  `smsp__inst_executed.sum` above is "
+               "from a hardware-counter pass.)"]
     md += ["", "Hot-loop SASS: `%s_hot_sass.txt`." % a.name, ""] if not a.no_sass else [""]
     open(base + "_ncu.md", "w").write("\n".join(md))
     if a.no_sass:
