@@ -88,6 +88,12 @@ def _ncu_profile(precision):
     out["pipe_active_pct"] = float(kv[PIPE_METRIC[precision] + "active"])
     out["pipe_elapsed_pct"] = float(kv[PIPE_METRIC[precision] + "elapsed"])
     out["kernel_ms_under_ncu"] = float(kv["duration_ms"])
+    key = "fp32" if precision == "f32" else "fp64"
+    if ("executed_%s_fma" % key) in kv:
+        # warp-instructions x 32 lanes; FMA = 2 flops (SURVEY.md 8(d) definition (2))
+        out["executed_flops_per_launch"] = 32.0 * (
+            2.0 * float(kv["executed_%s_fma" % key]) + float(kv["executed_%s_add" % key])
+            + float(kv["executed_%s_mul" % key]))
     return out
 
 
@@ -380,6 +386,12 @@ def run_ours(args):
                                               else ncu["pipe_active_pct"] / 100.0),
                          "frac_pipe_elapsed": (None if ncu["pipe_elapsed_pct"] is None
                                                else ncu["pipe_elapsed_pct"] / 100.0),
+                         "executed_tflops": (
+                             None if not ncu.get("executed_flops_per_launch") else
+                             ncu["executed_flops_per_launch"] / (kern_ms * 1e-3) / 1e12),
+                         "frac_executed": (
+                             None if not ncu.get("executed_flops_per_launch") else
+                             ncu["executed_flops_per_launch"] / (kern_ms * 1e-3) / 1e12 / peak),
                          "ncu": ncu,
                          "peak_source": "lane model 148 SM x %d lanes x 2 x %s (%s)" % (
                              FP32_LANES if prec == afm.F32 else FP64_LANES,

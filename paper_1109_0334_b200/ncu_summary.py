@@ -140,6 +140,15 @@ def main():
             ("dram_bytes_read", "%d" % to_bytes(*vals["dram__bytes_read.sum"])),
             ("dram_bytes_write", "%d" % to_bytes(*vals["dram__bytes_write.sum"]))]
     rows += [(m, _num(v[1])) for m, v in vals.items()]
+    # executed floating-point warp-instructions of the launch (source page): what
+    # bench.py turns into executed FLOP/s, SURVEY.md 8(d) definition (2)
+    opd = dict(ops)
+    for prefix, key in (("D", "fp64"), ("F", "fp32")):
+        fma = sum(v for k, v in opd.items() if k.split(".")[0] == prefix + "FMA")
+        add = sum(v for k, v in opd.items() if k.split(".")[0] == prefix + "ADD")
+        mul = sum(v for k, v in opd.items() if k.split(".")[0] == prefix + "MUL")
+        rows += [("executed_%s_fma" % key, fma), ("executed_%s_add" % key, add),
+                 ("executed_%s_mul" % key, mul)]
     with open(base + "_ncu.csv", "w", newline="") as f:
         w = csv.writer(f)
         w.writerow(("key", "value"))

@@ -293,15 +293,19 @@ def test_warp_packing_changes_no_result(afm, precision):
 
 
 @pytest.mark.parametrize("precision", [0, 1])
-@pytest.mark.parametrize("cfg_i,segs,workers", [(1, 0, 0), (1, 5, 1), (2, 3, 8), (3, 7, 2),
-                                                (4, 1, 4), (4, 2047, 3)])
-def test_segment_queue_changes_no_result(afm, cfg_i, segs, workers, precision):
+@pytest.mark.parametrize("cfg_i,segs,workers,boost", [
+    (1, 0, 0, 0), (1, 5, 1, 0), (2, 3, 8, 0), (3, 7, 2, 0), (4, 1, 4, 0), (4, 2047, 3, 0),
+    (1, 24, 1, 64), (1, 48, 2, 1), (1, 16, 1, 2)])
+def test_segment_queue_changes_no_result(afm, cfg_i, segs, workers, boost, precision):
     """afm_set_option("queue"): the time loop of every warp of particles is cut into
-    segments handed between persistent workers through a ticket queue in global
-    memory (integrate_misfit_f64_q, integrate_misfit_f32_q).  Misfits, and the swarm of an inversion, must be
-    bit-identical to the one-CTA-per-warp kernel: ragged particle counts, several
-    traces, every segment count from one to one tile per segment, fewer workers than
-    chains, all law families; and they must match the oracle."""
+    segments that persistent workers take from a priority queue in global memory
+    keyed by the segment index (integrate_misfit_f64_q, integrate_misfit_f32_q).
+    Misfits, and the swarm of an inversion, must be bit-identical to the
+    one-CTA-per-warp kernel: ragged particle counts, several traces, every segment
+    count from one to one tile per segment, fewer workers than chains (chains wait,
+    the lowest segment first), the boost of the chains that are behind on, off and
+    at its most eager (a worker pauses whenever 1/64 of the chains are a segment
+    ahead), all law families; and they must match the oracle."""
     import torch
     over = dict(n_cycles=12, n_skip_cycles=6)
     if cfg_i == 4:
@@ -310,8 +314,9 @@ def test_segment_queue_changes_no_result(afm, cfg_i, segs, workers, precision):
     T = wl["n_traces"]
     truths = None if wl["truth"] is not None else wlm.pixel_truths(wl)
     trace = oracle_trace(wl, truths=truths)
-    # (1, 5, 1): 626 chains on 592 workers, so chains also wait for a free worker
-    n = 20013 if (cfg_i, workers) == (1, 1) else T * (300 + 13)
+    # (1, 5, 1): 626 chains on 592 workers, so chains also wait for a free worker;
+    # the boost cases: 1 251 chains on 592 or 1 184 workers
+    n = 40013 if boost else 20013 if (cfg_i, workers) == (1, 1) else T * (300 + 13)
     params = wlm.draw_params(wl, n, seed=61)
     z0v0 = wlm.draw_initial_states(wl, n, seed=62) if cfg_i == 1 else None
     wp = wlm.scaled(wl, n_particles=77, n_iters=4)
@@ -320,6 +325,7 @@ def test_segment_queue_changes_no_result(afm, cfg_i, segs, workers, precision):
         afm.afm_set_option("queue", queue)
         afm.afm_set_option("segs", segs)
         afm.afm_set_option("workers", workers)
+        afm.afm_set_option("boost", boost)
         afm.afm_set_option("form", 1)           # the queue serves the throughput form
         try:
             out[queue] = _gpu_forward(afm, wl, params, trace, z0v0, precision=precision)
@@ -328,13 +334,14 @@ def test_segment_queue_changes_no_result(afm, cfg_i, segs, workers, precision):
                                    afm.cfg_from(wp, precision=precision), dump=True)
             out[queue, "pso"] = g["dump"].cpu().numpy()
         finally:
-            for name in ("queue", "segs", "workers", "form"):
+            for name in ("queue", "segs", "workers", "boost", "form"):
                 afm.afm_set_option(name, 0)
     assert np.array_equal(out[1], out[2])
     assert np.array_equal(out[1, "pso"], out[2, "pso"])
     if precision == 0:
-        Jo = _oracle_forward(wl, params, trace, z0v0)
-        assert rel_err(out[2], Jo).max() < TOL_F64
+        pick = np.arange(0, n, 16) if boost else np.arange(n)   # the oracle on every 16th
+        Jo = _oracle_forward(wl, params[pick], trace, None if z0v0 is None else z0v0[pick])
+        assert rel_err(out[2][pick], Jo).max() < TOL_F64
 
 
 @pytest.mark.parametrize("lanes", [1, 2, 8, 32])
