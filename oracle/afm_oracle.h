@@ -25,11 +25,18 @@
  *   problem; the cost cutoff and the asynchronous swarm on a hand-made cost
  *   callback whose stopping batch and result are written down by hand
  *   (tests/test_oracle_pso_rules.py).
+ *   The bound rule (clamp + zero velocity), the velocity-then-position order
+ *   and the strict-improvement / lowest-index tie-break are readings (R10) the
+ *   paper does not fix; what this file does with them is pinned: the inertia-only
+ *   swarm (c1 = c2 = 0) against its closed form, a geometric series with an
+ *   absorbing bound, and exact ties on a scripted cost with the winners written
+ *   down by hand (tests/test_oracle_pso_rules.py).
  * PARITY UNPINNED (design choices with nothing outside this file to check
- * against): the PSO bound rule (clamp + zero
- * velocity), the initial-velocity rule v0 = (U(lo,hi) - x0)/2, the
- * lowest-index tie-break, the Philox counter layout, the ring of three (R23)
- * and the chunked reading of "asynchronous" (R25).
+ * against): the initial-velocity rule
+ * v0 = (U(lo,hi) - x0)/2 beyond its range, the Philox counter layout, the
+ * divergence rule (R12), the ring of three (R23) and the chunked reading of
+ * "asynchronous" (R25); the last two have hand-written expectations on scripted
+ * costs only.
  */
 #ifndef AFM_ORACLE_H
 #define AFM_ORACLE_H

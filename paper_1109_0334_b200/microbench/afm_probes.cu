@@ -266,6 +266,52 @@ int main(int argc, char** argv) {
     }
   }
 
+  if (!strcmp(what, "all") || !strcmp(what, "rk4chain")) {
+    // the same warp with its tip resting inside the sample (d = a0 / 2, the contact
+    // force balanced by the stream term): every step runs in the general form
+    const double PI = 3.14159265358979323846;
+    const double k = 2.0, f0 = 7e4, Q = 100.0, R = 1e-8, a0 = 0.3e-9, H = 1e-19, Es = 1e9;
+    const double w0 = 2 * PI * f0, m = k / (w0 * w0), hh = 1.0 / (f0 * 256.0);
+    Particle64 P;
+    memset(&P, 0, sizeof(P));
+    P.nalpha = -hh * w0 / Q;
+    P.nbeta = -hh * hh * (k / m);
+    P.a0 = a0;
+    P.c0 = -H * hh * hh * R / (6.0 * m);
+    P.c1 = (4.0 / 3.0) * Es * sqrt(R) * hh * hh / m;
+    P.c2 = P.c0 / (a0 * a0);
+    DivergeTest T;
+    T.key_max = 0x7fe0000000000000LL;
+    T.key_min = -0x7fe0000000000000LL;
+    double safe = 1e-6;
+    memcpy(&T.safe_hi, (char*)&safe + 4, 4);
+    long long a0_bits;
+    memcpy(&a0_bits, &a0, 8);
+    const double d0 = 0.5 * a0, del = a0 - d0;
+    const double s = -P.nbeta * d0 - (P.c2 + P.c1 * del * sqrt(del));
+    printf("\n## RK4 step chain, tip in contact (general form), register-only, SM cycles per step\n");
+    printf("%-44s %10s %10s\n", "", "1 warp/SM", "1 warp/sub-partition");
+    const char* names[2] = {"throughput form, rk4_step", "latency form, rk4_step"};
+    for (int v = 0; v < 2; ++v) {
+      double res[2];
+      for (int g = 0; g < 2; ++g) {
+        const int ctas = g ? 4 * n_sm : n_sm;
+        const int steps = 20000;
+        for (int rep = 0; rep < 2; ++rep) {
+          if (v == 0) rk4chain_kernel<false, 1><<<ctas, 32>>>(P, s, d0, 0.0, a0_bits, T, steps, cyc, sink);
+          else rk4chain_kernel<true, 1><<<ctas, 32>>>(P, s, d0, 0.0, a0_bits, T, steps, cyc, sink);
+          CK(cudaDeviceSynchronize());
+        }
+        static long long hc[4096];
+        CK(cudaMemcpy(hc, cyc, 8 * ctas, cudaMemcpyDeviceToHost));
+        double mx = 0;
+        for (int i = 0; i < ctas; ++i) mx = hc[i] > mx ? (double)hc[i] : mx;
+        res[g] = mx / steps;
+      }
+      printf("%-44s %10.1f %10.1f\n", names[v], res[0], res[1]);
+    }
+  }
+
   if (!strcmp(what, "all") || !strcmp(what, "dispatch")) {
     printf("\n## ns per DFMA warp-instruction per SM sub-partition\n");
     printf("%-36s %8d %8d %8d %8d\n", "warps per sub-partition:", 1, 2, 4, 8);

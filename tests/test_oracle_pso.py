@@ -3,9 +3,10 @@
 Philox is pinned by published known-answer vectors.  The PSO is pinned by
 invariants, by a hand replay of Eq. 8 on the recorded swarm state, and by
 recovery of a known ground truth from a noise-free trace on a tiny swarm
-(north_star).  The bound rule, the v0 rule, the tie-break and the counter
-layout are design readings (R10/R11): "parity unpinned" beyond
-oracle = GPU.
+(north_star).  The bound rule, the update order and the tie-break are design
+readings (R10) pinned on a closed form and on scripted ties in
+tests/test_oracle_pso_rules.py; the v0 rule and the counter layout (R10/R11) are
+"parity unpinned" beyond oracle = GPU.
 """
 import math
 import os

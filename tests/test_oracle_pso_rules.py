@@ -247,3 +247,66 @@ def test_async_ring_uses_the_neighbours_bests_known_when_the_chunk_moves():
     sync = orc.pso_core(Script(rows), 1, _box(), _swarm(P, 2, c2=1.0, topology=1), seed,
                         [[0.0]])
     assert sync["dump"][1, 1, 0] == x0[1] + _r2(seed, 1, 0) * (x0[2] - x0[1])
+
+
+# ------------------------------------------------------------ closed forms and ties
+
+def test_inertia_only_swarm_follows_the_geometric_series_and_sticks_to_the_bounds():
+    """c1 = c2 = 0 leaves v <- w v, x <- x + v (PAPER.md:209-214 with both attractor
+    terms off): a closed form.  Inside the box x_t = x_0 + v_0 (w + w^2 + ... + w^t)
+    -- the velocity is updated BEFORE the position, so the first move is w v_0, not
+    v_0 -- and the first time that leaves the box the particle is put on the bound
+    it crossed with zero velocity, where it then stays for good (reading R10).  The
+    expectation below is that series and that absorbing bound, written out; x_0 and
+    v_0 are read from the first dump row.  Also the initial-state rule: x_0 in the
+    box and |v_0| <= (hi - lo) / 2."""
+    P, n_iters, D, w = 64, 12, 2, 0.9
+    lo, hi = [0.0, -3.0], [10.0, 5.0]
+    b = orc.Box()
+    for j in range(D):
+        b.lo[j], b.hi[j], b.log10[j] = lo[j], hi[j], 0
+    r = orc.pso_core(lambda th, U: 1.0, D, b, _swarm(P, n_iters, w=w), 7, np.zeros((1, 1)))
+    dmp = r["dump"]
+    x0, v0 = dmp[0, :, 0:D], dmp[0, :, D:2 * D]
+    lo, hi = np.asarray(lo), np.asarray(hi)
+    assert np.all(x0 >= lo) and np.all(x0 <= hi)
+    assert np.all(np.abs(v0) <= 0.5 * (hi - lo))
+    assert np.abs(v0).max() > 0.25 * (hi - lo).min()      # not a degenerate start
+    stuck = np.zeros((P, D), bool)
+    where = np.zeros((P, D))
+    n_stuck_seen = 0
+    for t in range(1, n_iters):
+        series = sum(w ** k for k in range(1, t + 1))
+        free = x0 + v0 * series
+        out_lo, out_hi = (free < lo) & ~stuck, (free > hi) & ~stuck
+        where = np.where(out_lo, lo, np.where(out_hi, hi, where))
+        stuck |= out_lo | out_hi
+        want_x = np.where(stuck, where, free)
+        want_v = np.where(stuck, 0.0, v0 * w ** t)
+        np.testing.assert_allclose(dmp[t, :, 0:D], want_x, rtol=0, atol=1e-12)
+        np.testing.assert_allclose(dmp[t, :, D:2 * D], want_v, rtol=0, atol=1e-12)
+        n_stuck_seen = int(stuck.sum())
+    assert 10 < n_stuck_seen < P * D          # both regimes are exercised
+
+
+def test_equal_costs_the_lowest_index_wins_and_a_tie_never_replaces_a_best():
+    """Scripted costs with exact ties (reading R10): among equal minima the particle
+    with the lowest index is the global best; a later cost EQUAL to a personal or
+    global best replaces neither (strict <).  Frozen swarm (w = c1 = c2 = 0), so
+    every position is x_0 and the expected winner is written down by hand."""
+    P = 5
+    script = Script([[5, 3, 3, 7, 3,        # batch 0: three-way tie at 3 -> particle 1
+                      3, 3, 3, 3, 3,        # batch 1: everybody ties with the best
+                      4, 2, 9, 2, 2]])      # batch 2: three-way tie at 2 -> particle 1
+    r = orc.pso_core(script, 1, _box(), _swarm(P, 3), 11, np.zeros((1, 1)))
+    x0 = np.array([_x0(11, p) for p in range(P)])
+    gh = r["gbest_hist"]
+    assert gh[0, 0, 0] == x0[1] and gh[0, 0, 1] == 3.0
+    assert gh[1, 0, 0] == x0[1] and gh[1, 0, 1] == 3.0      # ties replace nothing
+    assert gh[2, 0, 0] == x0[1] and gh[2, 0, 1] == 2.0      # 1 before 3 and 4
+    np.testing.assert_array_equal(r["dump"][1, :, -1], [3, 3, 3, 3, 3])   # pbestJ
+    np.testing.assert_array_equal(r["dump"][2, :, -1], [3, 2, 3, 2, 2])
+    # a second script where the tie is between the last two particles only
+    script = Script([[9, 9, 9, 1, 1]])
+    r = orc.pso_core(script, 1, _box(), _swarm(P, 1), 11, np.zeros((1, 1)))
+    assert r["theta_star"][0, 0] == x0[3] and r["J_star"][0] == 1.0
