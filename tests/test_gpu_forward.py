@@ -369,3 +369,34 @@ def test_latency_form_lanes_per_warp(afm, lanes):
     assert np.array_equal(out[32][1], out[lanes][1])
     assert np.array_equal(out[32][2], out[lanes][2])
     assert rel_err(out[lanes][0], _oracle_forward(wl, params, trace)).max() < TOL_F64
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_segment_queue_random_schedules_never_change_a_result(afm, precision):
+    """The priority queue under random schedules: segment counts, workers per
+    sub-partition (more and fewer than chains) and boost thresholds drawn at random,
+    batches of 1 251 and 2 188 chains on configs[1]'s shape (random phases, so the
+    chains are very unequal and the boost fires).  Every run must reproduce the
+    one-CTA-per-warp kernel bit for bit: a missing fence or a lost slot in the queue
+    would show here as a wrong or stale misfit."""
+    import torch
+    wl = wlm.scaled(wlm.config(1), n_cycles=40, n_skip_cycles=20)
+    trace = oracle_trace(wl)
+    rng = np.random.default_rng(5 + precision)
+    for n in (40013, 70001):
+        params = wlm.draw_params(wl, n, seed=71)
+        z0v0 = wlm.draw_initial_states(wl, n, seed=72)
+        afm.afm_set_option("queue", 1)
+        afm.afm_set_option("form", 1)           # the queue serves the throughput form
+        try:
+            ref = _gpu_forward(afm, wl, params, trace, z0v0, precision=precision)
+            afm.afm_set_option("queue", 2)
+            for _ in range(10):
+                afm.afm_set_option("segs", int(rng.integers(0, 160)))
+                afm.afm_set_option("workers", int(rng.choice([0, 1, 2, 3, 4, 6])))
+                afm.afm_set_option("boost", int(rng.choice([0, 1, 2, 5, 64])))
+                got = _gpu_forward(afm, wl, params, trace, z0v0, precision=precision)
+                assert np.array_equal(got, ref)
+        finally:
+            for name in ("queue", "form", "segs", "workers", "boost"):
+                afm.afm_set_option(name, 0)
