@@ -373,10 +373,11 @@ void afm_reset_launch_count(void);
  * of a DMT-law batch by trace, initial phase and stiffness so that the lanes of a
  * warp touch the sample together: 1 = never, 2 = always, 0 = auto in the
  * throughput regime; results do not depend on it), "queue" (segment-queue
- * scheduling of the throughput forms: the time loop of every warp of particles
- * is cut into segments that persistent workers take from a priority queue keyed
- * by the segment index, fewer workers than warps of particles, so that the warps
- * that are ahead wait for the ones that are behind; 1 = never, 2 = always,
+ * scheduling of the throughput forms and of the beam kernel: the time loop of
+ * every warp of particles is cut into segments that persistent workers take from
+ * a priority queue keyed by the segment index, fewer workers than warps of
+ * particles, so that the warps that are ahead wait for the ones that are behind;
+ * 1 = never, 2 = always,
  * 0 = auto: batches of at least 1.5 warps per SM sub-partition; results do not
  * depend on it), "segs" (segments per trajectory, 0 = auto, about 1 000 steps
  * each), "workers" (queue workers per SM sub-partition, 1..8, 0 = auto),

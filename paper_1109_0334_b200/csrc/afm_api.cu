@@ -399,11 +399,14 @@ int integrate_bpt(int64_t per, int block, int ppt, int variant, int lanes) {
 // r = 3.5 and 4: 3, r = 5.5: 4, r = 8 and 12: 5 (6 to 8 are slower), configs[4]
 // (r = 55): 5 or 6.  *use is false when the plain kernel should run.  Lock held.
 int make_queue(int64_t per, int n_traces, int n_tiles, int T, bool eligible,
-               SegQueue* q, int* workers, bool* use, cudaStream_t st) {
+               SegQueue* q, int* workers, bool* use, cudaStream_t st,
+               int ckpt_doubles = 4, int max_chains_per_sub = 0) {
   const int64_t chains = (int64_t)blocks_per_trace(per, 32) * n_traces;
   const int64_t subparts = (int64_t)4 * g_n_sm;
   *use = eligible && g_opt_queue != 1 && chains < (1 << 20);
   if (*use && g_opt_queue == 0) *use = (2 * chains >= 3 * subparts && n_tiles >= 32);
+  if (*use && g_opt_queue == 0 && max_chains_per_sub > 0)
+    *use = chains <= (int64_t)max_chains_per_sub * subparts;
   if (!*use) return AFM_OK;
   int per_sub = g_opt_workers > 0 ? g_opt_workers : (int)((chains * 100) / (subparts * 115));
   if (g_opt_workers == 0 && per_sub < 2) per_sub = 2;
@@ -433,7 +436,8 @@ int make_queue(int64_t per, int n_traces, int n_tiles, int T, bool eligible,
   q->timeout_cycles = 40000000000LL;  // ~20 s: only a corrupted queue gets there
   const size_t slot_bytes = ((size_t)q->n_tasks * 4 + 255) & ~(size_t)255;
   const size_t lvl_bytes = 3 * 2048 * 4;  // head[], tail[]: segs <= 2047; park[]
-  const size_t need = 256 + lvl_bytes + slot_bytes + (size_t)chains * 128 * 8;
+  const size_t need =
+      256 + lvl_bytes + slot_bytes + (size_t)chains * 32 * (size_t)ckpt_doubles * 8;
   if (need > ((size_t)2 << 30) && g_opt_queue == 0) {  // too many chains x segments
     *use = false;
     return AFM_OK;
@@ -1129,6 +1133,25 @@ static int beam_prepare(const afm_beam_cfg* c, BeamConsts* bc, BeamModeConsts* m
   return AFM_OK;
 }
 
+// The beam integrate kernel with or without the segment queue (make_queue decides).
+static int run_beam_integrate(const BeamConsts& bc, const BeamModeConsts& mo,
+                              const IntegrateIO& io, int block, cudaStream_t st) {
+  SegQueue q;
+  int workers = 0;
+  bool use_q = false;
+  // 65 536 particles (3.46 chains per sub-partition): 71.5 -> 56.9 ms with the queue;
+  // 1 048 576 particles: 886 ms without, 900 ms with it (three of these 166-register
+  // warps saturate a sub-partition and the checkpoint is 144 B per particle)
+  int rc = make_queue(io.per, io.n_traces, bc.n_tiles, bc.T, block == 32, &q, &workers,
+                      &use_q, st, 2 * bc.M + 2, 8);
+  if (rc) return rc;
+  if (use_q)
+    LAUNCHED(launch_beam_integrate_q(bc, mo, io, q, workers, st));
+  else
+    LAUNCHED(launch_beam_integrate(bc, mo, io, block, st));
+  return AFM_OK;
+}
+
 // cos(w t) at the three abscissae of every step + the trace: the point-mass
 // stream builder with unit amplitude and no offsets.
 static int beam_stream(const BeamConsts& bc, const double* trace, int n_traces,
@@ -1200,7 +1223,7 @@ int afm_beam_forward_batch(const double* params, int64_t n_particles,
     io.box = make_box(bounds, cfg->n_params);
     io.mode = 2;
   }
-  LAUNCHED(launch_beam_integrate(bc, mo, io, block_threads(), st));
+  if ((rc = run_beam_integrate(bc, mo, io, block_threads(), st))) return rc;
   return release_ws(st);
 }
 
@@ -1261,7 +1284,7 @@ int afm_beam_pso_invert(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
   int done = 0;
   for (int it = 0; it < swarm->n_iters; ++it) {
     const bool last = (it == swarm->n_iters - 1);
-    LAUNCHED(launch_beam_integrate(bc, mo, io, block, st));
+    if ((rc = run_beam_integrate(bc, mo, io, block, st))) return rc;
     LAUNCHED(launch_pso_gbest(
         box, D, T, bpt, (Cand*)g_ws.cand.p, pbest, gbest, gbestJ,
         gbest_hist ? gbest_hist + (size_t)it * T * (D + 1) : nullptr, th_dev,

@@ -307,6 +307,172 @@ __global__ void beam_integrate_f64(BeamConsts bc, BeamModeConsts mo, IntegrateIO
   }
 }
 
+// Segment-queue form (see integrate_misfit_f64_q in afm_kernels.cu): persistent
+// one-warp workers take (chain, segment) tasks from the priority queue; between
+// segments a chain rests as { a[M], b[M], J, diverged } per particle.  Same
+// arithmetic per particle as beam_integrate_f64: bit-identical results.  65 536
+// particles are 3.46 warps per SM sub-partition, which one CTA per warp spreads as
+// 3 on some sub-partitions and 4 on others for the whole solve.
+template <int M, int MODE>
+__global__ void __launch_bounds__(32)
+beam_integrate_f64_q(BeamConsts bc, BeamModeConsts mo, IntegrateIO io, int blocks_per_tr,
+                     SegQueue q) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double4* tile0 = reinterpret_cast<double4*>(smem_raw);
+  double4* tile1 = tile0 + (bc.T + kPadRows);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tile1 + (bc.T + kPadRows));
+  __shared__ Cand red[32];
+  __shared__ SegqWorker qworker;  // lane 0's queue state (one warp per CTA)
+
+  const int tid = threadIdx.x;
+  if (tid == 0) {
+    qworker.offered = 0u;
+    tile0[bc.T] = make_double4(0.0, 0.0, 0.0, 0.0);
+    tile1[bc.T] = make_double4(0.0, 0.0, 0.0, 0.0);
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    fence_mbar_init();
+  }
+  __syncthreads();
+  uint32_t n_wait0 = 0u, n_wait1 = 0u;  // completed phases of the two stages
+  const long long a0_bits = __double_as_longlong(bc.a0);
+
+  for (;;) {
+    int task = 0;
+    if (tid == 0) task = segq_pop(q, &qworker);
+    task = __shfl_sync(0xffffffffu, task, 0);
+    if (task < 0) break;
+    const int chain = task & 0xfffff;
+    const int seg = task >> 20;
+    const int s = chain / blocks_per_tr;
+    const int64_t li = (int64_t)(chain - s * blocks_per_tr) * 32 + tid;
+    const bool active = li < io.per;
+    const int64_t gp = (int64_t)s * io.per + (active ? li : io.per - 1);
+    AFM_CHECK(s < io.n_traces && gp >= 0 && gp < io.per * io.n_traces);
+    const double* stream = io.stream + (int64_t)s * bc.N * 4;
+    const int tile_begin = seg * q.tiles_per_seg;
+    const int tile_end = min(tile_begin + q.tiles_per_seg, bc.n_tiles);
+
+    if (tid == 0) {
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        const int tile = tile_begin + k;
+        if (tile < tile_end) {
+          const int st = tile & 1;
+          const int nb = tile * bc.T;
+          const uint32_t bytes = (uint32_t)min(bc.T, bc.N - nb) * 32u;
+          fence_proxy_async();
+          mbar_arrive_expect_tx(&bars[st], bytes);
+          bulk_g2s(st ? tile1 : tile0, stream + (int64_t)nb * 4, bytes, &bars[st]);
+        }
+      }
+    }
+
+    // a1: parameter map (every segment: the chain may have come from another SM)
+    double xloc[4], th[4] = {0.0, 0.0, 0.0, 1.0};
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      xloc[j] = 0.0;
+      if (j < bc.D) {
+        const double xv = io.params[gp * bc.D + j];
+        xloc[j] = xv;
+        th[j] = (io.mode != 0 && io.box.lg[j]) ? pow(10.0, xv) : xv;
+      }
+    }
+    Particle64 P;
+    load_particle(P, bc.law, th, 0.0, 0.0, bc.a0, bc.inv_a0sq, bc.c_vdw, bc.c_hertz,
+                  bc.c_visc, bc.c_force, bc.zc, bc.c_damp);
+    double a[M], b[M];
+    double J = 0.0;
+    bool bad = false;
+    double* ck = q.ckpt + (int64_t)chain * (32 * (2 * M + 2)) + tid;
+    if (seg == 0) {
+#pragma unroll
+      for (int i = 0; i < M; ++i) a[i] = b[i] = 0.0;  // from rest
+    } else {
+#pragma unroll
+      for (int i = 0; i < M; ++i) {
+        a[i] = __ldcg(ck + 32 * i);
+        b[i] = __ldcg(ck + 32 * (M + i));
+      }
+      J = __ldcg(ck + 32 * (2 * M));
+      bad = __ldcg(ck + 32 * (2 * M + 1)) != 0.0;
+    }
+
+    for (int tile = tile_begin; tile < tile_end; ++tile) {
+      const int st = tile & 1;
+      const double4* sp = st ? tile1 : tile0;
+      mbar_wait(&bars[st], (st ? n_wait1 : n_wait0) & 1u);
+      if (st) ++n_wait1; else ++n_wait0;
+      const int n_begin = tile * bc.T;
+      const int n_steps = min(bc.T, bc.N - n_begin);
+      AFM_CHECK(n_steps >= 1 && n_steps <= bc.T && n_begin + n_steps <= bc.N);
+      double4 r = sp[0];
+      for (int i = 0; i < n_steps; ++i) {
+        const double4 rn = sp[i + 1];
+        beam_rk4<M>(mo, P, bc.law, a0_bits, bc.zc, r.x, r.y, r.z, a, b);
+        const double u = beam_tip<M>(a);
+        bad |= !(fabs(u) <= bc.u_max);  // NaN fails the comparison
+        if (n_begin + i >= bc.n0) {
+          const double res = u - r.w;
+          J = fma(res, res, J);
+        }
+        r = rn;
+      }
+      __syncthreads();
+      if (tid == 0 && tile + 2 < tile_end) {
+        const int nb = (tile + 2) * bc.T;
+        const uint32_t bytes = (uint32_t)min(bc.T, bc.N - nb) * 32u;
+        fence_proxy_async();
+        mbar_arrive_expect_tx(&bars[st], bytes);
+        bulk_g2s(st ? tile1 : tile0, stream + (int64_t)nb * 4, bytes, &bars[st]);
+      }
+    }
+
+    if (tile_end < bc.n_tiles) {
+      // hand the chain on: state first, then the task (release / acquire)
+#pragma unroll
+      for (int i = 0; i < M; ++i) {
+        __stcg(ck + 32 * i, a[i]);
+        __stcg(ck + 32 * (M + i), b[i]);
+      }
+      __stcg(ck + 32 * (2 * M), J);
+      __stcg(ck + 32 * (2 * M + 1), bad ? 1.0 : 0.0);
+      __threadfence();
+      __syncwarp();
+      if (tid == 0) segq_push(q, chain, seg + 1);
+      continue;
+    }
+
+    // last segment: the epilogue of beam_integrate_f64
+#pragma unroll
+    for (int i = 0; i < M; ++i) bad |= !(fabs(a[i]) < CUDART_INF && fabs(b[i]) < CUDART_INF);
+    if (bad || !(J == J)) J = CUDART_INF;
+    if (active) io.J[gp] = J;
+    if (MODE == 1) {
+      double pb = CUDART_INF;
+      long long idx = 0x7fffffffffffffffLL;
+      if (active) {
+        double pq = io.pbestJ[gp];
+        if (J < pq) {
+          pq = J;
+          io.pbestJ[gp] = J;
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            if (j < bc.D) io.pbest[gp * bc.D + j] = xloc[j];
+        }
+        pb = pq;
+        idx = gp;
+      }
+      block_argmin(pb, idx, red);
+      if (tid == 0) {
+        io.cand[chain].J = pb;
+        io.cand[chain].idx = idx;
+      }
+    }
+  }
+}
+
 // One particle through the same step routine (tests, trace synthesis).
 template <int M>
 __global__ void beam_trajectory_kernel(BeamConsts bc, BeamModeConsts mo,
@@ -369,6 +535,38 @@ int launch_beam_integrate(const BeamConsts& bc, const BeamModeConsts& mo,
     case 2: return launch_beam_t<2>(bc, mo, io, block, st);
     case 4: return launch_beam_t<4>(bc, mo, io, block, st);
     case 8: return launch_beam_t<8>(bc, mo, io, block, st);
+    default: return -1;
+  }
+}
+
+template <int M>
+static int launch_beam_q_t(const BeamConsts& bc, const BeamModeConsts& mo,
+                           const IntegrateIO& io, const SegQueue& q, int workers,
+                           cudaStream_t st) {
+  const int bpt = blocks_per_trace(io.per, 32);
+  const size_t smem = (size_t)(bc.T + kPadRows) * 32 * 2 + 64;
+  if (smem > 48 * 1024) {
+    cudaFuncSetAttribute(beam_integrate_f64_q<M, 1>,
+                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(beam_integrate_f64_q<M, 0>,
+                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  }
+  launch_segq_init(q, st);
+  if (io.mode == 1)
+    beam_integrate_f64_q<M, 1><<<(unsigned)workers, 32, smem, st>>>(bc, mo, io, bpt, q);
+  else
+    beam_integrate_f64_q<M, 0><<<(unsigned)workers, 32, smem, st>>>(bc, mo, io, bpt, q);
+  return 2;
+}
+
+int launch_beam_integrate_q(const BeamConsts& bc, const BeamModeConsts& mo,
+                            const IntegrateIO& io, const SegQueue& q, int workers,
+                            cudaStream_t st) {
+  switch (bc.M) {
+    case 1: return launch_beam_q_t<1>(bc, mo, io, q, workers, st);
+    case 2: return launch_beam_q_t<2>(bc, mo, io, q, workers, st);
+    case 4: return launch_beam_q_t<4>(bc, mo, io, q, workers, st);
+    case 8: return launch_beam_q_t<8>(bc, mo, io, q, workers, st);
     default: return -1;
   }
 }

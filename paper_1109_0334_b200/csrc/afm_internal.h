@@ -136,7 +136,8 @@ struct SegQueue {
   int32_t boost_div;     // a task is behind when more than n_chains / boost_div chains
                          // have finished its level
   double* ckpt;          // [n_chains][4][32] doubles: d, w, J, diverged flag of a chain at
-                         // rest (FP32 kernel: [n_chains][8][32] floats, same size)
+                         // rest (FP32 kernel: [n_chains][8][32] floats, same size; beam
+                         // kernel: [n_chains][2 M + 2][32] doubles)
   long long timeout_cycles;
   int32_t n_chains;
   int32_t n_segs;
@@ -207,6 +208,9 @@ int launch_beam_setup(const afm_beam_cfg& cfg, double h, BeamModeConsts* dev_out
                       cudaStream_t st);
 int launch_beam_integrate(const BeamConsts& bc, const BeamModeConsts& mo,
                           const IntegrateIO& io, int block, cudaStream_t st);
+int launch_beam_integrate_q(const BeamConsts& bc, const BeamModeConsts& mo,
+                            const IntegrateIO& io, const SegQueue& q, int workers,
+                            cudaStream_t st);
 int launch_beam_trajectory(const BeamConsts& bc, const BeamModeConsts& mo,
                            const double* theta_dev, const double* stream,
                            double* tip_u, double* tip_v, cudaStream_t st);

@@ -146,3 +146,45 @@ def test_inversion_replays_the_oracle_and_recovers_the_truth(afm):
     rel = np.abs(r["theta_star"][0] - np.array(wf["truth"])) / np.array(wf["truth"])
     print("beam inversion theta* rel err", rel, "J*", r["J_star"])
     assert rel.max() < 1e-2
+
+
+@pytest.mark.parametrize("segs,workers,n_modes", [(0, 0, 8), (5, 1, 8), (36, 3, 4), (2, 8, 2)])
+def test_segment_queue_changes_no_beam_result(afm, segs, workers, n_modes):
+    """beam_integrate_f64_q (persistent workers, priority queue of time segments, the
+    modal state of a chain checkpointed between segments) against the one-CTA-per-warp
+    kernel: misfits of a ragged multi-trace batch and the swarm of a short inversion
+    must be bit-identical; (5, 1): 626 chains on 592 workers, so chains wait."""
+    import torch
+    wl = wlm.scaled(wlm.beam_workload(), n_cycles=36, n_skip_cycles=18, n_traces=3,
+                    n_particles=77, n_iters=3)
+    wl = dict(wl, beam=dict(wl["beam"], n_modes=n_modes))
+    B = orc.beam_from(wl)
+    truths = wlm.theta_of_coords(wl, wlm.draw_coords(wl, 3, seed=5))
+    trace = np.stack([orc.beam_window(B, t)[1] for t in truths]) + wlm.trace_noise(wl)
+    n = 3 * 6677 if workers == 1 else 3 * 313
+    params = wlm.draw_params(wl, n, seed=42)
+    cfg = afm.beam_cfg_from(wl)
+    t = torch.as_tensor(trace, device="cuda")
+    out = {}
+    for queue in (1, 2):
+        afm.afm_set_option("queue", queue)
+        afm.afm_set_option("segs", segs)
+        afm.afm_set_option("workers", workers)
+        try:
+            J = afm.afm_beam_forward_batch(torch.as_tensor(params, device="cuda"), t, cfg)
+            g = afm.afm_beam_pso_invert(afm.bounds_from(wl), afm.swarm_from(wl), 3, t, cfg,
+                                        dump=True)
+            torch.cuda.synchronize()
+            out[queue] = (J.cpu().numpy(), g["dump"].cpu().numpy(), g["theta_star"])
+        finally:
+            for name in ("queue", "segs", "workers"):
+                afm.afm_set_option(name, 0)
+    for a, b in zip(out[1], out[2]):
+        assert np.array_equal(a, b)
+    pick = np.arange(0, n, 97)
+    # the oracle on a sample of the batch (trace of each sampled particle's segment)
+    per = n // 3
+    for s in range(3):
+        idx = pick[(pick >= s * per) & (pick < (s + 1) * per)]
+        Jo = orc.beam_forward_batch(B, params[idx], trace[s:s + 1], n_traces=1, openmp=True)
+        assert rel_err(out[2][0][idx], Jo).max() < 1e-9
