@@ -383,7 +383,8 @@ void afm_reset_launch_count(void);
  * each), "workers" (queue workers per SM sub-partition, 1..8, 0 = auto),
  * "boost" (0 = auto, 1 = off, k >= 2: a worker that takes a segment which more
  * than 1/k of the warps of particles have already finished makes one other
- * worker of its sub-partition pause for that segment; auto = 2).
+ * worker of its sub-partition pause for that segment; auto = 2), "boost2"
+ * (0 = auto: a segment two behind makes two other workers pause, 1 = off).
  * Returns AFM_EINVAL for an unknown name or value. */
 int afm_set_option(const char* name, int64_t value);
 

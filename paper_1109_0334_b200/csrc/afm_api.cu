@@ -59,6 +59,7 @@ int g_opt_pack = 0;   // 0 = auto, 1 = never, 2 = always (DMT laws only)
 int g_opt_queue = 0;  // 0 = auto, 1 = never, 2 = always: segment-queue scheduling
 int g_opt_segs = 0;   // 0 = auto (~450 steps each): time segments per chain of the queue kernel
 int g_opt_workers = 0;  // 0 = auto: queue workers per SM sub-partition
+int g_opt_boost2 = 0;   // 0 = auto (on), 1 = off: a second parking place for a chain two segments behind
 int g_opt_boost = 0;    // 0 = auto (2), 1 = off, k >= 2: parking beside the chains that are behind
                         // more than 1/k of the chains by a whole segment
 int g_n_sm = 148;
@@ -452,6 +453,7 @@ int make_queue(int64_t per, int n_traces, int n_tiles, int T, bool eligible,
   q->park = q->tail + 2048;
   q->n_park = (g_opt_boost != 1 && subparts <= 2048) ? (int32_t)subparts : 0;
   q->boost_div = g_opt_boost >= 2 ? g_opt_boost : 2;
+  q->boost_two = g_opt_boost2 != 1 ? 1 : 0;
   q->slots = (int*)((char*)g_ws.segq.p + 256 + lvl_bytes);
   q->ckpt = (double*)((char*)g_ws.segq.p + 256 + lvl_bytes + slot_bytes);
   return AFM_OK;
@@ -1531,6 +1533,11 @@ int afm_set_option(const char* name, int64_t value) {
   if (!strcmp(name, "workers")) {
     if (value < 0 || value > 8) return fail(AFM_EINVAL, "workers must be in 0..8");
     g_opt_workers = (int)value;
+    return AFM_OK;
+  }
+  if (!strcmp(name, "boost2")) {
+    if (value < 0 || value > 1) return fail(AFM_EINVAL, "boost2 must be 0 or 1");
+    g_opt_boost2 = (int)value;
     return AFM_OK;
   }
   if (!strcmp(name, "boost")) {

@@ -174,35 +174,57 @@ __device__ __forceinline__ unsigned smsp_id() {
 // far above the rest (a warp with a particle stuck to the sample runs every step
 // in the general form): always picked up at once, always running, they still
 // fall behind and set the time of the batch.  A worker that takes a task of a
-// level most chains have already finished marks its sub-partition: one of the
-// other workers there, when it next comes for a task, parks until the marked
-// segment is over, and the chain that is behind runs with one warp fewer beside
-// it (a third faster at three warps per sub-partition).  q.park[smsp]: 0 = free,
-// 1 = a parking place is offered, 2 = taken.  Called by one lane.
+// level most chains have already finished offers a parking place on its
+// sub-partition -- two places if most chains have finished the level after it as
+// well: another worker there, when it next comes for a task, takes a place and
+// sleeps until the marked segment is over, and the chain that is behind runs
+// beside one warp fewer (a third faster at three warps per sub-partition) or
+// alone.  q.park[smsp]: bits 0-7 = places on offer, bits 8-15 = epoch, advanced
+// when a marked segment ends (which wakes the sleepers).  Called by one lane.
 struct SegqWorker {
-  unsigned offered;  // this worker's offer of a parking place is standing
+  unsigned offered;  // places this worker has put on offer for its current segment
 };
 __device__ __forceinline__ int segq_pop(const SegQueue& q, SegqWorker* wk) {
   unsigned& offered = wk->offered;
   const unsigned sp = smsp_id();
   if (sp >= (unsigned)q.n_park) return segq_take(q);
   unsigned* pk = &q.park[sp];
-  if (offered == 1u) {
+  if (offered != 0u) {
+    // the marked segment is over: withdraw what is left of the offer, wake the rest
     offered = 0u;
-    atomicExch(pk, 0u);  // the marked segment is over: release the parked worker
-  } else if (ld_relaxed_u32(pk) == 1u && atomicCAS(pk, 1u, 2u) == 1u) {
-    unsigned waited = 0;
-    while (ld_relaxed_u32(pk) == 2u && (int)ld_relaxed_u32(&q.ctrl[0]) < q.n_segs &&
-           ++waited < 200000u)
-      __nanosleep(2000);
+    unsigned w = ld_relaxed_u32(pk), seen;
+    do {
+      seen = w;
+      w = atomicCAS(pk, seen, ((seen & 0xff00u) + 0x100u) & 0xff00u);
+    } while (w != seen);
+  } else {
+    unsigned w = ld_relaxed_u32(pk);
+    while ((w & 0xffu) != 0u) {
+      const unsigned seen = w;
+      w = atomicCAS(pk, seen, seen - 1u);
+      if (w != seen) continue;
+      const unsigned epoch = seen & 0xff00u;
+      unsigned waited = 0;
+      while ((ld_relaxed_u32(pk) & 0xff00u) == epoch &&
+             (int)ld_relaxed_u32(&q.ctrl[0]) < q.n_segs && ++waited < 200000u)
+        __nanosleep(2000);
+      break;
+    }
   }
   const int task = segq_take(q);
   if (task >= 0) {
     const int l = task >> 20;
-    if (l + 1 < q.n_segs &&
-        (unsigned)q.boost_div * ld_relaxed_u32(&q.tail[l + 1]) > (unsigned)q.n_chains &&
-        atomicCAS(pk, 0u, 1u) == 0u)
-      offered = 1u;
+    const unsigned nc = (unsigned)q.n_chains, div = (unsigned)q.boost_div;
+    unsigned want = 0u;
+    if (l + 1 < q.n_segs && div * ld_relaxed_u32(&q.tail[l + 1]) > nc) {
+      want = 1u;
+      if (q.boost_two && l + 2 < q.n_segs && div * ld_relaxed_u32(&q.tail[l + 2]) > nc)
+        want = 2u;
+    }
+    if (want != 0u) {
+      atomicAdd(pk, want);
+      offered = want;
+    }
   }
   return task;
 }

@@ -133,6 +133,7 @@ struct SegQueue {
   unsigned* tail;        // [n_segs] tasks published (slots reserved) per level
   unsigned* park;        // [n_park] parking place per SM sub-partition (segq_pop)
   int32_t n_park;        // 4 * SMs, or 0: no boost of the chains that are behind
+  int32_t boost_two;     // 1: a task two levels behind gets a second parking place
   int32_t boost_div;     // a task is behind when more than n_chains / boost_div chains
                          // have finished its level
   double* ckpt;          // [n_chains][4][32] doubles: d, w, J, diverged flag of a chain at

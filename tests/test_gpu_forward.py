@@ -395,8 +395,9 @@ def test_segment_queue_random_schedules_never_change_a_result(afm, precision):
                 afm.afm_set_option("segs", int(rng.integers(0, 160)))
                 afm.afm_set_option("workers", int(rng.choice([0, 1, 2, 3, 4, 6])))
                 afm.afm_set_option("boost", int(rng.choice([0, 1, 2, 5, 64])))
+                afm.afm_set_option("boost2", int(rng.choice([0, 1])))
                 got = _gpu_forward(afm, wl, params, trace, z0v0, precision=precision)
                 assert np.array_equal(got, ref)
         finally:
-            for name in ("queue", "form", "segs", "workers", "boost"):
+            for name in ("queue", "form", "segs", "workers", "boost", "boost2"):
                 afm.afm_set_option(name, 0)
