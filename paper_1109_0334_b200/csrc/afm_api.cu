@@ -399,20 +399,33 @@ int integrate_bpt(int64_t per, int block, int ppt, int variant, int lanes) {
 // r chains per sub-partition, best workers per sub-partition): r = 2.5: 2,
 // r = 3.5 and 4: 3, r = 5.5: 4, r = 8 and 12: 5 (6 to 8 are slower), configs[4]
 // (r = 55): 5 or 6.  *use is false when the plain kernel should run.  Lock held.
+// Workers per SM sub-partition the queue kernels would run for this batch, 0 = the
+// plain kernel runs.  Lock held.
+int queue_per_sub(int64_t per, int n_traces, int64_t n_steps, bool eligible,
+                  int max_chains_per_sub) {
+  const int64_t chains = (int64_t)blocks_per_trace(per, 32) * n_traces;
+  const int64_t subparts = (int64_t)4 * g_n_sm;
+  bool use = eligible && g_opt_queue != 1 && chains < (1 << 20);
+  if (use && g_opt_queue == 0) use = (2 * chains >= 3 * subparts && n_steps >= 2048);
+  if (use && g_opt_queue == 0 && max_chains_per_sub > 0)
+    use = chains <= (int64_t)max_chains_per_sub * subparts;
+  if (!use) return 0;
+  int per_sub = g_opt_workers > 0 ? g_opt_workers : (int)((chains * 100) / (subparts * 115));
+  if (g_opt_workers == 0 && per_sub < 2) per_sub = 2;
+  if (g_opt_workers == 0 && per_sub > 5) per_sub = 5;
+  if (per_sub > 8) per_sub = 8;
+  return per_sub;
+}
+
 int make_queue(int64_t per, int n_traces, int n_tiles, int T, bool eligible,
                SegQueue* q, int* workers, bool* use, cudaStream_t st,
                int ckpt_doubles = 4, int max_chains_per_sub = 0) {
   const int64_t chains = (int64_t)blocks_per_trace(per, 32) * n_traces;
   const int64_t subparts = (int64_t)4 * g_n_sm;
-  *use = eligible && g_opt_queue != 1 && chains < (1 << 20);
-  if (*use && g_opt_queue == 0) *use = (2 * chains >= 3 * subparts && n_tiles >= 32);
-  if (*use && g_opt_queue == 0 && max_chains_per_sub > 0)
-    *use = chains <= (int64_t)max_chains_per_sub * subparts;
+  const int per_sub =
+      queue_per_sub(per, n_traces, (int64_t)n_tiles * T, eligible, max_chains_per_sub);
+  *use = per_sub > 0;
   if (!*use) return AFM_OK;
-  int per_sub = g_opt_workers > 0 ? g_opt_workers : (int)((chains * 100) / (subparts * 115));
-  if (g_opt_workers == 0 && per_sub < 2) per_sub = 2;
-  if (g_opt_workers == 0 && per_sub > 5) per_sub = 5;
-  if (per_sub > 8) per_sub = 8;
   *workers = (int)(per_sub * subparts);
   if (*workers > chains) *workers = (int)chains;
   // segments of about 1 000 steps (250 us at 3 FP64 warps per sub-partition: long
@@ -459,14 +472,32 @@ int make_queue(int64_t per, int n_traces, int n_tiles, int T, bool eligible,
   return AFM_OK;
 }
 
-int run_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block,
+int run_integrate_f64(const ModelConsts& mc_in, const IntegrateIO& io, int block,
                       int variant, cudaStream_t st) {
   SegQueue q;
   int workers = 0;
   bool use_q = false;
-  int rc = make_queue(io.per, io.n_traces, mc.n_tiles, mc.T, variant == 0 && block == 32,
-                      &q, &workers, &use_q, st);
+  const bool eligible = variant == 0 && block == 32;
+  // The queue kernels run 2 to 5 one-warp CTAs per sub-partition, so there is shared
+  // memory for longer time tiles (fewer barrier waits and bulk copies per step;
+  // configs[1]: 64 rows 12.31 ms, 128: 12.21, 256: 12.15, and 512 rows no longer
+  // fit 12 CTAs per SM: 18.1 ms).  The tile length changes no FP64 result (the
+  // misfit is summed step by step); the FP32 kernel folds its sum once per tile and
+  // keeps its own tile length.
+  ModelConsts mc = mc_in;
+  const int per_sub = queue_per_sub(io.per, io.n_traces, mc.N, eligible, 0);
+  if (per_sub > 0 && g_opt_tile == 0) {
+    int T = per_sub <= 3 ? 256 : (per_sub <= 5 ? 128 : 64);
+    if (T > mc.N) T = mc.N;
+    if (T > mc.T) {
+      mc.T = T;
+      mc.n_tiles = (mc.N + T - 1) / T;
+    }
+  }
+  int rc = make_queue(io.per, io.n_traces, mc.n_tiles, mc.T, eligible, &q, &workers,
+                      &use_q, st);
   if (rc) return rc;
+  if (!use_q) mc = mc_in;
   if ((rc = kev_record(0, st))) return rc;
   if (use_q)
     LAUNCHED(launch_integrate_f64_q(mc, io, q, workers, st));
