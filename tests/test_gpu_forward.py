@@ -378,8 +378,11 @@ def test_segment_queue_random_schedules_never_change_a_result(afm, precision):
     batches of 1 251 and 2 188 chains on configs[1]'s shape (random phases, so the
     chains are very unequal and the boost fires).  Every run must reproduce the
     one-CTA-per-warp kernel bit for bit: a missing fence or a lost slot in the queue
-    would show here as a wrong or stale misfit."""
+    would show here as a wrong or stale misfit.  AFM_QUEUE_STRESS=n repeats the
+    draw n times per batch instead of 10 (profiles/r2_bounds_check.md)."""
+    import os
     import torch
+    reps = int(os.environ.get("AFM_QUEUE_STRESS", "10"))
     wl = wlm.scaled(wlm.config(1), n_cycles=40, n_skip_cycles=20)
     trace = oracle_trace(wl)
     rng = np.random.default_rng(5 + precision)
@@ -391,7 +394,7 @@ def test_segment_queue_random_schedules_never_change_a_result(afm, precision):
         try:
             ref = _gpu_forward(afm, wl, params, trace, z0v0, precision=precision)
             afm.afm_set_option("queue", 2)
-            for _ in range(10):
+            for _ in range(reps):
                 afm.afm_set_option("segs", int(rng.integers(0, 160)))
                 afm.afm_set_option("workers", int(rng.choice([0, 1, 2, 3, 4, 6])))
                 afm.afm_set_option("boost", int(rng.choice([0, 1, 2, 5, 64])))
