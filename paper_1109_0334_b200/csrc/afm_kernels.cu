@@ -296,20 +296,21 @@ __global__ void integrate_misfit_f64(ModelConsts mc, IntegrateIO io,
 // ============================================================================
 // integrate-and-misfit, FP64, segment queue (throughput form, one warp per CTA).
 //
-// A forward batch of a few warps per SM sub-partition is unbalanced when every
-// warp is bound to one sub-partition for its whole trajectory: 2 048 warps on
-// 592 sub-partitions leave 3 on some and 4 on others, warps differ up to 3x in
-// cost (general-form steps), and the slowest sub-partition sets the time.  Here
-// the time loop of a warp of particles (a "chain") is cut into segments of
-// q.tiles_per_seg time tiles; a grid of persistent one-warp CTAs (workers, a
-// whole number per sub-partition) takes (chain, segment) tasks from a
-// multi-producer multi-consumer ticket queue in global memory.  A worker that
-// finishes a segment stores the chain's state (d, w, J, diverged flag: 32 B per
-// particle), publishes the chain's next segment at the tail of the queue and
-// takes the ticket at its head; since there are more workers than chains, the
-// published task is picked up at once by the worker that has waited longest, so
-// every chain is always running and the idle slots rotate evenly over all
-// sub-partitions.  The arithmetic of a particle is that of
+// With every warp of particles bound to one SM sub-partition for its whole
+// trajectory a batch is unbalanced twice over: 2 048 warps on 592 sub-partitions
+// leave 3 on some and 4 on others, and warps differ up to 2x in cost (general-form
+// steps; a warp with one particle stuck to the sample runs every step in the
+// general form), so the slowest warp sets the time.  Here the time loop of a warp
+// of particles (a "chain") is cut into segments of q.tiles_per_seg time tiles; a
+// grid of persistent one-warp CTAs (workers, a whole number per sub-partition,
+// FEWER than chains) takes (chain, segment) tasks from a priority queue in global
+// memory keyed by the segment index (segq_pop / segq_push in
+// afm_device_common.cuh).  A worker that finishes a segment stores the chain's
+// state (d, w, J, diverged flag: 32 B per particle), publishes the chain's next
+// segment and takes the oldest task of the lowest segment index on offer: the
+// chains that are ahead wait, the ones that are behind are picked up at once, and
+// the few that still cannot keep up get their sub-partition to themselves (the
+// boost in segq_pop).  The arithmetic of a particle is that of
 // integrate_misfit_f64<LAW, MODE, 1, false>, step for step: results are
 // bit-identical.
 // ============================================================================
