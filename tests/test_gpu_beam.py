@@ -188,3 +188,34 @@ def test_segment_queue_changes_no_beam_result(afm, segs, workers, n_modes):
         idx = pick[(pick >= s * per) & (pick < (s + 1) * per)]
         Jo = orc.beam_forward_batch(B, params[idx], trace[s:s + 1], n_traces=1, openmp=True)
         assert rel_err(out[2][0][idx], Jo).max() < 1e-9
+
+
+def test_full_size_batch_as_benched(afm):
+    """The batch bench.py --one-batch 7 times (65 536 particles x 40 960 steps x 8
+    modes, default options: the segment-queue kernel with 3 workers per
+    sub-partition): every 512th particle against the oracle at 1e-9, every misfit
+    finite, and the plain kernel gives the same bits."""
+    import torch
+    wl = wlm.beam_workload()
+    B = orc.beam_from(wl)
+    trace = _trace(wl, B)
+    n = 65536
+    params = wlm.draw_params(wl, n, seed=1)
+    cfg = afm.beam_cfg_from(wl)
+    t = torch.as_tensor(trace, device="cuda")
+    p = torch.as_tensor(params, device="cuda")
+    J = afm.afm_beam_forward_batch(p, t, cfg)
+    afm.afm_set_option("queue", 1)
+    try:
+        Jp = afm.afm_beam_forward_batch(p, t, cfg)
+        torch.cuda.synchronize()
+    finally:
+        afm.afm_set_option("queue", 0)
+    assert torch.equal(J, Jp)
+    Jg = J.cpu().numpy()
+    assert np.all(np.isfinite(Jg))
+    pick = np.arange(0, n, 512)
+    Jo = orc.beam_forward_batch(B, params[pick], trace, openmp=True)
+    e = rel_err(Jg[pick], Jo)
+    print("beam full size: median %.2e max %.2e" % (np.median(e), e.max()))
+    assert e.max() < 1e-9, (e.max(), int(e.argmax()))
