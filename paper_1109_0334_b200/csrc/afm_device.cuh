@@ -157,6 +157,26 @@ __device__ __forceinline__ double accel_both(const Particle64& P, double s,
       : LAT          ? fma(P.nalpha, w, vdw_plus(P.c0, d * d, b0))
                      : fma(P.nalpha, w, fma(P.c0, rcp_fast(d * d), b0));
   const double del = P.a0 - d;
+  if (WFOLD && (LAT || LAW != AFM_LAW_DMT_VISC)) {
+    // stages 1 and 3 (their velocity is known before the square-root chain ends):
+    // the correction of the square root is folded into the sum,
+    //   c1 del sqrt(del) [+ c3 sqrt(del) w] = M (1 + p),  M = (c1 del [+ c3 w]) g0,
+    // so the stage ends one FMA after p instead of three operations (the general
+    // form is what the slowest warp of a batch runs, and a lone warp in the latency
+    // regime: configs[1] 12.21 -> 12.03 ms, configs[2] 693 -> 671 ms, configs[0]
+    // 6.05 -> 5.90 ms).  One more instruction for the plain DMT law, three more
+    // with the viscous term: there the throughput form keeps the short count
+    // (configs[4] 54.7 ms against 55.4).
+    const double y0 = rsqrt_seed(del);
+    const double g0 = del * y0;
+    const double e = fma(-g0, y0, 1.0);
+    const double p = fma(0.375, e, 0.5) * e;
+    const double cm = (LAW == AFM_LAW_DMT_VISC) ? fma(P.c3, w, P.c1 * del) : P.c1 * del;
+    const double M = cm * g0;
+    const double R = fma(P.nalpha, w, P.c2 + b0);
+    const double g_c = fma(M, p, M + R);
+    return ge_pos(d, a0_bits) ? g_free : g_c;
+  }
   const double sq = sqrt_fast(del);
   const double part = fma(P.c1 * del, sq, P.c2 + b0);
   // viscous term -nu sqrt(delta) w joins the -alpha w term: one coefficient
