@@ -63,40 +63,41 @@ __device__ __forceinline__ double sqrt_fast(double x) {
   return fma(g0, p, g0);
 }
 
-// exp(x) with a short dependent chain (the LJ+exp law is latency-bound: a swarm
-// of 8 192 particles is 256 warps on 592 sub-partitions).  x = n ln2 + f with
-// n = rint(x log2 e), |f| <= 0.3466; exp(f) by its Taylor polynomial of degree
-// 13 (remainder f^14/14! <= 4.2e-18 relative) evaluated by Estrin's scheme: four
-// FMA levels instead of thirteen; 2^n goes into the exponent field.  Below
-// x log2 e = -1000 the result is 0 (exp < 1e-301: the adhesion term vanishes
-// against any tolerance), above 1023 it is +Inf (a diverging trajectory, R12).
+// exp(x) with few instructions and a short dependent chain (the LJ+exp law runs in
+// the latency regime: a swarm of 8 192 particles is 256 warps on 592 sub-partitions,
+// and a lone warp issues one FP64 instruction every 2.5 cycles).  x = n ln2 + f with
+// n = rint(x log2 e), |f| <= 0.3466; exp(f) by a polynomial of degree 11 -- the
+// Chebyshev fit on [-ln2/2, ln2/2] (mpmath.chebyfit at 60 digits, coefficients
+// rounded to FP64: relative error <= 1.7e-17; the Taylor polynomial needs degree 13
+// for that) -- evaluated by Estrin's scheme: four FMA levels; 2^n goes into the
+// exponent field.  n is clamped on the ALU pipe (two FP64 compares and four selects
+// on the result cost 15 % of a configs[3] batch): at n = 1024 the exponent field is
+// all ones (non-finite: a diverging trajectory, R12), at n = -1022 the result is
+// below 2^-1021 (the true value is smaller still; the adhesion term vanishes against
+// any tolerance either way).
 __device__ __forceinline__ double exp_fast(double x) {
-  const double t = x * 1.4426950408889634;
   const double magic = 6755399441055744.0;  // 1.5 * 2^52: rint by add/sub
-  const double nm = t + magic;
+  const double nm = fma(x, 1.4426950408889634, magic);
   const double n = nm - magic;
   double f = fma(n, -6.93147180369123816490e-01, x);  // ln2 high part
   f = fma(n, -1.90821492927058770002e-10, f);         // ln2 low part
   const double f2 = f * f;
-  const double a0 = fma(f, 1.0, 1.0);
-  const double a1 = fma(f, 1.0 / 6.0, 0.5);
-  const double a2 = fma(f, 1.0 / 120.0, 1.0 / 24.0);
-  const double a3 = fma(f, 1.0 / 5040.0, 1.0 / 720.0);
-  const double a4 = fma(f, 1.0 / 362880.0, 1.0 / 40320.0);
-  const double a5 = fma(f, 1.0 / 39916800.0, 1.0 / 3628800.0);
-  const double a6 = fma(f, 1.0 / 6227020800.0, 1.0 / 479001600.0);
+  const double a0 = f + 1.0;
+  const double a1 = fma(f, 0.1666666666666668, 0.5000000000000019);
+  const double a2 = fma(f, 0.008333333333319601, 0.0416666666664881);
+  const double a3 = fma(f, 0.00019841269890047113, 0.0013888888952314775);
+  const double a4 = fma(f, 2.755724091857897e-06, 2.4801485482328494e-05);
+  const double a5 = fma(f, 2.5110037605963777e-08, 2.763263963904103e-07);
   const double f4 = f2 * f2;
   const double b0 = fma(a1, f2, a0);
   const double b1 = fma(a3, f2, a2);
   const double b2 = fma(a5, f2, a4);
   const double f8 = f4 * f4;
   const double g0 = fma(b1, f4, b0);
-  const double g1 = fma(a6, f4, b2);
-  const double pv = fma(g1, f8, g0);
+  const double pv = fma(b2, f8, g0);
   // 2^n into the exponent: n is the low word of nm (two's complement)
-  const int ni = __double2loint(nm);
-  const double r = __hiloint2double(__double2hiint(pv) + (ni << 20), __double2loint(pv));
-  return (t > 1023.0) ? CUDART_INF : ((t < -1000.0) ? 0.0 : r);
+  const int nc = max(min(__double2loint(nm), 1024), -1022);
+  return __hiloint2double(__double2hiint(pv) + (nc << 20), __double2loint(pv));
 }
 
 // ---- per-particle constants in registers ------------------------------------
@@ -194,9 +195,10 @@ __device__ __forceinline__ double accel_smooth(const Particle64& P, double s,
     const double r = rcp_fast(d * d);
     const double r2 = r * r;
     const double r4 = r2 * r2;
-    double f = fma(P.c0, r4, fma(P.c1, r, b0));
-    f = fma(P.c2, exp_fast(d * P.c3), f);
-    return fma(P.nalpha, w, f);
+    // the exponential is the last operand to arrive (its chain is the longer one),
+    // so everything else is summed before it (configs[3] FP64 batch 22.1 -> 21.2 ms)
+    const double g = fma(P.nalpha, w, fma(P.c0, r4, fma(P.c1, r, b0)));
+    return fma(P.c2, exp_fast(d * P.c3), g);
   }
   if (LAW == AFM_LAW_HOOKE || LAW == AFM_LAW_KELVIN_VOIGT) {
     // the paper's sample models (Eq. 11, 12): a spring (and a damper) that act
@@ -258,12 +260,15 @@ __device__ __forceinline__ void rk4_combine(double dw, double w, double k1, doub
                                             double k3, double k4, double& dn,
                                             double& wn) {
   const double sixth = 1.0 / 6.0;
-  const double t23 = k2 + k3;
   if (LAT) {
     const double a12 = k1 + k2;
     dn = fma(k3, sixth, fma(a12, sixth, dw));
-    wn = fma((a12 + t23) + (k3 + k4), sixth, w);
+    // w' one FMA after k4 and two after k3 (k1 + 2 k2 is ready before k3): the next
+    // step's first stage takes w' into its constant term, and w' used to arrive
+    // after that stage's reciprocal (configs[2] 671 -> 641 ms, configs[0] 5.9 -> 5.7)
+    wn = fma(k4, sixth, fma(fma(2.0, k3, fma(2.0, k2, k1)), sixth, w));
   } else {
+    const double t23 = k2 + k3;
     const double s3 = k1 + t23;
     dn = fma(s3, sixth, dw);
     wn = fma((s3 + t23) + k4, sixth, w);
@@ -339,7 +344,7 @@ __device__ __forceinline__ void rk4_step(const Particle64 (&P)[PPT], double s0,
       const double w3 = fma(0.5, k2, w[q]);
       const double k3 =
           accel_smooth<LAW>(P[q], sh, stage3_gap(d2[q], k1), w3);
-      const double k4 = accel_smooth<LAW>(P[q], s1, d[q] + w3, w[q] + k3);
+      const double k4 = accel_smooth<LAW>(P[q], s1, fma(0.5, k2, dw[q]), w[q] + k3);  // = d + w3
       rk4_combine<LAT>(dw[q], w[q], k1, k2, k3, k4, d[q], w[q]);
       bad[q] |= diverged_step(d[q], T);
     }
