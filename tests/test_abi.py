@@ -177,7 +177,8 @@ def test_new_entry_points_validate_before_touching_the_device(lib):
                                  z.ctypes.data, z.ctypes.data, z.ctypes.data, z.ctypes.data,
                                  z.ctypes.data, None) == afm.EINVAL
     for name, bad in (("form", 3), ("lanes", 3), ("pack", 5), ("ppt", 4), ("tile", -1),
-                      ("queue", 3), ("segs", 5000), ("workers", 9), ("kernel_events", 2)):
+                      ("queue", 3), ("segs", 5000), ("workers", 9), ("boost", 65), ("boost2", 2),
+                      ("kernel_events", 2)):
         with pytest.raises(afm.AfmError):
             afm.afm_set_option(name, bad)
         assert afm.afm_set_option(name, 0) is None
