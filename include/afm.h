@@ -163,6 +163,54 @@ int afm_forward_batch_host(const double* params, int64_t n_particles,
                            const double* z0v0, double* misfit,
                            void* cuda_stream);
 
+/* ---- forward problem + cost for callers that must not allocate ------------
+ * Same computation and same arguments as afm_forward_batch (device pointers,
+ * asynchronous on cuda_stream), for callers that cannot let this library call
+ * cudaMalloc / cudaFree on their behalf.  The ordinary calls keep a device
+ * workspace that is created on first use and re-created (free + malloc)
+ * whenever a larger batch arrives.  Two kinds of caller cannot live with that:
+ *   - the acquisition loop of a running microscope, the paper's "near
+ *     real-time" setting: cudaMalloc and cudaFree take
+ *     driver-wide locks, may wait for all work on the device and have no upper
+ *     bound on their duration, so one of them in the middle of a scan line
+ *     breaks the loop's timing;
+ *   - a process whose device memory is already owned by someone else's pool
+ *     (a framework's caching allocator, a vendor acquisition stack): an
+ *     allocation made behind the pool's back can fail although the pool has
+ *     room, or take memory the pool counts on.
+ * This entry point calls no cudaMalloc, cudaFree, event/stream creation or
+ * allocating library routine.  Its only scratch, the time-tile stream (one
+ * 32-byte row per trace and RK4 step: the drive at the three RK4 abscissae and
+ * the shifted trace sample), lives in an array of AFM_NOALLOC_MAX_ROWS rows
+ * (4 MiB) that is compiled into the library's device image: every GPU on which
+ * this library's kernels are loaded holds those 4 MiB until the process exits,
+ * whether or not this call is ever used.
+ *   Limit: cfg->n_traces * cfg->steps_per_cycle * cfg->n_cycles must not
+ *     exceed AFM_NOALLOC_MAX_ROWS, else AFM_EINVAL with the numbers in
+ *     afm_last_error() (configs[0]..[3] of BASELINE.json fit with one trace;
+ *     configs[4]'s 256 traces do not: use afm_forward_batch there).
+ *   First call on a device: looks up the device address of the built-in array
+ *     (a runtime query that also loads the library's kernels onto that device)
+ *     and remembers it for the life of the process.  Make that first call once
+ *     per device at start-up, with that device current and outside any stream
+ *     capture; later calls only enqueue two kernels.
+ *   Sharing: there is ONE array per device, used by every call and never
+ *     cleared; it holds what the previous call left there.  That is harmless
+ *     in sequence, because each call writes every row it is going to read
+ *     before it reads it, but two calls that overlap on the GPU (different
+ *     streams, or different host threads, without an ordering between them)
+ *     overwrite each other's rows and both return garbage.  Keep all calls on
+ *     one stream, or order them with events of your own.
+ *   Scheduling: runs the plain one-launch integrate kernel.  The warp packing
+ *     and the segment queue of afm_forward_batch need scratch that grows with
+ *     the batch and are not used here, so large batches run at the speed of
+ *     afm_set_option("queue", 1) + ("pack", 1); the misfits are the same. */
+#define AFM_NOALLOC_MAX_ROWS 131072
+int afm_forward_batch_noalloc(const double* params, int64_t n_particles,
+                              const double* trace, const afm_cfg* cfg,
+                              const double* z0v0, double* misfit,
+                              void* cuda_stream);
+
 /* ---- inverse problem by PSO (Eq. 8) -------------
  * One independent swarm per trace.  Philox4x32-10 random numbers, key =
  * seed, counter = (particle, iteration, purpose) (reading R11), so

@@ -22,8 +22,8 @@ OK, EINVAL, ECUDA, EUNSUPPORTED = 0, -1, -2, -3
 
 # every symbol include/afm.h declares (tests check the library exports them all)
 SYMBOLS = (
-    "afm_forward_batch", "afm_forward_batch_host", "afm_pso_invert",
-    "afm_pso_invert_host", "afm_pso_step", "afm_pso_step_host", "afm_pso_init",
+    "afm_forward_batch", "afm_forward_batch_host", "afm_forward_batch_noalloc",
+    "afm_pso_invert", "afm_pso_invert_host", "afm_pso_step", "afm_pso_step_host", "afm_pso_init",
     "afm_kernel_times",
     "afm_pso_shard_init", "afm_pso_shard_eval", "afm_pso_shard_move",
     "afm_beam_modes", "afm_beam_forward_batch", "afm_beam_pso_invert",
@@ -105,6 +105,8 @@ def lib():
         vp, dp, i32, i64, u64 = C.c_void_p, C.c_void_p, C.c_int32, C.c_int64, C.c_uint64
         L.afm_forward_batch.argtypes = [dp, i64, dp, C.POINTER(Cfg), dp, dp, vp]
         L.afm_forward_batch_host.argtypes = [dp, i64, dp, C.POINTER(Cfg), dp, dp, vp]
+        L.afm_forward_batch_noalloc.argtypes = [dp, i64, dp, C.POINTER(Cfg), dp, dp, vp]
+        L.afm_forward_batch_noalloc.restype = C.c_int
         L.afm_pso_invert.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), u64, dp,
                                      C.POINTER(Cfg), dp, dp, dp, dp,
                                      C.POINTER(i32), vp]
@@ -258,6 +260,42 @@ def afm_forward_batch(params, trace, cfg, z0v0=None, misfit=None, stream=None):
         misfit = _dev_f64(misfit, "misfit")
     _check(lib().afm_forward_batch(_ptr(params), P, _ptr(trace), C.byref(cfg),
                                    _ptr(z0v0), _ptr(misfit), _stream_ptr(stream)))
+    return misfit
+
+
+# Rows (one per trace and RK4 step) of the scratch array built into the library
+# for afm_forward_batch_noalloc: AFM_NOALLOC_MAX_ROWS of include/afm.h.
+NOALLOC_MAX_ROWS = 131072
+
+
+def afm_forward_batch_noalloc(params, trace, cfg, misfit, z0v0=None, stream=None):
+    """afm_forward_batch for callers that must not let the library allocate device
+    memory (an instrument's acquisition loop that cannot absorb the stall of a
+    cudaMalloc/cudaFree; a process whose device memory is owned by another pool).
+    The library's only scratch sits in a 4 MiB array inside its own device image,
+    so cfg.n_traces * cfg.n_steps may not exceed NOALLOC_MAX_ROWS (AfmError
+    otherwise).  All tensors, `misfit` included, are the caller's: nothing is
+    created here.  Make the first call on each device at start-up (it looks up the
+    array's device address); calls must not overlap on the GPU, they share the
+    array.  See include/afm.h."""
+    params = _dev_f64(params, "params")
+    trace = _dev_f64(trace, "trace")
+    misfit = _dev_f64(misfit, "misfit")
+    P = params.shape[0]
+    if params.numel() != P * max(cfg.n_params, 0) and cfg.n_params > 0:
+        raise ValueError("params must be [P][D]")
+    if trace.numel() != cfg.n_traces * cfg.n_window:
+        raise ValueError("trace must hold n_traces * W = %d samples"
+                         % (cfg.n_traces * cfg.n_window))
+    if misfit.numel() != P:
+        raise ValueError("misfit must be [P]")
+    if z0v0 is not None:
+        z0v0 = _dev_f64(z0v0, "z0v0")
+        if z0v0.numel() != 2 * P:
+            raise ValueError("z0v0 must be [P][2]")
+    _check(lib().afm_forward_batch_noalloc(_ptr(params), P, _ptr(trace), C.byref(cfg),
+                                           _ptr(z0v0), _ptr(misfit),
+                                           _stream_ptr(stream)))
     return misfit
 
 

@@ -1624,3 +1624,112 @@ void afm_shutdown(void) {
 }
 
 }  // extern "C"
+
+// =================================================================================
+// afm_forward_batch_noalloc (include/afm.h): the forward batch for callers that
+// cannot let the library allocate -- a microscope's acquisition loop, where a
+// cudaMalloc / cudaFree (driver-wide lock, possible device-wide wait, no bound on
+// its duration) in the middle of a scan line breaks the timing, or a process whose
+// device memory already belongs to another component's pool.  Everything above
+// takes its scratch from the grow-only workspace g_ws; this call takes its one
+// piece of scratch, the time-tile stream, from an array that is part of the
+// library's device image, and touches neither g_ws nor any event.
+// =================================================================================
+namespace {
+
+// The time-tile stream of one call: [n_traces][N] rows of 32 bytes (FP64 kernel:
+// double4; FP32 kernel: float4 in the first half).  4 MiB on every device that
+// loads this library, until the process exits.
+constexpr int64_t kNoallocRowBytes = 32;
+static __device__ __align__(256) unsigned char
+    g_noalloc_stream[(size_t)AFM_NOALLOC_MAX_ROWS * kNoallocRowBytes];
+
+// In host code the name g_noalloc_stream is only the handle the runtime registered
+// for the array -- host memory, not where the array lives on the GPU.  A kernel
+// handed &g_noalloc_stream[0] would fault, or on a system where the GPU can read
+// host memory quietly work on the wrong bytes.  The real address differs per
+// device and comes from cudaGetSymbolAddress with that device current; it is
+// looked up on the first call on each device and kept.
+constexpr int kNoallocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+void* g_noalloc_dev_ptr[kNoallocMaxDevices] = {};
+
+int noalloc_stream_address(void** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess)
+    return fail(AFM_ECUDA, "no CUDA device: %s", cudaGetErrorString(e));
+  if (dev < 0 || dev >= kNoallocMaxDevices)
+    return fail(AFM_EUNSUPPORTED, "afm_forward_batch_noalloc: device ordinal %d is "
+                                  "beyond the %d this call keeps addresses for",
+                dev, kNoallocMaxDevices);
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (g_noalloc_dev_ptr[dev] == nullptr) {
+    int major = 0;
+    CUDA_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10)
+      return fail(AFM_EUNSUPPORTED,
+                  "device %d has compute capability %d.x; this library is built for "
+                  "sm_100a only", dev, major);
+    void* p = nullptr;
+    CUDA_TRY(cudaGetSymbolAddress(&p, g_noalloc_stream));
+    if (p == nullptr)
+      return fail(AFM_ECUDA, "cudaGetSymbolAddress returned a null address for the "
+                             "built-in scratch array on device %d", dev);
+    g_noalloc_dev_ptr[dev] = p;
+  }
+  *out = g_noalloc_dev_ptr[dev];
+  return AFM_OK;
+}
+
+}  // namespace
+
+extern "C" int afm_forward_batch_noalloc(const double* params, int64_t n_particles,
+                                         const double* trace, const afm_cfg* cfg,
+                                         const double* z0v0, double* misfit,
+                                         void* cuda_stream) {
+  int rc = validate_forward(params, n_particles, trace, cfg, misfit);
+  if (rc) return rc;
+  const int64_t rows =
+      (int64_t)cfg->n_traces * cfg->steps_per_cycle * cfg->n_cycles;
+  if (rows > (int64_t)AFM_NOALLOC_MAX_ROWS)
+    return fail(AFM_EINVAL,
+                "afm_forward_batch_noalloc: n_traces * steps_per_cycle * n_cycles = "
+                "%d * %d * %d = %lld rows of the time-tile stream, the built-in "
+                "scratch holds %d (4 MiB); use afm_forward_batch for this size",
+                cfg->n_traces, cfg->steps_per_cycle, cfg->n_cycles, (long long)rows,
+                (int)AFM_NOALLOC_MAX_ROWS);
+  void* scratch = nullptr;
+  if ((rc = noalloc_stream_address(&scratch))) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const bool f32 = (cfg->precision == AFM_F32);
+  const int block = block_threads();
+  const int ppt = particles_per_thread();
+  ModelConsts mc;
+  ModelConstsF32 mf;
+  make_consts(cfg, block, &mc);
+  make_consts_f32(cfg, &mf);
+  // Nothing in the array has to start at zero: the kernel below reads rows
+  // [0, n_traces * N) only, and build_stream writes every one of them first, on
+  // the same stream.  Whatever an earlier, longer call left behind is never read.
+  if (f32)
+    LAUNCHED(launch_build_stream_f32(mf, trace, cfg->n_traces, (float*)scratch, st));
+  else
+    LAUNCHED(launch_build_stream(mc, trace, cfg->n_traces, (double*)scratch, st));
+  IntegrateIO io;
+  memset(&io, 0, sizeof(io));
+  io.params = params;
+  io.z0v0 = z0v0;
+  io.stream = (const double*)scratch;
+  io.J = misfit;
+  io.per = n_particles / cfg->n_traces;
+  io.n_traces = cfg->n_traces;
+  io.mode = 0;
+  io.lanes = pick_lanes(cfg, io.per, cfg->n_traces);
+  if (f32)
+    LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
+  else
+    LAUNCHED(launch_integrate_f64(mc, io, block,
+                                  pick_variant(io.per, io.n_traces, ppt), st));
+  return AFM_OK;
+}
