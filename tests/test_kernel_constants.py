@@ -10,7 +10,9 @@ of the range reduction must add up to ln 2.
 import os
 import re
 
-import mpmath as mp
+import pytest
+
+mp = pytest.importorskip("mpmath")   # a box without mpmath skips this file, the rest still collects
 
 SRC = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))),
                    "paper_1109_0334_b200", "csrc", "afm_device.cuh")
