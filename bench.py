@@ -303,6 +303,7 @@ def run_ours(args):
     barrier()
     launches = afm.afm_launch_count()
     kernel_times = afm.afm_kernel_times(min(args.steps, 64))
+    kernel_name = afm.afm_last_integrate_kernel()   # which form the library chose to run
     afm.afm_set_option("kernel_events", 0)
     step_ms = [e[0].elapsed_time(e[2]) for e in ev]
     fwd_ms = [e[0].elapsed_time(e[1]) for e in ev]
@@ -372,13 +373,15 @@ def run_ours(args):
             "clocks": clocks,
             "forward_ms": fwd_total_ms / args.steps,
             "roofline": {"bound": "alu",
-                         "kernel": "integrate_misfit_%s_q" % args.precision,
+                         "kernel": kernel_name,
                          "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                          "frac": achieved / peak,
                          "kernel_ms": kern_ms,
                          "kernel_ms_source": "CUDA events recorded by the library around "
-                                             "each integrate launch on its stream, mean of "
-                                             "%d timed launches" % len(kernel_times),
+                                             "each launch of that kernel alone (the queue "
+                                             "reset kernel comes before the start event) on "
+                                             "its stream, mean of %d timed launches"
+                                             % len(kernel_times),
                          "flops_per_particle_step": FLOPS_PER_STEP[wl["law"]],
                          "algorithmic_bytes": int(P * (8 * D + 16 + 8) + N * 32),
                          "traffic": ncu["traffic"],

@@ -406,6 +406,24 @@ int afm_fma_peak(int32_t precision, double seconds, double* tflops,
  * the option on or off resets the record. */
 int afm_kernel_times(double* ms, int32_t max_n, int32_t* n_out);
 
+/* Health of the segment-queue kernels (option "queue").  A queue worker that
+ * waits about 20 s for a task gives up, which only a corrupted queue can cause;
+ * the chains it would have run keep whatever their output slots held before.
+ * The synchronous calls check for this themselves and return AFM_ECUDA.  The
+ * asynchronous device-pointer calls (afm_forward_batch, afm_beam_forward_batch,
+ * afm_pso_shard_eval) cannot: call this after them, before trusting their
+ * outputs.  Waits for cuda_stream, then returns AFM_OK, or AFM_ECUDA if a worker
+ * has given up since the last check (the flag is cleared by the check). */
+int afm_queue_status(void* cuda_stream);
+
+/* Name of the integrate kernel that the most recent compute call on the calling
+ * thread launched: "integrate_misfit_f64", "integrate_misfit_f64_q" (segment
+ * queue), "integrate_misfit_f32", "integrate_misfit_f32_q", "beam_integrate_f64",
+ * "beam_integrate_f64_q", or "" before the first one.  The event pairs of
+ * afm_kernel_times bracket exactly that kernel (the queue's reset kernel is
+ * launched before the start event).  Static storage; never NULL. */
+const char* afm_last_integrate_kernel(void);
+
 /* Kernel launches enqueued by this library on the calling thread since the
  * last reset (bench.py's gpu_launches). */
 int64_t afm_launch_count(void);

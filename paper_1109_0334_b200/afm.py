@@ -24,7 +24,7 @@ OK, EINVAL, ECUDA, EUNSUPPORTED = 0, -1, -2, -3
 SYMBOLS = (
     "afm_forward_batch", "afm_forward_batch_host", "afm_forward_batch_noalloc",
     "afm_pso_invert", "afm_pso_invert_host", "afm_pso_step", "afm_pso_step_host", "afm_pso_init",
-    "afm_kernel_times",
+    "afm_kernel_times", "afm_queue_status", "afm_last_integrate_kernel",
     "afm_pso_shard_init", "afm_pso_shard_eval", "afm_pso_shard_move",
     "afm_beam_modes", "afm_beam_forward_batch", "afm_beam_pso_invert",
     "afm_beam_trajectory", "afm_philox4x32_10", "afm_trajectory", "afm_fma_peak",
@@ -119,6 +119,10 @@ def lib():
         L.afm_pso_step_host.restype = C.c_int
         L.afm_kernel_times.argtypes = [C.POINTER(C.c_double), i32, C.POINTER(i32)]
         L.afm_kernel_times.restype = C.c_int
+        L.afm_last_integrate_kernel.argtypes = []
+        L.afm_last_integrate_kernel.restype = C.c_char_p
+        L.afm_queue_status.argtypes = [vp]
+        L.afm_queue_status.restype = C.c_int
         L.afm_pso_init.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), i32, i32,
                                    u64, dp, dp, dp, dp, dp, dp, vp]
         L.afm_pso_shard_init.argtypes = [C.POINTER(Bounds), C.POINTER(SwarmCfg), i32,
@@ -403,6 +407,19 @@ def afm_pso_step_host(bounds, swarm, n_dims, n_traces, seed, iteration, do_move,
                                    _hptr(st["pbestJ"]), _hptr(st["gbest"]),
                                    _hptr(st["gbestJ"]), _stream_ptr(stream)))
     return st
+
+
+def afm_queue_status(stream=None):
+    """Waits for `stream` and raises AfmError if a segment-queue worker has given up
+    since the last check: call it after the asynchronous device-tensor calls
+    (afm_forward_batch, afm_beam_forward_batch, afm_pso_shard_eval) before trusting
+    their outputs."""
+    _check(lib().afm_queue_status(_stream_ptr(stream)))
+
+
+def afm_last_integrate_kernel():
+    """Name of the integrate kernel the last compute call of this thread launched."""
+    return lib().afm_last_integrate_kernel().decode()
 
 
 def afm_kernel_times(max_n=64):

@@ -21,6 +21,7 @@ using namespace afm;
 
 thread_local char g_err[512] = "";
 thread_local int64_t g_launches = 0;
+thread_local const char* g_last_kernel = "";  // afm_last_integrate_kernel()
 
 int fail(int code, const char* fmt, ...) {
   va_list ap;
@@ -417,13 +418,19 @@ int queue_per_sub(int64_t per, int n_traces, int64_t n_steps, bool eligible,
   return per_sub;
 }
 
+// per_sub_decided >= 0: the caller has already asked queue_per_sub (with the true
+// step count, before it chose the tile length) and this call must not decide again
+// from the tile-rounded count n_tiles * T, which can differ just below the threshold.
 int make_queue(int64_t per, int n_traces, int n_tiles, int T, bool eligible,
                SegQueue* q, int* workers, bool* use, cudaStream_t st,
-               int ckpt_doubles = 4, int max_chains_per_sub = 0) {
+               int ckpt_doubles = 4, int max_chains_per_sub = 0,
+               int per_sub_decided = -1) {
   const int64_t chains = (int64_t)blocks_per_trace(per, 32) * n_traces;
   const int64_t subparts = (int64_t)4 * g_n_sm;
   const int per_sub =
-      queue_per_sub(per, n_traces, (int64_t)n_tiles * T, eligible, max_chains_per_sub);
+      per_sub_decided >= 0
+          ? per_sub_decided
+          : queue_per_sub(per, n_traces, (int64_t)n_tiles * T, eligible, max_chains_per_sub);
   *use = per_sub > 0;
   if (!*use) return AFM_OK;
   *workers = (int)(per_sub * subparts);
@@ -495,14 +502,17 @@ int run_integrate_f64(const ModelConsts& mc_in, const IntegrateIO& io, int block
     }
   }
   int rc = make_queue(io.per, io.n_traces, mc.n_tiles, mc.T, eligible, &q, &workers,
-                      &use_q, st);
+                      &use_q, st, 4, 0, per_sub);
   if (rc) return rc;
   if (!use_q) mc = mc_in;
+  // the queue is reset before the start event: the pair brackets one kernel
+  if (use_q) LAUNCHED(launch_segq_init(q, st));
   if ((rc = kev_record(0, st))) return rc;
   if (use_q)
     LAUNCHED(launch_integrate_f64_q(mc, io, q, workers, st));
   else
     LAUNCHED(launch_integrate_f64(mc, io, block, variant, st));
+  g_last_kernel = use_q ? "integrate_misfit_f64_q" : "integrate_misfit_f64";
   return kev_record(1, st);
 }
 
@@ -514,11 +524,13 @@ int run_integrate_f32(const ModelConstsF32& mf, const IntegrateIO& io, int block
   int rc = make_queue(io.per, io.n_traces, mf.n_tiles, mf.T, ppt == 1 && block == 32, &q,
                       &workers, &use_q, st);
   if (rc) return rc;
+  if (use_q) LAUNCHED(launch_segq_init(q, st));
   if ((rc = kev_record(0, st))) return rc;
   if (use_q)
     LAUNCHED(launch_integrate_f32_q(mf, io, q, workers, st));
   else
     LAUNCHED(launch_integrate_f32(mf, io, block, ppt, st));
+  g_last_kernel = use_q ? "integrate_misfit_f32_q" : "integrate_misfit_f32";
   return kev_record(1, st);
 }
 
@@ -720,23 +732,13 @@ int afm_pso_init(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
                             pbest, pbestJ, gbest, gbestJ, cuda_stream);
 }
 
-int afm_pso_step(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
-                 int32_t n_dims, int32_t n_traces, uint64_t seed,
-                 int32_t iteration, int32_t do_move, const double* J, double* x,
-                 double* v, double* pbest, double* pbestJ, double* gbest,
-                 double* gbestJ, void* cuda_stream) {
-  if (n_dims < 1 || n_dims > 4) return fail(AFM_EINVAL, "n_dims must be 1..4");
-  if (n_traces < 1) return fail(AFM_EINVAL, "n_traces must be >= 1");
-  if (iteration < 0) return fail(AFM_EINVAL, "iteration must be >= 0");
-  int rc = validate_bounds(bounds, n_dims);
-  if (rc) return rc;
-  if ((rc = validate_swarm(swarm))) return rc;
-  if ((rc = reject_async(swarm, "afm_pso_step"))) return rc;
-  if (!J || !x || !v || !pbest || !pbestJ || !gbest || !gbestJ)
-    return fail(AFM_EINVAL, "NULL swarm array");
-  if ((rc = check_device())) return rc;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  std::lock_guard<std::mutex> lock(g_ws.mu);
+// afm_pso_step on device arrays, arguments validated, workspace lock held.
+static int pso_step_locked(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                           int32_t n_dims, int32_t n_traces, uint64_t seed,
+                           int32_t iteration, int32_t do_move, const double* J,
+                           double* x, double* v, double* pbest, double* pbestJ,
+                           double* gbest, double* gbestJ, cudaStream_t st) {
+  int rc;
   const int64_t per = swarm->n_particles;
   const int block = 128;
   const int bpt = blocks_per_trace(per, block);
@@ -754,6 +756,37 @@ int afm_pso_step(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
                              (uint32_t)iteration, 1, RingEdges{0, 0, nullptr, nullptr, 0}, J, x, v, pbest,
                              pbestJ, gbest, nullptr, st));
   return release_ws(st);
+}
+
+static int validate_pso_step(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                             int32_t n_dims, int32_t n_traces, int32_t iteration,
+                             const double* J, const double* x, const double* v,
+                             const double* pbest, const double* pbestJ,
+                             const double* gbest, const double* gbestJ) {
+  if (n_dims < 1 || n_dims > 4) return fail(AFM_EINVAL, "n_dims must be 1..4");
+  if (n_traces < 1) return fail(AFM_EINVAL, "n_traces must be >= 1");
+  if (iteration < 0) return fail(AFM_EINVAL, "iteration must be >= 0");
+  int rc = validate_bounds(bounds, n_dims);
+  if (rc) return rc;
+  if ((rc = validate_swarm(swarm))) return rc;
+  if ((rc = reject_async(swarm, "afm_pso_step"))) return rc;
+  if (!J || !x || !v || !pbest || !pbestJ || !gbest || !gbestJ)
+    return fail(AFM_EINVAL, "NULL swarm array");
+  return AFM_OK;
+}
+
+int afm_pso_step(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
+                 int32_t n_dims, int32_t n_traces, uint64_t seed,
+                 int32_t iteration, int32_t do_move, const double* J, double* x,
+                 double* v, double* pbest, double* pbestJ, double* gbest,
+                 double* gbestJ, void* cuda_stream) {
+  int rc = validate_pso_step(bounds, swarm, n_dims, n_traces, iteration, J, x, v, pbest,
+                             pbestJ, gbest, gbestJ);
+  if (rc) return rc;
+  if ((rc = check_device())) return rc;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  return pso_step_locked(bounds, swarm, n_dims, n_traces, seed, iteration, do_move, J, x,
+                         v, pbest, pbestJ, gbest, gbestJ, (cudaStream_t)cuda_stream);
 }
 
 static int pso_invert_locked(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
@@ -1182,6 +1215,7 @@ static int run_beam_integrate(const BeamConsts& bc, const BeamModeConsts& mo,
     LAUNCHED(launch_beam_integrate_q(bc, mo, io, q, workers, st));
   else
     LAUNCHED(launch_beam_integrate(bc, mo, io, block, st));
+  g_last_kernel = use_q ? "beam_integrate_f64_q" : "beam_integrate_f64";
   return AFM_OK;
 }
 
@@ -1344,6 +1378,7 @@ int afm_beam_pso_invert(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
                            cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaMemcpyAsync(J_star, Js_dev, (size_t)T * 8, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
+  if ((rc = check_queue_flag(st))) return rc;  // run_beam_integrate may use the queue
   if (n_iters_done) *n_iters_done = done;
   return release_ws(st);
 }
@@ -1472,27 +1507,23 @@ int afm_pso_step_host(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
                       int32_t iteration, int32_t do_move, const double* J, double* x,
                       double* v, double* pbest, double* pbestJ, double* gbest,
                       double* gbestJ, void* cuda_stream) {
-  if (n_dims < 1 || n_dims > 4) return fail(AFM_EINVAL, "n_dims must be 1..4");
-  if (n_traces < 1) return fail(AFM_EINVAL, "n_traces must be >= 1");
-  int rc = validate_swarm(swarm);
+  int rc = validate_pso_step(bounds, swarm, n_dims, n_traces, iteration, J, x, v, pbest,
+                             pbestJ, gbest, gbestJ);
   if (rc) return rc;
-  if (!J || !x || !v || !pbest || !pbestJ || !gbest || !gbestJ)
-    return fail(AFM_EINVAL, "NULL swarm array");
   if ((rc = check_device())) return rc;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t PT = (size_t)swarm->n_particles * n_traces;
   const size_t nd = PT * n_dims, nt = (size_t)n_traces;
   // device image: J, x, v, pbest, pbestJ, gbest, gbestJ
   const size_t total = PT + 3 * nd + PT + nt * n_dims + nt;
-  double* base;
-  {
-    std::lock_guard<std::mutex> lock(g_ws.mu);
-    if ((rc = acquire_ws(st))) return rc;
-    if (g_ws.h_state.ensure(total * 8))
-      return fail(AFM_ECUDA, "cudaMalloc of the swarm staging buffer failed");
-    base = (double*)g_ws.h_state.p;
-    g_ws.last_stream = st;
-  }
+  // One lock over staging, step, copy-back and synchronisation: another thread
+  // that needs a larger h_state would otherwise free it under the copies in flight.
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  if ((rc = acquire_ws(st))) return rc;
+  if (g_ws.h_state.ensure(total * 8))
+    return fail(AFM_ECUDA, "cudaMalloc of the swarm staging buffer failed");
+  double* base = (double*)g_ws.h_state.p;
+  g_ws.last_stream = st;  // same stream: no self-wait
   double* dJ = base;
   double* dx = dJ + PT;
   double* dv = dx + nd;
@@ -1505,17 +1536,28 @@ int afm_pso_step_host(const afm_bounds* bounds, const afm_swarm_cfg* swarm,
       {dpbJ, pbestJ, PT}, {dg, gbest, nt * n_dims}, {dgJ, gbestJ, nt}};
   for (const auto& c : in)
     CUDA_TRY(cudaMemcpyAsync(c.d, c.h, c.n * 8, cudaMemcpyHostToDevice, st));
-  rc = afm_pso_step(bounds, swarm, n_dims, n_traces, seed, iteration, do_move, dJ, dx, dv,
-                    dpb, dpbJ, dg, dgJ, cuda_stream);
+  rc = pso_step_locked(bounds, swarm, n_dims, n_traces, seed, iteration, do_move, dJ, dx,
+                       dv, dpb, dpbJ, dg, dgJ, st);
   if (rc) return rc;
   const struct { double* h; const double* d; size_t n; } out[] = {
       {x, dx, nd}, {v, dv, nd}, {pbest, dpb, nd}, {pbestJ, dpbJ, PT},
       {gbest, dg, nt * n_dims}, {gbestJ, dgJ, nt}};
   for (const auto& c : out)
     CUDA_TRY(cudaMemcpyAsync(c.h, c.d, c.n * 8, cudaMemcpyDeviceToHost, st));
+  if ((rc = release_ws(st))) return rc;  // after the last read of h_state
   CUDA_TRY(cudaStreamSynchronize(st));
   return AFM_OK;
 }
+
+int afm_queue_status(void* cuda_stream) {
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  if (!g_ws.segq.p) return AFM_OK;  // no queue kernel has run: nothing to wait for
+  CUDA_TRY(cudaStreamSynchronize(st));
+  return check_queue_flag(st);
+}
+
+const char* afm_last_integrate_kernel(void) { return g_last_kernel; }
 
 int64_t afm_launch_count(void) { return g_launches; }
 void afm_reset_launch_count(void) { g_launches = 0; }
@@ -1731,5 +1773,6 @@ extern "C" int afm_forward_batch_noalloc(const double* params, int64_t n_particl
   else
     LAUNCHED(launch_integrate_f64(mc, io, block,
                                   pick_variant(io.per, io.n_traces, ppt), st));
+  g_last_kernel = f32 ? "integrate_misfit_f32" : "integrate_misfit_f64";
   return AFM_OK;
 }

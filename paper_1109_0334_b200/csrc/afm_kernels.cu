@@ -916,13 +916,13 @@ static int launch_integrate_q_t(const ModelConsts& mc, const IntegrateIO& io,
   auto kern = integrate_misfit_f64_q<LAW, MODE>;
   if (smem > 48 * 1024)
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  launch_segq_init(q, st);
   kern<<<(unsigned)workers, 32, smem, st>>>(mc, io, bpt, q);
-  return 2;
+  return 1;
 }
 
 // Segment-queue form of the throughput kernel (one warp per CTA, `workers`
 // persistent CTAs); q.n_chains must be blocks_per_trace(io.per, 32) * n_traces.
+// The caller resets the queue first (launch_segq_init on the same stream).
 int launch_integrate_f64_q(const ModelConsts& mc, const IntegrateIO& io,
                            const SegQueue& q, int workers, cudaStream_t st) {
 #define AFM_DISPATCH_Q(LAWV)                                                   \

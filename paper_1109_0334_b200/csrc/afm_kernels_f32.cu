@@ -519,9 +519,8 @@ static int launch_integrate32_q_t(const ModelConstsF32& mf, const IntegrateIO& i
   auto kern = integrate_misfit_f32_q<LAW, MODE>;
   if (smem > 48 * 1024)
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  launch_segq_init(q, st);
-  kern<<<(unsigned)workers, 32, smem, st>>>(mf, io, bpt, q);
-  return 2;
+  kern<<<(unsigned)workers, 32, smem, st>>>(mf, io, bpt, q);  // queue reset by the caller
+  return 1;
 }
 
 int launch_integrate_f32_q(const ModelConstsF32& mf, const IntegrateIO& io,

@@ -57,6 +57,10 @@ class CudaBackend:
                                            do_move, first, gathered, st, rank=rank,
                                            swarm_particles=swarm_particles)
 
+    def status(self):
+        """Raises if a segment-queue kernel of this run lost a chain (afm_queue_status)."""
+        self.afm.afm_queue_status()
+
 
 class ShardedSwarm:
     """PSO inversion of `trace` with the swarm sharded over `group`.
@@ -166,6 +170,8 @@ class ShardedSwarm:
         import torch
         for it in range(self.n_iters):
             self.step(do_move=(it + 1 < self.n_iters))
+        if hasattr(self.backend, "status"):
+            self.backend.status()   # the shard calls are asynchronous: check once, at the end
         th, Js = self.state["theta_star"], self.state["J_star"]
         if self.shard == "traces" and self.world > 1:
             # once, outside the loop: collect every rank's pixels

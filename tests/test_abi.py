@@ -122,6 +122,27 @@ def test_product_package_never_imports_the_oracle():
                     assert not pat.search(text), (f, pat.search(text).group(0))
 
 
+def test_queue_status_is_ok_before_any_queue_kernel_has_run(lib):
+    """afm_queue_status has nothing to wait for, and makes no CUDA call, until a
+    segment-queue kernel has been launched (this runs on a box with no GPU)."""
+    assert lib.afm_queue_status(None) == afm.OK
+
+
+def test_pso_step_host_validates_like_pso_step(lib):
+    """The host-buffer step checks bounds and iteration up front (it used to leave
+    that to the device-buffer call, after staging)."""
+    w0 = wlm.config(0)
+    b, sw = afm.bounds_from(w0), afm.swarm_from(w0)
+    p16 = C.c_void_p(16)
+    args = lambda bb, it: (C.byref(bb), C.byref(sw), 2, 1, 0, it, 1, p16, p16, p16, p16,
+                           p16, p16, p16, None)
+    assert lib.afm_pso_step_host(*args(b, -1)) == afm.EINVAL
+    bad = afm.bounds_from(w0)
+    bad.lo[0], bad.hi[0] = 2.0, 1.0
+    assert lib.afm_pso_step_host(*args(bad, 0)) == afm.EINVAL
+    assert lib.afm_pso_step(*args(bad, 0)) == afm.EINVAL
+
+
 def test_new_entry_points_validate_before_touching_the_device(lib):
     """Beam model, sharded swarm, probes, options: bad arguments are AFM_EINVAL
     without any CUDA call (this runs on a box with no GPU)."""

@@ -329,6 +329,7 @@ def test_segment_queue_changes_no_result(afm, cfg_i, segs, workers, boost, preci
         afm.afm_set_option("form", 1)           # the queue serves the throughput form
         try:
             out[queue] = _gpu_forward(afm, wl, params, trace, z0v0, precision=precision)
+            afm.afm_queue_status()              # no worker gave up (raises otherwise)
             g = afm.afm_pso_invert(afm.bounds_from(wp), afm.swarm_from(wp), 3,
                                    torch.as_tensor(trace, device="cuda"),
                                    afm.cfg_from(wp, precision=precision), dump=True)
