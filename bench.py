@@ -53,9 +53,10 @@ FLOPS_PER_STEP = {wlm.LAW_DMT: 57.0, wlm.LAW_DMT_VISC: 57.0, wlm.LAW_LJ_EXP: 93.
 # FP64 FMA peak of the lane model: 148 SMs x 64 lanes x 2 flops x clock
 N_SM, FP64_LANES, FP32_LANES = 148, 64, 128
 # ncu figures of the dominant kernel (DRAM traffic per launch, pipe utilisation) are
-# read from the machine-written summary profiles/<PROFILE>_ncu.csv
-# (python -m paper_1109_0334_b200.ncu_summary) and reported only while the library
-# source is the one that summary was made from; otherwise they are null.
+# read from the machine-written summary profiles/<PROFILE>_ncu.csv (key,value rows
+# taken from `ncu -i <report> --page raw --csv`, with the hash of the library source
+# the report belongs to) and reported only while the library source is the one that
+# summary was made from; otherwise they are null.
 PROFILE = {"f64": "r2_cfg1_f64", "f32": "r2_cfg1_f32"}
 PIPE_METRIC = {"f64": "sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_",
                "f32": "sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_"}
@@ -65,7 +66,7 @@ def _ncu_profile(precision):
     """dict(traffic, pipe_active_pct, pipe_elapsed_pct, ...) from the committed ncu
     summary of this precision's integrate kernel, or the reason it is not usable."""
     import csv
-    from paper_1109_0334_b200 import ncu_summary
+    from paper_1109_0334_b200 import build as afm_build
     path = os.path.join(ROOT, "profiles", PROFILE[precision] + "_ncu.csv")
     out = {"file": os.path.relpath(path, ROOT), "traffic": None, "pipe_active_pct": None,
            "pipe_elapsed_pct": None}
@@ -75,7 +76,7 @@ def _ncu_profile(precision):
     kv = dict((r[0], r[1]) for r in csv.reader(open(path)) if len(r) == 2)
     out["kernel"] = kv.get("kernel", "").split("(")[0]
     out["registers_per_thread"] = kv.get("launch__registers_per_thread")
-    sha = ncu_summary.source_sha()
+    sha = afm_build.source_sha()
     if kv.get("source_sha") != sha:
         out["status"] = "stale: summary made from source %s, running %s" % (
             kv.get("source_sha"), sha)

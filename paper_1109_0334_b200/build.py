@@ -7,6 +7,7 @@ nvcc cross-compiles for sm_100a only (no GPU needed to build).  The output
 sits next to this file so that it travels with the source tree; it is
 git-ignored.
 """
+import hashlib
 import os
 import subprocess
 import sys
@@ -26,6 +27,19 @@ NVCC_FLAGS = [
     "--cudart", "static",
     "-shared",
 ]
+
+
+def source_sha():
+    """Hash of the library source (csrc/* and include/afm.h, in sorted file order).
+    bench.py reports ncu-derived figures from profiles/ only while this equals the
+    hash recorded in the summary they come from."""
+    h = hashlib.sha256()
+    files = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC))
+    files.append(os.path.join(ROOT, "include", "afm.h"))
+    for f in files:
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
 
 
 def _nvcc():
