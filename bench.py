@@ -433,12 +433,15 @@ def _targets(out, ncu, precision):
         v = by[p]["pipe_active_pct"]
         return {"pipe_active_pct": v, "pipe_elapsed_pct": by[p]["pipe_elapsed_pct"],
                 "bar_pct": bar, "met": None if v is None else bool(v >= bar),
-                "source": by[p]["file"], "status": by[p]["status"]}
+                "source": "builder capture: ncu summary %s committed by the builder, not "
+                          "measured by this run" % by[p]["file"],
+                "status": by[p]["status"]}
     ms = ex.get("cfg2_inversion_ms")
     return {"fp64_pipe_ge_60pct_configs1": pipe("f64", 60.0),
             "fp32_pipe_ge_50pct_configs1": pipe("f32", 50.0),
             "configs2_inversion_lt_100ms": {"ms": ms, "met": None if ms is None
-                                            else bool(ms < 100.0)}}
+                                            else bool(ms < 100.0),
+                                            "source": "this run (extras.cfg2_inversion_ms)"}}
 
 
 def _event_ms(torch, fn, reps):
@@ -499,11 +502,35 @@ def extras(afm, torch, dev, main_prec):
     tr = trace_of(wl)
     out = torch.empty(P, dtype=torch.float64, device=dev)
     cfg = afm.cfg_from(wl, precision=other)
+    afm.afm_set_option("kernel_events", 1)
     ms = _event_ms(torch, lambda: afm.afm_forward_batch(params, tr, cfg, z0v0=z0v0,
                                                         misfit=out), 3)
+    kt = afm.afm_kernel_times(3)          # the 3 timed launches, the kernel alone
+    kname = afm.afm_last_integrate_kernel()
+    afm.afm_set_option("kernel_events", 0)
     name = "f64" if other == afm.F64 else "f32"
     ex["cfg1_%s_forward_ms" % name] = ms
     ex["cfg1_%s_particle_steps_per_s" % name] = P * wl["n_steps"] / (ms * 1e-3)
+    # the roofline block of the other precision, built like the headline's
+    pk = _peaks()
+    kms = float(np.mean(kt))
+    ach = FLOPS_PER_STEP[wl["law"]] * P * wl["n_steps"] / (kms * 1e-3) / 1e12
+    peak = pk["fp64_tflops"] if other == afm.F64 else pk["fp32_tflops"]
+    prof = _ncu_profile(name)
+    ex["roofline_%s" % name] = {
+        "bound": "alu", "kernel": kname, "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+        "frac": ach / peak, "kernel_ms": kms,
+        "kernel_ms_source": "CUDA events recorded by the library around each launch of "
+                            "that kernel alone, mean of %d launches, no L2 flush between "
+                            "them" % len(kt),
+        "flops_per_particle_step": FLOPS_PER_STEP[wl["law"]],
+        "traffic": prof["traffic"],
+        "frac_pipe_active": (None if prof["pipe_active_pct"] is None
+                             else prof["pipe_active_pct"] / 100.0),
+        "frac_pipe_elapsed": (None if prof["pipe_elapsed_pct"] is None
+                              else prof["pipe_elapsed_pct"] / 100.0),
+        "ncu_source": "builder capture %s (%s)" % (prof["file"], prof["status"]),
+        "frac_of_measured": ach / ex["fma_peak_measured_tflops"][name]}
 
     # configs[3] (both precisions) and configs[4]: one full-size forward batch and the
     # full inversion, measured (not extrapolated)
@@ -790,6 +817,55 @@ def run_one_batch(args):
     return 0
 
 
+def run_pso_step(args):
+    """--pso-step CFG: rows a5-a7 of SURVEY.md 8(a) on their own (afm_pso_step:
+    pso_best_kernel, pso_gbest_kernel, pso_move_kernel) on a swarm of configs[CFG]'s
+    size with seeded synthetic misfits, for ncu captures of the PSO kernels and their
+    share of the HBM roofline.  Prints a small JSON line; NOT the bench line."""
+    import torch
+    from paper_1109_0334_b200 import afm
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    wl = wlm.config(args.pso_step)
+    T, per, D = wl["n_traces"], wl["swarm"]["n_particles"], wl["n_params"]
+    P = T * per
+    b, sw = afm.bounds_from(wl), afm.swarm_from(wl)
+    state = afm.afm_pso_init(b, sw, D, T, wl["pso_seed"])
+    g = torch.Generator(device=dev)
+    g.manual_seed(1234)
+    Js = [torch.rand(P, dtype=torch.float64, device=dev, generator=g) for _ in range(4)]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    for i in range(args.warmup):
+        afm.afm_pso_step(b, sw, D, T, wl["pso_seed"], i, True, Js[i % 4], state)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(args.steps)]
+    afm.afm_reset_launch_count()
+    for i in range(args.steps):
+        flush.zero_()
+        ev[i][0].record()
+        afm.afm_pso_step(b, sw, D, T, wl["pso_seed"], args.warmup + i, True, Js[i % 4], state)
+        ev[i][1].record()
+    torch.cuda.synchronize()
+    ms = float(np.mean([a.elapsed_time(z) for a, z in ev]))
+    # no-improvement lower bound: best reads J, pbestJ; move reads x, v, pbest and
+    # writes x, v (a personal best that improves adds 8 D + 8 bytes read/written)
+    algo = 16 * P + 40 * D * P
+    hbm = None
+    try:
+        hbm = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+    except Exception:
+        pass
+    print(json.dumps({"pso_step": args.pso_step, "particles": P, "n_traces": T, "dims": D,
+                      "ms_per_step": ms, "launches_per_step": afm.afm_launch_count() / args.steps,
+                      "algorithmic_bytes_per_step": algo,
+                      "achieved_gbs": algo / (ms * 1e-3) / 1e9,
+                      "hbm_peak_gbs": hbm,
+                      "frac": None if not hbm else algo / (ms * 1e-3) / 1e9 / hbm,
+                      "l2": "256 MB buffer zeroed between timed steps"}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -805,6 +881,8 @@ def main():
     ap.add_argument("--one-batch", type=int, default=None, choices=[0, 1, 2, 3, 4, 7],
                     help="profiling aid: one full-size forward batch of configs[N]; "
                          "7 = the paper's 8-mode beam workload")
+    ap.add_argument("--pso-step", type=int, default=None, choices=[0, 1, 2, 3, 4],
+                    help="profiling aid: afm_pso_step alone on a swarm of configs[N]'s size")
     ap.add_argument("--beam-particles", type=int, default=65536)
     ap.add_argument("--invert", action="store_true",
                     help="with --one-batch: time the full PSO inversion instead")
@@ -820,6 +898,8 @@ def main():
         return run_sharded(args)
     if args.one_batch is not None:
         return run_one_batch(args)
+    if args.pso_step is not None:
+        return run_pso_step(args)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     return run_reference(args) if args.impl == "reference" else run_ours(args)

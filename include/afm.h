@@ -431,7 +431,8 @@ void afm_reset_launch_count(void);
 
 /* Tuning knobs (optional).  name: "block" (threads per CTA of the integrate
  * kernel: 32, 64 or 128; 0 = auto), "tile" (steps per time tile; 0 = auto),
- * "ppt" (particles per thread: 1 or 2; 0 = auto), "form" (FP64 kernel form:
+ * "ppt" (particles per thread of the FP32 kernel: 1 or 2; 0 = auto = 1; the FP64
+ * kernels always take one), "form" (FP64 kernel form:
  * 1 = throughput, fewest FP64 instructions; 2 = latency, shortest dependent
  * chains; 0 = auto by warps per SM sub-partition), "lanes" (latency form of the
  * DMT laws: particles per warp, a power of two up to 32; 0 = auto, as many as

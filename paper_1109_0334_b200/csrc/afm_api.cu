@@ -312,15 +312,15 @@ void make_consts_f32(const afm_cfg* c, ModelConstsF32* mf) {
 
 // Launch shape of the integrate kernels: one warp per CTA and one particle per
 // thread unless afm_set_option says otherwise (measured on B200, DESIGN.md 6:
-// 64- and 128-thread CTAs change nothing, two particles per thread cost 28 %).
+// 64- and 128-thread CTAs change nothing; two particles per thread cost the FP64
+// kernel 28 %, so "ppt" now reaches the FP32 kernel only).
 int block_threads() { return g_opt_block > 0 ? g_opt_block : 32; }
 int particles_per_thread() { return g_opt_ppt > 0 ? g_opt_ppt : 1; }
 
 // Kernel form of the FP64 integrate kernel (afm_device.cuh, vdw_plus): the
 // latency form below two warps per SM sub-partition, where nothing hides the
 // dependent chains; the throughput form (fewest FP64 instructions) above.
-int pick_variant(int64_t per, int n_traces, int ppt) {
-  if (ppt == 2) return 2;
+int pick_variant(int64_t per, int n_traces, int /*ppt: FP32 kernel only*/) {
   if (g_opt_form == 1) return 0;
   if (g_opt_form == 2) return 1;
   const int64_t warps = ((per + 31) / 32) * n_traces;
@@ -387,8 +387,9 @@ int pick_lanes(const afm_cfg* cfg, int64_t per, int n_traces) {
 }
 
 // CTAs per trace of the FP64 integrate kernel for a launch decision.
-int integrate_bpt(int64_t per, int block, int ppt, int variant, int lanes) {
-  return variant == 1 ? blocks_per_trace(per, lanes) : blocks_per_trace(per, block * ppt);
+int integrate_bpt(int64_t per, int block, int /*ppt: FP32 kernel only*/, int variant,
+                  int lanes) {
+  return variant == 1 ? blocks_per_trace(per, lanes) : blocks_per_trace(per, block);
 }
 
 // Segment-queue scheduling (integrate_misfit_f64_q / _f32_q): the time loop of every

@@ -875,15 +875,13 @@ static int launch_integrate_t(const ModelConsts& mc, const IntegrateIO& io,
   return 1;
 }
 
-// variant: 0 = throughput form, 1 = latency form (short dependent chains),
-// 2 = two particles per thread (throughput form)
+// variant: 0 = throughput form, 1 = latency form (short dependent chains).
+// (Two particles per thread, PPT = 2, was measured and rejected for FP64 -- 28 %
+// slower on configs[1], DESIGN.md 6 -- and is no longer instantiated.)
 int launch_integrate_f64(const ModelConsts& mc, const IntegrateIO& io, int block,
                          int variant, cudaStream_t st) {
 #define AFM_DISPATCH(LAWV)                                                      \
   case LAWV:                                                                    \
-    if (variant == 2)                                                           \
-      return io.mode ? launch_integrate_t<LAWV, 1, 2, false>(mc, io, block, st) \
-                     : launch_integrate_t<LAWV, 0, 2, false>(mc, io, block, st);\
     if (variant == 1)                                                           \
       return io.mode ? launch_integrate_t<LAWV, 1, 1, true>(mc, io, block, st)  \
                      : launch_integrate_t<LAWV, 0, 1, true>(mc, io, block, st); \
