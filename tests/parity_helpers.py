@@ -2,6 +2,9 @@
 (the oracle plays the paper's 'CPU solver that synthesises the experimental
 trace') and marshal the same workload dict for both sides.
 No arithmetic of the method lives here."""
+import json
+import os
+
 import numpy as np
 
 from oracle import binding as orc
@@ -35,3 +38,21 @@ def rel_err(a, b):
     e = np.where(both_inf, 0.0, e)
     e = np.where((a == b), 0.0, e)
     return e
+
+
+def record_parity(label, precision, e, tol, n_above, n_excused_repo, n_excused_c15):
+    """Append one row of parity statistics to the file named by $AFM_PARITY_STATS
+    (profiles/r3_parity_stats.md is made from such a run); no-op when it is unset.
+    e: relative errors of the sample; n_above: how many are >= tol; n_excused_*: how
+    many of those the repository's R15 rule and SURVEY.md c-15's one-ulp rule excuse."""
+    path = os.environ.get("AFM_PARITY_STATS")
+    if not path:
+        return
+    e = np.asarray(e, dtype=np.float64)
+    fin = e[np.isfinite(e)]
+    row = dict(label=label, precision=precision, n=int(e.size), tol=tol,
+               median=float(np.median(fin)), p99=float(np.percentile(fin, 99)),
+               max=float(fin.max()), above_tol=int(n_above),
+               excused_repo_rule=int(n_excused_repo), excused_c15_one_ulp=int(n_excused_c15))
+    with open(path, "a") as f:
+        f.write(json.dumps(row) + "\n")

@@ -13,7 +13,7 @@ import pytest
 
 from oracle import binding as orc
 from paper_1109_0334_b200 import workloads as wlm
-from parity_helpers import oracle_trace, rel_err
+from parity_helpers import oracle_trace, record_parity, rel_err
 
 pytestmark = pytest.mark.gpu
 
@@ -65,6 +65,7 @@ def _check_bulk_and_outliers(wl, params, trace, z0v0, Jg, Jo, label, max_outlier
     out = np.flatnonzero(e >= TOL_F32)
     assert out.size <= max_outliers, (out.size, e[out])
     M = orc.model_from(wl)
+    moves = []
     for i in out:
         p = params[i:i + 1]
         z = None if z0v0 is None else z0v0[i:i + 1]
@@ -82,6 +83,12 @@ def _check_bulk_and_outliers(wl, params, trace, z0v0, Jg, Jo, label, max_outlier
             moved = max(moved, abs(J2 - J0) / J0)
         print("  outlier %d: err %.2e, oracle moves %.2e under a 1e-10 perturbation"
               % (i, e[i], moved))
+        moves.append(moved)
+    # recorded before asserting: excused by the repository's rule (ILL, TOL/4 at one
+    # FP32 ulp) and by SURVEY.md c-15 as written (the full TOL at one ulp = 4 ILL)
+    record_parity("%s shape, %d particles" % (label, e.size), "f32", e, TOL_F32, out.size,
+                  sum(m > ILL for m in moves), sum(m > 4 * ILL for m in moves))
+    for i, moved in zip(out, moves):
         assert moved > ILL, (int(i), e[i], moved)
     return e
 
