@@ -57,7 +57,7 @@ N_SM, FP64_LANES, FP32_LANES = 148, 64, 128
 # taken from `ncu -i <report> --page raw --csv`, with the hash of the library source
 # the report belongs to) and reported only while the library source is the one that
 # summary was made from; otherwise they are null.
-PROFILE = {"f64": "r2_cfg1_f64", "f32": "r2_cfg1_f32"}
+PROFILE = {"f64": "r3_cfg1_f64", "f32": "r3_cfg1_f32"}
 PIPE_METRIC = {"f64": "sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_",
                "f32": "sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_"}
 
